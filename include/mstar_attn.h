@@ -1,0 +1,156 @@
+/*
+ * mstar_attn.h -- C ABI of the B200 (sm_100a) paged-KV attention library.
+ *
+ * The one data-parallel hot path of the M* serving runtime (arxiv/paper_2606_12688): attention over
+ * a paged KV cache.  PAPER.md:134 (sec. 3.3) -- "KVCacheEngine, a modality-agnostic transformer
+ * engine with FlashInfer-based paged-attention KV-cache state"; PAPER.md:198 -- "three labels over a
+ * single paged KV pool ... each denoise step can then apply paged attention, reading page tables in
+ * place"; PAPER.md:430 (App. I) -- "paged-attention prefill and decode".  The paper gives no formula;
+ * the operations are the textbook ones restated in DESIGN.md section 1 and oracle/mstar_oracle.c.
+ *
+ * Conventions common to every entry point
+ *   - Every pointer named "device" is a CUDA device pointer; plain scalars are host values.
+ *     `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - OWNERSHIP: the library allocates and frees no device memory.  All buffers, including the
+ *     workspace, are the caller's.  Workspace contents need no initialisation and are clobbered.
+ *   - ASYNC: a call only enqueues work on `stream` and never synchronises, so a sequence of calls
+ *     is CUDA-graph capturable (PAPER.md:134, :212 rely on CUDA-graph replay).  All per-sequence
+ *     metadata (block_table, seq_lens, cu_seqlens_q, slot_mapping) is read on the DEVICE; the host
+ *     passes only shape bounds.
+ *   - ERRORS: the return value is an mstar_status.  0 = enqueued.  A negative value means nothing
+ *     was enqueued: NULL/misaligned pointers, unsupported geometry, workspace too small, or a CUDA
+ *     launch error (MSTAR_ERR_CUDA; cudaGetLastError is consumed).  Device-side CONTENT (page ids
+ *     out of range, seq_len beyond the block-table row, duplicate slots) is not validated:
+ *     undefined behaviour.
+ *   - dtype: Q, K, V, out are bf16 (bit patterns; the header has no bf16 type on purpose).
+ *     Accumulation is fp32.  `scale` multiplies q.k before the softmax (natural exponent).
+ *   - GQA: query head h reads KV head h / (num_q_heads / num_kv_heads).
+ *   - Slots of the pool that hold no token (tails of last pages, unreferenced pages) may contain
+ *     anything, including NaN/Inf; results do not depend on them.
+ *   - Results are run-to-run deterministic (no floating-point atomics).
+ */
+#ifndef MSTAR_ATTN_H_
+#define MSTAR_ATTN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    MSTAR_OK = 0,
+    MSTAR_ERR_INVALID_ARG = -1,
+    MSTAR_ERR_UNSUPPORTED = -2,
+    MSTAR_ERR_WORKSPACE_TOO_SMALL = -3,
+    MSTAR_ERR_CUDA = -4
+} mstar_status;
+
+/* flags */
+#define MSTAR_FLAG_OUT_F32 1u /* `out` is fp32 instead of bf16 (diagnostic: separates kernel error from
+                                 output rounding).  Unknown bits => MSTAR_ERR_INVALID_ARG. */
+
+/*
+ * The paged K/V pool ("a single paged KV pool").  Caller-owned device memory, bf16.
+ * Element (page, kv_head, token_in_page, d) of K lives at
+ *     k_pool + page*stride_page + kv_head*stride_head + token_in_page*stride_token + d     (elements)
+ * and likewise for V.  The default "HND" layout [num_pages][Hkv][page_size][D] has
+ * stride_token = D, stride_head = page_size*D, stride_page = Hkv*page_size*D; a token-major "NHD"
+ * pool (stride_head = D, stride_token = Hkv*D) is equally valid.  Strides must be multiples of 8
+ * elements (16 B) and the base pointers 128-B aligned (TMA requirements).
+ * Supported: page_size in {16, 32}; head_dim in {64, 128}; num_pages*Hkv*page_size < 2^31 rows.
+ */
+typedef struct {
+    void* k_pool;
+    void* v_pool;
+    int64_t num_pages;
+    int32_t page_size;
+    int32_t num_kv_heads;
+    int32_t head_dim;
+    int64_t stride_page;
+    int64_t stride_head;
+    int64_t stride_token;
+} mstar_kv_pool;
+
+/*
+ * mstar_kv_append ("reshape_and_cache"; step a1 of DESIGN.md).  Writes the step's new K/V rows into
+ * their pages once, instead of concatenating K/V "at every layer and for every step".
+ *   k_new, v_new   device, [num_tokens][Hkv][D] bf16, contiguous, 16-B aligned
+ *   slot_mapping   device, [num_tokens] int64; slot = page*page_size + token_in_page; slot < 0 = skip
+ * Bit copy; other slots keep their bits.  Two tokens naming the same slot in one call: undefined.
+ */
+int mstar_kv_append(const mstar_kv_pool* pool, const void* k_new, const void* v_new,
+                    const int64_t* slot_mapping, int64_t num_tokens, void* stream);
+
+/*
+ * mstar_paged_attn_decode (steps a2 + a3): one query token per sequence over block-table K/V, as a
+ * split-K ("flash-decoding") pass plus a log-sum-exp combine.
+ *   out            device, [S][Hq][D] bf16 (fp32 with MSTAR_FLAG_OUT_F32)
+ *   lse_out        device, [S][Hq] fp32 natural-log LSE = ln sum_j exp(scale*q.k_j), or NULL
+ *   q              device, [S][Hq][D] bf16 contiguous, 16-B aligned
+ *   block_table    device, [S][block_table_stride] int32; row s lists the physical page of logical
+ *                  page 0,1,...; only the first ceil(seq_lens[s]/page_size) entries are read
+ *   seq_lens       device, [S] int32, KV length of each sequence (0 => out = 0, lse = -inf)
+ *   max_seq_len    host upper bound on seq_lens (sizes the partition grid; may over-estimate)
+ *   num_partitions split-K partitions per sequence; 0 = automatic.  Partition i of a sequence covers
+ *                  tokens [i*c, (i+1)*c) with c = ceil(max_seq_len/num_partitions) rounded up to a
+ *                  multiple of 64; partitions past a sequence's end are empty.  1 = no combine pass.
+ *   workspace      device, >= mstar_paged_attn_decode_workspace_bytes(...) bytes, 16-B aligned
+ * Requires Hq % Hkv == 0 and Hq/Hkv <= 16.
+ */
+size_t mstar_paged_attn_decode_workspace_bytes(int32_t num_seqs, int32_t num_q_heads, int32_t head_dim,
+                                               int32_t max_partitions);
+int mstar_paged_attn_decode(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool,
+                            const int32_t* block_table, int64_t block_table_stride,
+                            const int32_t* seq_lens, int32_t num_seqs, int32_t num_q_heads,
+                            int32_t max_seq_len, float scale, int32_t num_partitions, uint32_t flags,
+                            void* workspace, size_t workspace_bytes, void* stream);
+/* The partition count the automatic choice (num_partitions = 0) would use; for sizing the workspace. */
+int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv_heads,
+                                                int32_t max_seq_len);
+
+/*
+ * mstar_paged_attn_prefill (step a4): many query tokens per sequence, causal over a cached prefix.
+ * Query row i (0-based within sequence s, n_s = cu_seqlens_q[s+1]-cu_seqlens_q[s] rows) attends to
+ * KV positions j <= (seq_lens[s] - n_s) + i when causal != 0 (bottom-right aligned mask), to all
+ * seq_lens[s] positions when causal == 0.  The new tokens' K/V are read from the pool: call
+ * mstar_kv_append first (same stream).
+ *   out            device, [total_q][Hq][D] bf16 (fp32 with MSTAR_FLAG_OUT_F32)
+ *   lse_out        device, [total_q][Hq] fp32 or NULL
+ *   q              device, [total_q][Hq][D] bf16 contiguous, ragged by cu_seqlens_q
+ *   cu_seqlens_q   device, [S+1] int32, cu_seqlens_q[0] = 0, cu_seqlens_q[S] = total_q
+ *   seq_lens       device, [S] int32, total KV length INCLUDING the new tokens (>= n_s)
+ *   max_q_len, max_seq_len   host upper bounds on n_s and seq_lens
+ */
+size_t mstar_paged_attn_prefill_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads,
+                                                int32_t head_dim);
+int mstar_paged_attn_prefill(void* out, float* lse_out, const void* q, const int32_t* cu_seqlens_q,
+                             const mstar_kv_pool* pool, const int32_t* block_table,
+                             int64_t block_table_stride, const int32_t* seq_lens, int32_t num_seqs,
+                             int32_t total_q, int32_t max_q_len, int32_t max_seq_len,
+                             int32_t num_q_heads, float scale, int32_t causal, uint32_t flags,
+                             void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * mstar_build_slot_mapping: device-side helper so that append -> prefill stays graph-capturable.
+ * slot_mapping_out[cu_seqlens_q[s] + i] = block_table[s][j / page_size]*page_size + j % page_size
+ * with j = seq_lens[s] - n_s + i.   slot_mapping_out: device, [total_q] int64.
+ */
+int mstar_build_slot_mapping(const int32_t* block_table, int64_t block_table_stride,
+                             const int32_t* cu_seqlens_q, const int32_t* seq_lens, int32_t num_seqs,
+                             int32_t total_q, int32_t page_size, int64_t* slot_mapping_out, void* stream);
+
+/* Number of kernels the last call on this thread enqueued (bench.py's gpu_launches claim). */
+int32_t mstar_last_launch_count(void);
+
+/* Human-readable name of a status code (static storage). */
+const char* mstar_status_string(int status);
+
+/* Library version, "major.minor.patch" (static storage). */
+const char* mstar_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MSTAR_ATTN_H_ */

@@ -1,0 +1,30 @@
+"""B200 (sm_100a) paged-KV attention: the hot path of the M* serving runtime (arxiv/paper_2606_12688).
+
+The product is the C-ABI library ``libmstar_attn.so`` (``include/mstar_attn.h``); this package is its thin
+Python binding.  Names mirror the C entry points:
+
+    kv_append            <- mstar_kv_append
+    paged_attn_decode    <- mstar_paged_attn_decode   (split-K + LSE combine)
+    paged_attn_prefill   <- mstar_paged_attn_prefill  (causal over a cached prefix)
+    build_slot_mapping   <- mstar_build_slot_mapping
+
+There is no CPU fallback: without the built library every call raises ``MstarError``.
+"""
+from .binding import (  # noqa: F401
+    EXPORTS,
+    KVPool,
+    LIB_PATH,
+    MSTAR_FLAG_OUT_F32,
+    MstarError,
+    build_slot_mapping,
+    decode_auto_partitions,
+    decode_workspace_bytes,
+    kv_append,
+    last_launch_count,
+    load_library,
+    paged_attn_decode,
+    paged_attn_prefill,
+    prefill_workspace_bytes,
+    status_string,
+    version,
+)

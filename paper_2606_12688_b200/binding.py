@@ -1,0 +1,235 @@
+"""Thin ctypes binding of ``include/mstar_attn.h``: argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``libmstar_attn.so``; there is no CPU or PyTorch
+fallback -- if the library is missing or a call fails this module raises.  PyTorch provides device
+memory and streams only: tensors cross the boundary as raw device pointers, the stream as
+``torch.cuda.current_stream().cuda_stream``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import torch
+
+_PKG_DIR = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG_DIR, "libmstar_attn.so")
+
+MSTAR_OK = 0
+MSTAR_FLAG_OUT_F32 = 1
+
+EXPORTS = (
+    "mstar_kv_append",
+    "mstar_paged_attn_decode_workspace_bytes",
+    "mstar_paged_attn_decode",
+    "mstar_paged_attn_decode_auto_partitions",
+    "mstar_paged_attn_prefill_workspace_bytes",
+    "mstar_paged_attn_prefill",
+    "mstar_build_slot_mapping",
+    "mstar_last_launch_count",
+    "mstar_status_string",
+    "mstar_version",
+)
+
+
+class MstarError(RuntimeError):
+    pass
+
+
+class _KvPoolStruct(ctypes.Structure):
+    _fields_ = [
+        ("k_pool", ctypes.c_void_p),
+        ("v_pool", ctypes.c_void_p),
+        ("num_pages", ctypes.c_int64),
+        ("page_size", ctypes.c_int32),
+        ("num_kv_heads", ctypes.c_int32),
+        ("head_dim", ctypes.c_int32),
+        ("stride_page", ctypes.c_int64),
+        ("stride_head", ctypes.c_int64),
+        ("stride_token", ctypes.c_int64),
+    ]
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """Load the C-ABI library (built in-tree by ``paper_2606_12688_b200.build``).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise MstarError(
+            "%s not found: build it with `python -m paper_2606_12688_b200.build` "
+            "(there is no CPU fallback)" % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    c = ctypes
+    lib.mstar_kv_append.restype = c.c_int
+    lib.mstar_kv_append.argtypes = [c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p, c.c_void_p, c.c_int64,
+                                    c.c_void_p]
+    lib.mstar_paged_attn_decode_workspace_bytes.restype = c.c_size_t
+    lib.mstar_paged_attn_decode_workspace_bytes.argtypes = [c.c_int32] * 4
+    lib.mstar_paged_attn_decode_auto_partitions.restype = c.c_int32
+    lib.mstar_paged_attn_decode_auto_partitions.argtypes = [c.c_int32] * 3
+    lib.mstar_paged_attn_decode.restype = c.c_int
+    lib.mstar_paged_attn_decode.argtypes = [
+        c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_int64, c.c_void_p,
+        c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_uint32, c.c_void_p, c.c_size_t, c.c_void_p]
+    lib.mstar_paged_attn_prefill_workspace_bytes.restype = c.c_size_t
+    lib.mstar_paged_attn_prefill_workspace_bytes.argtypes = [c.c_int32] * 4
+    lib.mstar_paged_attn_prefill.restype = c.c_int
+    lib.mstar_paged_attn_prefill.argtypes = [
+        c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_int64,
+        c.c_void_p, c.c_int32, c.c_int32, c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_uint32,
+        c.c_void_p, c.c_size_t, c.c_void_p]
+    lib.mstar_build_slot_mapping.restype = c.c_int
+    lib.mstar_build_slot_mapping.argtypes = [c.c_void_p, c.c_int64, c.c_void_p, c.c_void_p, c.c_int32, c.c_int32,
+                                             c.c_int32, c.c_void_p, c.c_void_p]
+    lib.mstar_last_launch_count.restype = c.c_int32
+    lib.mstar_last_launch_count.argtypes = []
+    lib.mstar_status_string.restype = c.c_char_p
+    lib.mstar_status_string.argtypes = [c.c_int]
+    lib.mstar_version.restype = c.c_char_p
+    lib.mstar_version.argtypes = []
+    _lib = lib
+    return lib
+
+
+def status_string(status: int) -> str:
+    return load_library().mstar_status_string(int(status)).decode()
+
+
+def version() -> str:
+    return load_library().mstar_version().decode()
+
+
+def last_launch_count() -> int:
+    return int(load_library().mstar_last_launch_count())
+
+
+def _check(status: int, what: str) -> None:
+    if status != MSTAR_OK:
+        raise MstarError("%s failed: %s (%d)" % (what, status_string(status), status))
+
+
+def _stream() -> ctypes.c_void_p:
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t: Optional[torch.Tensor]) -> ctypes.c_void_p:
+    return ctypes.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _want(t: torch.Tensor, dtype, name: str) -> None:
+    if not t.is_cuda:
+        raise MstarError("%s must be a CUDA tensor (the C ABI takes device pointers)" % name)
+    if t.dtype != dtype:
+        raise MstarError("%s must be %s, got %s" % (name, dtype, t.dtype))
+    if not t.is_contiguous():
+        raise MstarError("%s must be contiguous" % name)
+
+
+class KVPool:
+    """The paged K/V pool: two bf16 tensors viewed as [num_pages, Hkv, page_size, D] (any strides whose
+    innermost is 1).  Holds references to the tensors; owns nothing else."""
+
+    def __init__(self, k_pool: torch.Tensor, v_pool: torch.Tensor):
+        for t, nm in ((k_pool, "k_pool"), (v_pool, "v_pool")):
+            if not t.is_cuda or t.dtype != torch.bfloat16 or t.dim() != 4 or t.stride(3) != 1:
+                raise MstarError("%s must be a CUDA bf16 tensor [num_pages, Hkv, page_size, D] with unit inner stride" % nm)
+        if k_pool.shape != v_pool.shape or k_pool.stride() != v_pool.stride():
+            raise MstarError("k_pool and v_pool must share shape and strides")
+        self.k_pool, self.v_pool = k_pool, v_pool
+        self.num_pages, self.num_kv_heads, self.page_size, self.head_dim = (int(x) for x in k_pool.shape)
+        self.c = _KvPoolStruct(
+            k_pool.data_ptr(), v_pool.data_ptr(), self.num_pages, self.page_size, self.num_kv_heads,
+            self.head_dim, int(k_pool.stride(0)), int(k_pool.stride(1)), int(k_pool.stride(2)))
+
+
+def kv_append(pool: KVPool, k_new: torch.Tensor, v_new: torch.Tensor, slot_mapping: torch.Tensor) -> None:
+    """mstar_kv_append: scatter k_new/v_new [T,Hkv,D] bf16 into the pool at slot_mapping [T] int64."""
+    _want(k_new, torch.bfloat16, "k_new"); _want(v_new, torch.bfloat16, "v_new")
+    _want(slot_mapping, torch.int64, "slot_mapping")
+    T = int(slot_mapping.shape[0])
+    if tuple(k_new.shape) != (T, pool.num_kv_heads, pool.head_dim) or k_new.shape != v_new.shape:
+        raise MstarError("k_new/v_new must be [T, Hkv, D]")
+    lib = load_library()
+    _check(lib.mstar_kv_append(ctypes.byref(pool.c), _ptr(k_new), _ptr(v_new), _ptr(slot_mapping), T, _stream()),
+           "mstar_kv_append")
+
+
+def decode_auto_partitions(num_seqs: int, num_kv_heads: int, max_seq_len: int) -> int:
+    return int(load_library().mstar_paged_attn_decode_auto_partitions(num_seqs, num_kv_heads, max_seq_len))
+
+
+def decode_workspace_bytes(num_seqs: int, num_q_heads: int, head_dim: int, max_partitions: int) -> int:
+    return int(load_library().mstar_paged_attn_decode_workspace_bytes(num_seqs, num_q_heads, head_dim,
+                                                                       max_partitions))
+
+
+def paged_attn_decode(out: torch.Tensor, q: torch.Tensor, pool: KVPool, block_table: torch.Tensor,
+                      seq_lens: torch.Tensor, max_seq_len: int, scale: float, num_partitions: int = 0,
+                      workspace: Optional[torch.Tensor] = None, lse_out: Optional[torch.Tensor] = None) -> None:
+    """mstar_paged_attn_decode.  out [S,Hq,D] bf16 or fp32 (fp32 selects MSTAR_FLAG_OUT_F32)."""
+    _want(q, torch.bfloat16, "q"); _want(block_table, torch.int32, "block_table")
+    _want(seq_lens, torch.int32, "seq_lens")
+    S, Hq, D = (int(x) for x in q.shape)
+    flags = 0
+    if out.dtype == torch.float32:
+        flags |= MSTAR_FLAG_OUT_F32
+    elif out.dtype != torch.bfloat16:
+        raise MstarError("out must be bf16 or fp32")
+    if not out.is_cuda or not out.is_contiguous() or tuple(out.shape) != (S, Hq, D):
+        raise MstarError("out must be a contiguous CUDA tensor [S, Hq, D]")
+    if lse_out is not None:
+        _want(lse_out, torch.float32, "lse_out")
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    lib = load_library()
+    _check(lib.mstar_paged_attn_decode(
+        _ptr(out), _ptr(lse_out), _ptr(q), ctypes.byref(pool.c), _ptr(block_table),
+        int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens), S, Hq, int(max_seq_len),
+        float(scale), int(num_partitions), flags, _ptr(workspace), ws_bytes, _stream()), "mstar_paged_attn_decode")
+
+
+def prefill_workspace_bytes(num_seqs: int, total_q: int, num_q_heads: int, head_dim: int) -> int:
+    return int(load_library().mstar_paged_attn_prefill_workspace_bytes(num_seqs, total_q, num_q_heads, head_dim))
+
+
+def paged_attn_prefill(out: torch.Tensor, q: torch.Tensor, cu_seqlens_q: torch.Tensor, pool: KVPool,
+                       block_table: torch.Tensor, seq_lens: torch.Tensor, max_q_len: int, max_seq_len: int,
+                       scale: float, causal: bool = True, workspace: Optional[torch.Tensor] = None,
+                       lse_out: Optional[torch.Tensor] = None) -> None:
+    """mstar_paged_attn_prefill.  q/out [T,Hq,D]; K/V of the new tokens must already be in the pool."""
+    _want(q, torch.bfloat16, "q"); _want(cu_seqlens_q, torch.int32, "cu_seqlens_q")
+    _want(block_table, torch.int32, "block_table"); _want(seq_lens, torch.int32, "seq_lens")
+    T, Hq, D = (int(x) for x in q.shape)
+    S = int(cu_seqlens_q.shape[0]) - 1
+    flags = 0
+    if out.dtype == torch.float32:
+        flags |= MSTAR_FLAG_OUT_F32
+    elif out.dtype != torch.bfloat16:
+        raise MstarError("out must be bf16 or fp32")
+    if not out.is_cuda or not out.is_contiguous() or tuple(out.shape) != (T, Hq, D):
+        raise MstarError("out must be a contiguous CUDA tensor [T, Hq, D]")
+    if lse_out is not None:
+        _want(lse_out, torch.float32, "lse_out")
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    lib = load_library()
+    _check(lib.mstar_paged_attn_prefill(
+        _ptr(out), _ptr(lse_out), _ptr(q), _ptr(cu_seqlens_q), ctypes.byref(pool.c), _ptr(block_table),
+        int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens), S, T, int(max_q_len),
+        int(max_seq_len), Hq, float(scale), 1 if causal else 0, flags, _ptr(workspace), ws_bytes, _stream()),
+        "mstar_paged_attn_prefill")
+
+
+def build_slot_mapping(block_table: torch.Tensor, cu_seqlens_q: torch.Tensor, seq_lens: torch.Tensor,
+                       total_q: int, page_size: int, slot_mapping_out: torch.Tensor) -> None:
+    """mstar_build_slot_mapping: device-side slot mapping of the step's new tokens."""
+    _want(block_table, torch.int32, "block_table"); _want(cu_seqlens_q, torch.int32, "cu_seqlens_q")
+    _want(seq_lens, torch.int32, "seq_lens"); _want(slot_mapping_out, torch.int64, "slot_mapping_out")
+    S = int(seq_lens.shape[0])
+    lib = load_library()
+    _check(lib.mstar_build_slot_mapping(_ptr(block_table), int(block_table.stride(0)), _ptr(cu_seqlens_q),
+                                        _ptr(seq_lens), S, int(total_q), int(page_size), _ptr(slot_mapping_out),
+                                        _stream()), "mstar_build_slot_mapping")

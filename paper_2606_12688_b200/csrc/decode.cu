@@ -1,0 +1,612 @@
+// decode.cu -- steps a2 + a3: split-K ("flash-decoding") paged decode attention and its LSE combine.
+//
+// Design.  The path is an HBM stream: every K/V byte of every sequence is read
+// exactly once, 4*G*D flops per 2*D*2 bytes.  One persistent CTA per SM; work items are
+// (sequence, split-K partition, kv head).  Inside a CTA
+//   * one PRODUCER warp walks the block table and issues TMA tensor copies (cp.async.bulk.tensor,
+//     128-B swizzle) of whole (page, kv head) slabs into a deep shared-memory ring of 64-token stages,
+//     running ahead across work items so the stream never drains between items;
+//   * four CONSUMER warps each own 16 tokens of every stage: S = Q K^T with warp-level bf16 MMA
+//     (the G grouped query heads padded into the 16 MMA rows; the tensor pipe is otherwise idle),
+//     online softmax in fp32 with warp-shuffle max / sum reductions, O += P V with MMA;
+//   * at the end of an item the four warps merge their (m, l, O) through shared memory and write one
+//     fp32 partial; the combine kernel merges partitions by log-sum-exp and rounds to bf16 once.
+// Full/empty mbarriers per stage are the only synchronisation in the steady state.
+#include <cuda_bf16.h>
+
+#include "host_common.h"
+#include "ptx.cuh"
+
+namespace mstar {
+
+constexpr int kDecodeConsumerWarps = 4;
+constexpr int kDecodeTok = 16 * kDecodeConsumerWarps;  // tokens per ring stage
+constexpr int kDecodeThreads = 32 * (kDecodeConsumerWarps + 1);
+constexpr int kMaxStages = 16;
+
+struct DecodeParams {
+    const uint16_t* q;
+    const int32_t* block_table;
+    int64_t bt_stride;
+    const int32_t* seq_lens;
+    int32_t S, Hq, Hkv, G;
+    int32_t chunk;   // tokens per partition, multiple of kDecodeTok
+    int32_t nparts;  // partition slots per (sequence, head) in the workspace
+    float scale_log2;
+    float* part_O;  // [S*Hq][nparts][D]
+    float* part_m;  // [S*Hq][nparts]   (log2 domain: max of scale*log2e*q.k)
+    float* part_l;  // [S*Hq][nparts]
+    void* out;
+    float* lse;
+    int32_t out_f32;
+    int32_t direct;  // nparts == 1: write the final output, no combine pass
+    int32_t nstages;
+};
+
+struct ItemInfo {
+    int32_t s, kvh, part, tok0, ntok;
+};
+
+template <int D, int GH>
+struct DecodeSmem {
+    static constexpr int kStageBytes = 2 * kDecodeTok * D * 2;
+    static constexpr int kQBytes = GH * D * 2;
+    static constexpr int kMergeBytes = kDecodeConsumerWarps * GH * (D + 2) * 4;
+    // fixed part after the ring: Q slots, merge buffer, barriers, item info
+    static constexpr int kFixed = 2 * kQBytes + kMergeBytes + (2 * kMaxStages + 4) * 8 + 2 * 32;
+    static size_t bytes(int nstages, int S) {
+        return 1024 + (size_t)nstages * kStageBytes + kFixed + (size_t)(S + 1) * 4 + 16;
+    }
+};
+
+__device__ __forceinline__ void store_out_vec(void* out, int out_f32, size_t idx, const float* v, int n) {
+    if (out_f32) {
+        float* o = reinterpret_cast<float*>(out) + idx;
+        for (int i = 0; i < n; ++i) o[i] = v[i];
+    } else {
+        __nv_bfloat16* o = reinterpret_cast<__nv_bfloat16*>(out) + idx;
+        for (int i = 0; i < n; i += 2) {
+            *reinterpret_cast<uint32_t*>(o + i) = pack_bf16x2(v[i], v[i + 1]);
+        }
+    }
+}
+
+template <int D, int PAGE, int GH>
+__global__ void __launch_bounds__(kDecodeThreads, 1)
+decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_constant__ CUtensorMap vmap,
+                     const DecodeParams p) {
+    constexpr int NW = kDecodeConsumerWarps;
+    constexpr int TOK = kDecodeTok;
+    constexpr int PPS = TOK / PAGE;  // pages per stage
+    constexpr int NH = D / 64;       // 64-column halves per row
+    constexpr int HT = TOK * 128;    // bytes of one half tile (TOK rows x 128 B)
+    constexpr int KBYTES = NH * HT;  // K part of a stage
+    using SM = DecodeSmem<D, GH>;
+    constexpr int VEC = D / 32;
+
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t* gbase = smem_raw + (base - smem_u32(smem_raw));
+    const int nstages = p.nstages;
+    const uint32_t ring = base;
+    const uint32_t qbuf = ring + nstages * SM::kStageBytes;
+    uint8_t* g_after = gbase + (size_t)nstages * SM::kStageBytes;
+    uint16_t* qbuf_g = reinterpret_cast<uint16_t*>(g_after);
+    float* merge_O = reinterpret_cast<float*>(g_after + 2 * SM::kQBytes);        // [NW][GH][D]
+    float* merge_m = merge_O + NW * GH * D;                                      // [NW][GH]
+    float* merge_l = merge_m + NW * GH;                                          // [NW][GH]
+    uint64_t* bars_g = reinterpret_cast<uint64_t*>(g_after + 2 * SM::kQBytes + SM::kMergeBytes);
+    const uint32_t bars = smem_u32(bars_g);
+    ItemInfo* info = reinterpret_cast<ItemInfo*>(bars_g + 2 * kMaxStages + 4);
+    int32_t* cum = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(info) + 2 * 32);
+    auto full_bar = [&](int st) { return bars + 8u * st; };
+    auto empty_bar = [&](int st) { return bars + 8u * (kMaxStages + st); };
+    auto qfull_bar = [&](int qs) { return bars + 8u * (2 * kMaxStages + qs); };
+    auto qempty_bar = [&](int qs) { return bars + 8u * (2 * kMaxStages + 2 + qs); };
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < nstages; ++i) {
+            mbar_init(full_bar(i), 1);
+            mbar_init(empty_bar(i), NW);
+        }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(qfull_bar(i), 1);
+            mbar_init(qempty_bar(i), NW);
+        }
+        fence_mbar_init();
+    }
+    // zero the Q slots once: rows >= G are MMA padding and must stay 0 (bulk copies only write rows < G)
+    for (int i = threadIdx.x; i < 2 * SM::kQBytes / 4; i += blockDim.x) reinterpret_cast<uint32_t*>(qbuf_g)[i] = 0u;
+    fence_proxy_async_smem();
+    __syncthreads();
+
+    if (warp == NW) {
+        // =============================== PRODUCER ===============================
+        prefetch_tensormap(&kmap);
+        prefetch_tensormap(&vmap);
+        // exclusive prefix sum of per-sequence partition counts -> compact work list
+        int carry = 0;
+        for (int s0 = 0; s0 < p.S; s0 += 32) {
+            const int s = s0 + lane;
+            const int n = (s < p.S) ? (p.seq_lens[s] + p.chunk - 1) / p.chunk : 0;
+            int incl = n;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += t;
+            }
+            if (s < p.S) cum[s] = carry + incl - n;
+            carry += __shfl_sync(0xffffffffu, incl, 31);
+        }
+        if (lane == 0) cum[p.S] = carry;
+        __syncwarp();
+        const int n_items = carry * p.Hkv;
+        const uint64_t pol = policy_evict_first();
+
+        // this lane's TMA op within a stage: (page i, K or V, 64-column half)
+        constexpr int OPS = PPS * 2 * NH;
+        const int op_page = lane / (2 * NH);
+        const int op_isv = (lane % (2 * NH)) / NH;
+        const int op_half = lane % NH;
+        const uint32_t op_off = op_isv * KBYTES + op_half * HT + op_page * (PAGE * 128);
+
+        int st = 0, ph = 0, qs = 0, qph = 0;
+        for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+            const int pi = item / p.Hkv, kvh = item - pi * p.Hkv;
+            int lo = 0, hi = p.S;  // cum[lo] <= pi < cum[hi]
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if (cum[mid] <= pi) lo = mid; else hi = mid;
+            }
+            const int s = lo, part = pi - cum[lo];
+            const int L = p.seq_lens[s];
+            const int tok0 = part * p.chunk;
+            const int ntok = min(L - tok0, p.chunk);
+            const int ntiles = (ntok + TOK - 1) / TOK;
+
+            mbar_wait(qempty_bar(qs), qph ^ 1);
+            if (lane == 0) {
+                info[qs] = ItemInfo{s, kvh, part, tok0, ntok};
+                mbar_arrive_expect_tx(qfull_bar(qs), (uint32_t)(p.G * D * 2));
+                bulk_load_1d(qbuf + qs * SM::kQBytes, p.q + ((size_t)s * p.Hq + (size_t)kvh * p.G) * D,
+                             (uint32_t)(p.G * D * 2), qfull_bar(qs));
+            }
+            qs ^= 1;
+            if (qs == 0) qph ^= 1;
+
+            const int32_t* bt = p.block_table + (size_t)s * p.bt_stride + tok0 / PAGE;
+            int pg_next = -1;
+            {
+                const int npg0 = min(PPS, (ntok + PAGE - 1) / PAGE);
+                if (lane < OPS && op_page < npg0) pg_next = __ldg(bt + op_page);
+            }
+            for (int t = 0; t < ntiles; ++t) {
+                const int rem = ntok - t * TOK;
+                const int npg = min(PPS, (rem + PAGE - 1) / PAGE);
+                const int pg = pg_next;
+                pg_next = -1;
+                if (t + 1 < ntiles) {  // prefetch the next stage's page ids ahead of the ring wait
+                    const int npg1 = min(PPS, (rem - TOK + PAGE - 1) / PAGE);
+                    if (lane < OPS && op_page < npg1) pg_next = __ldg(bt + (t + 1) * PPS + op_page);
+                }
+                mbar_wait(empty_bar(st), ph ^ 1);
+                if (lane == 0) mbar_arrive_expect_tx(full_bar(st), (uint32_t)(npg * PAGE * D * 2 * 2));
+                __syncwarp();
+                if (pg >= 0)
+                    tma_load_4d(ring + st * SM::kStageBytes + op_off, op_isv ? &vmap : &kmap, full_bar(st),
+                                op_half * 64, 0, kvh, pg, pol);
+                if (++st == nstages) { st = 0; ph ^= 1; }
+            }
+        }
+        // sentinel: tell the consumers to stop
+        mbar_wait(qempty_bar(qs), qph ^ 1);
+        if (lane == 0) {
+            info[qs].ntok = -1;
+            mbar_arrive(qfull_bar(qs));
+        }
+    } else {
+        // =============================== CONSUMERS ===============================
+        const int w = warp;
+        const int g = lane >> 2, t4 = lane & 3;
+        if (p.direct) {  // empty sequences get out = 0, lse = -inf (no work item ever touches them)
+            for (int s = blockIdx.x * NW + w; s < p.S; s += gridDim.x * NW) {
+                if (p.seq_lens[s] != 0) continue;
+                for (int i = lane; i < p.Hq * D; i += 32) {
+                    const size_t idx = (size_t)s * p.Hq * D + i;
+                    if (p.out_f32) reinterpret_cast<float*>(p.out)[idx] = 0.f;
+                    else reinterpret_cast<uint16_t*>(p.out)[idx] = 0;
+                }
+                if (p.lse) for (int h = lane; h < p.Hq; h += 32) p.lse[(size_t)s * p.Hq + h] = -INFINITY;
+            }
+        }
+        // ldmatrix source rows / chunk selectors of this lane (see DESIGN.md 4.2 for the fragment maps)
+        const uint32_t k_row = w * 16 + (lane >> 4) * 8 + (lane & 7);
+        const uint32_t k_csel = (lane >> 3) & 1;
+        const uint32_t v_row = w * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
+        const uint32_t v_csel = lane >> 4;
+
+        int st = 0, ph = 0, qs = 0, qph = 0;
+        while (true) {
+            mbar_wait(qfull_bar(qs), qph);
+            const ItemInfo it = info[qs];
+            if (it.ntok < 0) break;
+            // Q fragments (A operand), rows = grouped query heads
+            uint32_t qa[D / 16][4];
+            {
+                const uint16_t* qb = qbuf_g + qs * (SM::kQBytes / 2);
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    qa[ks][0] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + 2 * t4);
+                    qa[ks][2] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + 8 + 2 * t4);
+                    if (GH == 16) {
+                        qa[ks][1] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + 2 * t4);
+                        qa[ks][3] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + 8 + 2 * t4);
+                    } else {
+                        qa[ks][1] = 0u;
+                        qa[ks][3] = 0u;
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(qempty_bar(qs));
+            qs ^= 1;
+            if (qs == 0) qph ^= 1;
+
+            float o[D / 8][4];
+#pragma unroll
+            for (int j = 0; j < D / 8; ++j) o[j][0] = o[j][1] = o[j][2] = o[j][3] = 0.f;
+            float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;  // rows g and g+8 (raw q.k units)
+
+            const int ntiles = (it.ntok + TOK - 1) / TOK;
+            for (int t = 0; t < ntiles; ++t) {
+                mbar_wait(full_bar(st), ph);
+                const int nv = min(16, it.ntok - t * TOK - w * 16);  // valid tokens in this warp's slice
+                if (nv > 0) {
+                    const uint32_t kb = ring + st * SM::kStageBytes;
+                    const uint32_t vb = kb + KBYTES;
+                    // ---- S = Q K^T for 16 tokens (two n-blocks of 8)
+                    float sc[2][4];
+#pragma unroll
+                    for (int b = 0; b < 2; ++b) sc[b][0] = sc[b][1] = sc[b][2] = sc[b][3] = 0.f;
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        const uint32_t chunk = 2 * ks + k_csel;
+                        uint32_t b0, b1, b2, b3;
+                        ldsm_x4(kb + (chunk >> 3) * HT + swz128(k_row, chunk & 7), b0, b1, b2, b3);
+                        mma_bf16_16816(sc[0], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b0, b1);
+                        mma_bf16_16816(sc[1], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b2, b3);
+                    }
+                    // ---- mask the ragged tail (slots >= seq_len may hold anything, incl. NaN)
+                    uint32_t vmask_lo = 0xffffffffu, vmask_hi = 0xffffffffu;
+                    if (nv < 16) {
+#pragma unroll
+                        for (int b = 0; b < 2; ++b) {
+                            const int c = b * 8 + 2 * t4;
+                            if (c >= nv) sc[b][0] = sc[b][2] = -INFINITY;
+                            if (c + 1 >= nv) sc[b][1] = sc[b][3] = -INFINITY;
+                        }
+                        vmask_lo = (2 * t4 < nv ? 0x0000ffffu : 0u) | (2 * t4 + 1 < nv ? 0xffff0000u : 0u);
+                        vmask_hi = (8 + 2 * t4 < nv ? 0x0000ffffu : 0u) | (8 + 2 * t4 + 1 < nv ? 0xffff0000u : 0u);
+                    }
+                    // ---- online softmax (fp32), row max over the quad by shuffles
+                    float mx0 = fmaxf(fmaxf(sc[0][0], sc[0][1]), fmaxf(sc[1][0], sc[1][1]));
+                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+                    const float mn0 = fmaxf(m0, mx0);
+                    const float a0 = fast_exp2((m0 - mn0) * p.scale_log2);
+                    const float ms0 = mn0 * p.scale_log2;
+                    m0 = mn0;
+                    const float p00 = fast_exp2(sc[0][0] * p.scale_log2 - ms0);
+                    const float p01 = fast_exp2(sc[0][1] * p.scale_log2 - ms0);
+                    const float p10 = fast_exp2(sc[1][0] * p.scale_log2 - ms0);
+                    const float p11 = fast_exp2(sc[1][1] * p.scale_log2 - ms0);
+                    l0 = l0 * a0 + (p00 + p01) + (p10 + p11);
+                    uint32_t pa[4];
+                    pa[0] = pack_bf16x2(p00, p01);
+                    pa[2] = pack_bf16x2(p10, p11);
+                    pa[1] = 0u;
+                    pa[3] = 0u;
+                    float a1 = 1.f;
+                    if (GH == 16) {
+                        float mx1 = fmaxf(fmaxf(sc[0][2], sc[0][3]), fmaxf(sc[1][2], sc[1][3]));
+                        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+                        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+                        const float mn1 = fmaxf(m1, mx1);
+                        a1 = fast_exp2((m1 - mn1) * p.scale_log2);
+                        const float ms1 = mn1 * p.scale_log2;
+                        m1 = mn1;
+                        const float q00 = fast_exp2(sc[0][2] * p.scale_log2 - ms1);
+                        const float q01 = fast_exp2(sc[0][3] * p.scale_log2 - ms1);
+                        const float q10 = fast_exp2(sc[1][2] * p.scale_log2 - ms1);
+                        const float q11 = fast_exp2(sc[1][3] * p.scale_log2 - ms1);
+                        l1 = l1 * a1 + (q00 + q01) + (q10 + q11);
+                        pa[1] = pack_bf16x2(q00, q01);
+                        pa[3] = pack_bf16x2(q10, q11);
+                    }
+                    // ---- O = O * alpha + P V
+#pragma unroll
+                    for (int jj = 0; jj < D / 16; ++jj) {
+                        const uint32_t chunk = 2 * jj + v_csel;
+                        uint32_t b0, b1, b2, b3;
+                        ldsm_x4_trans(vb + (chunk >> 3) * HT + swz128(v_row, chunk & 7), b0, b1, b2, b3);
+                        if (nv < 16) {  // 0 * NaN guard: zero V rows that hold no token
+                            b0 &= vmask_lo; b1 &= vmask_hi; b2 &= vmask_lo; b3 &= vmask_hi;
+                        }
+                        o[2 * jj][0] *= a0; o[2 * jj][1] *= a0; o[2 * jj + 1][0] *= a0; o[2 * jj + 1][1] *= a0;
+                        if (GH == 16) {
+                            o[2 * jj][2] *= a1; o[2 * jj][3] *= a1; o[2 * jj + 1][2] *= a1; o[2 * jj + 1][3] *= a1;
+                        }
+                        mma_bf16_16816(o[2 * jj], pa[0], pa[1], pa[2], pa[3], b0, b1);
+                        mma_bf16_16816(o[2 * jj + 1], pa[0], pa[1], pa[2], pa[3], b2, b3);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty_bar(st));
+                if (++st == nstages) { st = 0; ph ^= 1; }
+            }
+
+            // ---- merge the four warps' (m, l, O) through shared memory
+            l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
+            l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+            if (GH == 16) {
+                l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
+                l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+            }
+            {
+                float* mo = merge_O + (size_t)w * GH * D;
+#pragma unroll
+                for (int j = 0; j < D / 8; ++j) {
+                    *reinterpret_cast<float2*>(mo + g * D + j * 8 + 2 * t4) = make_float2(o[j][0], o[j][1]);
+                    if (GH == 16)
+                        *reinterpret_cast<float2*>(mo + (g + 8) * D + j * 8 + 2 * t4) = make_float2(o[j][2], o[j][3]);
+                }
+                if (t4 == 0) {
+                    merge_m[w * GH + g] = m0 * p.scale_log2;
+                    merge_l[w * GH + g] = l0;
+                    if (GH == 16) {
+                        merge_m[w * GH + g + 8] = m1 * p.scale_log2;
+                        merge_l[w * GH + g + 8] = l1;
+                    }
+                }
+            }
+            named_bar_sync(1, NW * 32);
+            for (int r = w; r < p.G; r += NW) {
+                float M = -INFINITY;
+#pragma unroll
+                for (int x = 0; x < NW; ++x) M = fmaxf(M, merge_m[x * GH + r]);
+                float acc[VEC];
+#pragma unroll
+                for (int i = 0; i < VEC; ++i) acc[i] = 0.f;
+                float lsum = 0.f;
+#pragma unroll
+                for (int x = 0; x < NW; ++x) {
+                    const float mx = merge_m[x * GH + r];
+                    const float a = (mx == -INFINITY) ? 0.f : fast_exp2(mx - M);
+                    lsum += a * merge_l[x * GH + r];
+                    const float* src = merge_O + ((size_t)x * GH + r) * D + lane * VEC;
+#pragma unroll
+                    for (int i = 0; i < VEC; ++i) acc[i] += a * src[i];
+                }
+                const size_t row = (size_t)it.s * p.Hq + (size_t)it.kvh * p.G + r;
+                if (p.direct) {
+                    const float inv = 1.f / lsum;
+#pragma unroll
+                    for (int i = 0; i < VEC; ++i) acc[i] *= inv;
+                    store_out_vec(p.out, p.out_f32, row * D + lane * VEC, acc, VEC);
+                    if (p.lse && lane == 0) p.lse[row] = (M + log2f(lsum)) * 0.6931471805599453f;
+                } else {
+                    float* dst = p.part_O + (row * p.nparts + it.part) * D + lane * VEC;
+#pragma unroll
+                    for (int i = 0; i < VEC; ++i) dst[i] = acc[i];
+                    if (lane == 0) {
+                        p.part_m[row * p.nparts + it.part] = M;
+                        p.part_l[row * p.nparts + it.part] = lsum;
+                    }
+                }
+            }
+            named_bar_sync(1, NW * 32);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// step a3: merge the partitions of every (sequence, head) row by log-sum-exp, normalise, round once.
+// One warp per row; lanes own D/32 consecutive output elements.  Partition count per sequence is
+// ceil(seq_len / chunk): the same arithmetic the split-K kernel used.
+template <int D>
+__global__ void __launch_bounds__(128) decode_combine_kernel(const float* __restrict__ part_O,
+                                                             const float* __restrict__ part_m,
+                                                             const float* __restrict__ part_l,
+                                                             const int32_t* __restrict__ seq_lens, int32_t chunk,
+                                                             int32_t nparts, int32_t Hq, int32_t n_rows,
+                                                             void* __restrict__ out, float* __restrict__ lse,
+                                                             int32_t out_f32) {
+    constexpr int VEC = D / 32;
+    const int lane = threadIdx.x & 31;
+    const int row = blockIdx.x * 4 + (threadIdx.x >> 5);
+    if (row >= n_rows) return;
+    const int s = row / Hq;
+    const int L = seq_lens[s];
+    const int np = (L + chunk - 1) / chunk;
+    float acc[VEC];
+#pragma unroll
+    for (int i = 0; i < VEC; ++i) acc[i] = 0.f;
+    float lse_v = -INFINITY;
+    if (np > 0) {
+        const float* pm = part_m + (size_t)row * nparts;
+        const float* pl = part_l + (size_t)row * nparts;
+        float M = -INFINITY;
+        for (int i = lane; i < np; i += 32) M = fmaxf(M, pm[i]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+        float lsum = 0.f;
+        const float* po = part_O + (size_t)row * nparts * D + lane * VEC;
+#pragma unroll 4
+        for (int i = 0; i < np; ++i) {
+            const float a = fast_exp2(pm[i] - M);
+            lsum += a * pl[i];
+            if constexpr (VEC == 4) {
+                const float4 v = *reinterpret_cast<const float4*>(po + (size_t)i * D);
+                acc[0] += a * v.x; acc[1] += a * v.y; acc[2] += a * v.z; acc[3] += a * v.w;
+            } else {
+                const float2 v = *reinterpret_cast<const float2*>(po + (size_t)i * D);
+                acc[0] += a * v.x; acc[1] += a * v.y;
+            }
+        }
+        const float inv = 1.f / lsum;
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) acc[i] *= inv;
+        lse_v = (M + log2f(lsum)) * 0.6931471805599453f;
+    }
+    store_out_vec(out, out_f32, (size_t)row * D + lane * VEC, acc, VEC);
+    if (lse && lane == 0) lse[row] = lse_v;
+}
+
+// ---------------------------------------------------------------------------------------------
+static int32_t round_up(int32_t x, int32_t m) { return (x + m - 1) / m * m; }
+
+static int32_t auto_chunk(int32_t S, int32_t Hkv, int32_t max_seq_len) {
+    // ~8 work items per SM at the length upper bound, 128..512-token partitions, at most 128 partitions
+    const int64_t upper = (int64_t)S * Hkv * (max_seq_len > 0 ? max_seq_len : 1);
+    int64_t c = upper / ((int64_t)device_sm_count() * 8);
+    if (c < 128) c = 128;
+    if (c > 512) c = 512;
+    int32_t chunk = round_up((int32_t)c, kDecodeTok);
+    if ((max_seq_len + chunk - 1) / chunk > 128) chunk = round_up((max_seq_len + 127) / 128, kDecodeTok);
+    return chunk;
+}
+
+static void partition_plan(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t num_partitions, int32_t* chunk,
+                           int32_t* nparts) {
+    const int32_t msl = max_seq_len > 0 ? max_seq_len : 1;
+    if (num_partitions <= 0) {
+        *chunk = auto_chunk(S, Hkv, msl);
+    } else {
+        *chunk = round_up((msl + num_partitions - 1) / num_partitions, kDecodeTok);
+    }
+    *nparts = (msl + *chunk - 1) / *chunk;
+    if (num_partitions > 0 && *nparts > num_partitions) *nparts = num_partitions;
+}
+
+template <int D, int PAGE, int GH>
+static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, cudaStream_t stream) {
+    using SM = DecodeSmem<D, GH>;
+    const int max_smem = device_max_smem_optin();
+    int nstages = (int)(((int64_t)max_smem - 1024 - SM::kFixed - (int64_t)(p.S + 1) * 4 - 16) / SM::kStageBytes);
+    if (nstages > kMaxStages) nstages = kMaxStages;
+    if (nstages < 2) return MSTAR_ERR_UNSUPPORTED;
+    p.nstages = nstages;
+    const size_t smem = SM::bytes(nstages, p.S);
+    auto kern = decode_splitk_kernel<D, PAGE, GH>;
+    static bool attr_set = false;  // per instantiation
+    if (!attr_set) {
+        MSTAR_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+        attr_set = true;
+    }
+    int grid = device_sm_count();
+    if (grid > max_items) grid = max_items;
+    if (grid < 1) grid = 1;
+    kern<<<grid, kDecodeThreads, smem, stream>>>(maps.k, maps.v, p);
+    MSTAR_CUDA_OK(cudaGetLastError());
+    launch_count_add(1);
+    return MSTAR_OK;
+}
+
+}  // namespace mstar
+
+extern "C" int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv_heads,
+                                                           int32_t max_seq_len) {
+    int32_t chunk, nparts;
+    mstar::partition_plan(num_seqs, num_kv_heads, max_seq_len, 0, &chunk, &nparts);
+    return nparts;
+}
+
+extern "C" size_t mstar_paged_attn_decode_workspace_bytes(int32_t num_seqs, int32_t num_q_heads, int32_t head_dim,
+                                                          int32_t max_partitions) {
+    if (num_seqs <= 0 || num_q_heads <= 0 || head_dim <= 0 || max_partitions <= 1) return 256;
+    const size_t rows = (size_t)num_seqs * num_q_heads * max_partitions;
+    return 256 + rows * head_dim * 4 + 2 * rows * 4 + 256;
+}
+
+extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool,
+                                       const int32_t* block_table, int64_t block_table_stride,
+                                       const int32_t* seq_lens, int32_t num_seqs, int32_t num_q_heads,
+                                       int32_t max_seq_len, float scale, int32_t num_partitions, uint32_t flags,
+                                       void* workspace, size_t workspace_bytes, void* stream) {
+    using namespace mstar;
+    launch_count_reset();
+    int rc = check_pool(pool);
+    if (rc != MSTAR_OK) return rc;
+    if (flags & ~MSTAR_FLAG_OUT_F32) return MSTAR_ERR_INVALID_ARG;
+    if (num_seqs < 0 || num_q_heads <= 0 || max_seq_len < 0 || num_partitions < 0) return MSTAR_ERR_INVALID_ARG;
+    if (!(scale > 0.f) || !(scale < 3.0e38f)) return MSTAR_ERR_INVALID_ARG;  // positive and finite
+    if (num_seqs == 0) return MSTAR_OK;
+    if (!out || !q || !block_table || !seq_lens) return MSTAR_ERR_INVALID_ARG;
+    if (!aligned(out, 16) || !aligned(q, 16) || !aligned(block_table, 4) || !aligned(seq_lens, 4))
+        return MSTAR_ERR_INVALID_ARG;
+    if (num_q_heads % pool->num_kv_heads) return MSTAR_ERR_INVALID_ARG;
+    const int G = num_q_heads / pool->num_kv_heads;
+    if (G > 16) return MSTAR_ERR_UNSUPPORTED;
+    if (num_seqs > 16384) return MSTAR_ERR_UNSUPPORTED;
+    const int D = pool->head_dim, PAGE = pool->page_size;
+
+    DecodeParams p{};
+    partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, &p.chunk, &p.nparts);
+    p.direct = (p.nparts == 1);
+    if (!p.direct) {
+        const size_t need = mstar_paged_attn_decode_workspace_bytes(num_seqs, num_q_heads, D, p.nparts);
+        if (!workspace || !aligned(workspace, 16)) return MSTAR_ERR_INVALID_ARG;
+        if (workspace_bytes < need) return MSTAR_ERR_WORKSPACE_TOO_SMALL;
+        const size_t rows = (size_t)num_seqs * num_q_heads * p.nparts;
+        p.part_O = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + 256);
+        p.part_m = p.part_O + rows * D;
+        p.part_l = p.part_m + rows;
+    }
+    p.q = reinterpret_cast<const uint16_t*>(q);
+    p.block_table = block_table;
+    p.bt_stride = block_table_stride;
+    p.seq_lens = seq_lens;
+    p.S = num_seqs;
+    p.Hq = num_q_heads;
+    p.Hkv = pool->num_kv_heads;
+    p.G = G;
+    p.scale_log2 = scale * 1.4426950408889634f;
+    p.out = out;
+    p.lse = lse_out;
+    p.out_f32 = (flags & MSTAR_FLAG_OUT_F32) ? 1 : 0;
+
+    PoolMaps maps;
+    rc = get_pool_maps(pool, &maps);
+    if (rc != MSTAR_OK) return rc;
+
+    const int64_t max_items64 = (int64_t)num_seqs * p.nparts * pool->num_kv_heads;
+    const int max_items = max_items64 > (1 << 30) ? (1 << 30) : (int)max_items64;
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool g16 = G > 8;
+#define MSTAR_DECODE_CASE(DD, PP)                                                                  \
+    if (D == DD && PAGE == PP)                                                                     \
+        rc = g16 ? launch_decode<DD, PP, 16>(maps, p, max_items, st) : launch_decode<DD, PP, 8>(maps, p, max_items, st);
+    rc = MSTAR_ERR_UNSUPPORTED;
+    MSTAR_DECODE_CASE(128, 16)
+    MSTAR_DECODE_CASE(128, 32)
+    MSTAR_DECODE_CASE(64, 16)
+    MSTAR_DECODE_CASE(64, 32)
+#undef MSTAR_DECODE_CASE
+    if (rc != MSTAR_OK) return rc;
+
+    if (!p.direct) {
+        const int n_rows = num_seqs * num_q_heads;
+        const int blocks = (n_rows + 3) / 4;
+        if (D == 128)
+            decode_combine_kernel<128><<<blocks, 128, 0, st>>>(p.part_O, p.part_m, p.part_l, seq_lens, p.chunk,
+                                                              p.nparts, num_q_heads, n_rows, out, lse_out, p.out_f32);
+        else
+            decode_combine_kernel<64><<<blocks, 128, 0, st>>>(p.part_O, p.part_m, p.part_l, seq_lens, p.chunk,
+                                                             p.nparts, num_q_heads, n_rows, out, lse_out, p.out_f32);
+        MSTAR_CUDA_OK(cudaGetLastError());
+        launch_count_add(1);
+    }
+    return MSTAR_OK;
+}

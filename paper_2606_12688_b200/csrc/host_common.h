@@ -1,0 +1,48 @@
+// host_common.h -- host-side helpers shared by the launchers: status plumbing, launch counting,
+// argument checks and the TMA tensor-map cache for the K/V pools.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/mstar_attn.h"
+
+namespace mstar {
+
+// thread-local count of kernels the current API call has enqueued
+void launch_count_reset();
+void launch_count_add(int n);
+
+inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+// Validates the pool geometry common to all entry points.  Returns MSTAR_OK or a negative status.
+int check_pool(const mstar_kv_pool* pool);
+
+// One tensor map per pool tensor: 4-D view (D, page_size, Hkv, num_pages) of bf16 with a
+// (64, page_size, 1, 1) box and 128-B swizzle, so that a (page, kv head, 64-column half) slab lands in
+// shared memory as page_size rows of 128 B, conflict-free for ldmatrix.  Cached per
+// (pointer, geometry); thread-safe.
+struct PoolMaps {
+    CUtensorMap k;
+    CUtensorMap v;
+};
+int get_pool_maps(const mstar_kv_pool* pool, PoolMaps* out);
+
+// 3-D view (D, Hq, total_rows) of a contiguous [rows][Hq][D] bf16 tensor with a (64, 1, box_rows) box,
+// 128-B swizzle.  Not cached (cheap, pointer changes every call).
+int make_rows_map(const void* base, int64_t rows, int32_t num_heads, int32_t head_dim, int32_t box_rows,
+                  CUtensorMap* out);
+
+int device_sm_count();
+int device_max_smem_optin();
+
+#define MSTAR_CUDA_OK(expr)                         \
+    do {                                            \
+        cudaError_t e__ = (expr);                   \
+        if (e__ != cudaSuccess) {                   \
+            (void)cudaGetLastError();               \
+            return MSTAR_ERR_CUDA;                  \
+        }                                           \
+    } while (0)
+
+}  // namespace mstar

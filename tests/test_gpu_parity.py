@@ -1,0 +1,289 @@
+"""GPU parity: the CUDA path through the C ABI vs the fp64 oracle on the same seeded inputs.
+
+Gates (R11, from BASELINE.json north_star): page scatter bit-exact; attention output
+max-abs <= 2e-2 and per-row max-rel <= 1e-2 against the oracle.  All tests here need a B200.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2606_12688_b200 as mstar
+import workloads as W
+from tests.gpu_util import DeviceBatch, bf16_tensor, bits_of, f64_of
+from tests.util import check_parity, compact_pool_after_append, decode_q, f64_from_bf16_bits
+
+pytestmark = pytest.mark.gpu
+
+
+def small_batch(seed, lens, q_lens=None, Hq=8, Hkv=2, D=64, p=16, pool=None, **kw):
+    rng = np.random.default_rng(seed)
+    q_lens = [min(1, l) for l in lens] if q_lens is None else q_lens
+    pages = sum((l + p - 1) // p for l in lens)
+    return W.make_batch(rng, "t", lens, q_lens, Hq, Hkv, D, p, pool or max(2 * pages, 4), **kw)
+
+
+def oracle_decode(b):
+    k, v = compact_pool_after_append(b)
+    return oracle.paged_decode(decode_q(b), k, v, b.compact_block_table, b.seq_lens, b.scale)
+
+
+def run_decode_case(b, parts_list=(0,), layout="HND", check_f32=True):
+    db = DeviceBatch(b, layout=layout)
+    db.append()
+    want, want_lse = oracle_decode(b)
+    stats = {}
+    for parts in parts_list:
+        out, lse = db.decode(num_partitions=parts)
+        stats[parts] = check_parity(f64_of(out), want, "%s parts=%d" % (b.name, parts))
+        got_lse = f64_of(lse)
+        fin = np.isfinite(want_lse)
+        assert np.array_equal(np.isneginf(got_lse), np.isneginf(want_lse))
+        assert np.abs(got_lse[fin] - want_lse[fin]).max(initial=0.0) < 2e-3
+        if check_f32:
+            out32, _ = db.decode(num_partitions=parts, out_dtype=torch.float32)
+            a, r = check_parity(f64_of(out32), want, "%s parts=%d f32" % (b.name, parts))
+            assert r <= 6e-3  # without the bf16 output rounding the kernel error alone (bf16 P) must be smaller
+    return stats
+
+
+# ----------------------------------------------------------------------------- append
+
+@pytest.mark.parametrize("layout", ["HND", "NHD"])
+def test_append_bit_exact_whole_pool(layout):
+    b = small_batch(101, [1, 17, 33, 100, 64], q_lens=[1, 5, 33, 40, 64], Hq=4, Hkv=2, D=128, p=16)
+    db = DeviceBatch(b, layout=layout)
+    db.append()
+    torch.cuda.synchronize()
+    k_ref, v_ref = b.full_pool()
+    oracle.kv_append(k_ref, v_ref, b.k_new, b.v_new, b.slot_mapping)
+    assert np.array_equal(bits_of(db.k_pool), k_ref)
+    assert np.array_equal(bits_of(db.v_pool), v_ref)
+
+
+def test_append_negative_slots_and_config3_scale():
+    b = W.config3_prefill()
+    db = DeviceBatch(b)
+    slot = b.slot_mapping.copy()
+    slot[::7] = -1
+    db.slot_mapping = torch.from_numpy(slot).cuda()
+    db.append()
+    k_ref, v_ref = b.k_store.copy(), b.v_store.copy()
+    cslot = b.compact_slot_mapping.copy()
+    cslot[::7] = -1
+    oracle.kv_append(k_ref, v_ref, b.k_new, b.v_new, cslot)
+    kg, vg = db.store_rows_bits()
+    assert np.array_equal(kg, k_ref) and np.array_equal(vg, v_ref)
+    # pages no sequence references keep their poison
+    unused = np.setdiff1d(np.arange(b.num_pages), b.used_pages)[:64]
+    assert np.all(bits_of(db.k_pool[torch.from_numpy(unused).cuda()]) == 0x7FC0)
+
+
+def test_build_slot_mapping_matches_generator():
+    b = small_batch(102, [40, 17, 33, 5, 64], q_lens=[40, 1, 16, 5, 3], p=32)
+    db = DeviceBatch(b)
+    out = torch.full((b.total_q,), -5, dtype=torch.int64, device="cuda")
+    mstar.build_slot_mapping(db.block_table, db.cu_seqlens_q, db.seq_lens, b.total_q, b.page_size, out)
+    assert np.array_equal(out.cpu().numpy(), b.slot_mapping)
+
+
+# ----------------------------------------------------------------------------- decode
+
+def test_decode_config1_tiny():
+    run_decode_case(W.config1_tiny_decode(), parts_list=(0, 1, 2, 3, 16))
+
+
+@pytest.mark.parametrize("D,p", [(64, 16), (64, 32), (128, 16), (128, 32)])
+@pytest.mark.parametrize("G", [1, 2, 4, 7, 8, 16])
+def test_decode_edge_lengths(D, p, G):
+    """Lengths straddling page / stage (64) / partition boundaries, incl. L = 0 and L = 1."""
+    lens = [0, 1, p - 1, p, p + 1, 2 * p - 1, 63, 64, 65, 127, 128, 129, 191, 257, 300]
+    Hkv = 2
+    b = small_batch(200 + G, lens, Hq=G * Hkv, Hkv=Hkv, D=D, p=p, table_width=40)
+    run_decode_case(b, parts_list=(0, 1, 3, 9), check_f32=(G in (1, 7)))
+
+
+def test_decode_many_sequences_and_nhd_layout():
+    rng = np.random.default_rng(7)
+    lens = rng.integers(1, 700, 300).tolist()
+    b = small_batch(210, lens, Hq=8, Hkv=4, D=128, p=16)
+    run_decode_case(b, parts_list=(0, 2), layout="NHD", check_f32=False)
+
+
+def test_decode_len1_bit_exact_and_unit_values():
+    """Closed forms on the GPU: L = 1 => out = V row bit-for-bit; V == 1 => out == 1 exactly."""
+    b = small_batch(220, [1, 1, 1, 200, 1000], Hq=8, Hkv=2, D=128, p=16)
+    db = DeviceBatch(b)
+    db.append()
+    out, _ = db.decode(num_partitions=0)
+    k, v = compact_pool_after_append(b)
+    got = bits_of(out)
+    for s in range(3):
+        for h in range(8):
+            assert np.array_equal(got[s, h], v[b.compact_block_table[s, 0], h // 4, 0])
+    db.v_pool[~torch.isnan(db.v_pool)] = 1.0
+    for parts in (0, 1, 5):
+        out, _ = db.decode(num_partitions=parts)
+        assert torch.all(out.float() == 1.0)
+
+
+def test_decode_page_permutation_and_shared_prefix_bit_identical():
+    lens = [300, 300, 77, 77]
+    b = small_batch(230, lens, Hq=8, Hkv=2, D=128, p=16, share_with=[-1, 0, -1, 2], shared_tokens=64, pool=128)
+    db = DeviceBatch(b)
+    db.append()
+    out1, _ = db.decode(num_partitions=3)
+    # relabel physical pages: new id of old page i is perm[i]
+    perm = torch.from_numpy(np.random.default_rng(5).permutation(b.num_pages)).cuda()
+    k2, v2 = torch.empty_like(db.k_pool), torch.empty_like(db.v_pool)
+    k2[perm], v2[perm] = db.k_pool, db.v_pool
+    bt2 = torch.where(db.block_table >= 0, perm[db.block_table.clamp(min=0).long()].int(), db.block_table)
+    out2 = torch.empty_like(out1)
+    ws = torch.empty(mstar.decode_workspace_bytes(4, 8, 128, 3), dtype=torch.uint8, device="cuda")
+    mstar.paged_attn_decode(out2, db.q_decode, mstar.KVPool(k2, v2), bt2.contiguous(), db.seq_lens, 300, float(b.scale),
+                            num_partitions=3, workspace=ws)
+    assert torch.equal(out1.view(torch.int16), out2.view(torch.int16))
+    # duplicated prefix: sequence 1 gets private copies of the shared pages
+    free = np.setdiff1d(np.arange(b.num_pages), b.used_pages)
+    bt3 = db.block_table.clone()
+    for i in range(4):
+        db.k_pool[free[i]] = db.k_pool[bt3[1, i].item()]
+        db.v_pool[free[i]] = db.v_pool[bt3[1, i].item()]
+        bt3[1, i] = int(free[i])
+    out3 = torch.empty_like(out1)
+    mstar.paged_attn_decode(out3, db.q_decode, db.pool, bt3, db.seq_lens, 300, float(b.scale), num_partitions=3,
+                            workspace=ws)
+    assert torch.equal(out1.view(torch.int16), out3.view(torch.int16))
+
+
+def test_decode_deterministic_and_graph_capturable():
+    b = small_batch(240, [500, 123, 64, 1], Hq=14, Hkv=2, D=128, p=16)
+    db = DeviceBatch(b)
+    want, _ = oracle_decode(b)
+    S, Hq, D = 4, 14, 128
+    out = torch.zeros((S, Hq, D), dtype=torch.bfloat16, device="cuda")
+    ws = torch.empty(mstar.decode_workspace_bytes(S, Hq, D, 4), dtype=torch.uint8, device="cuda")
+
+    def step():
+        db.append()
+        mstar.paged_attn_decode(out, db.q_decode, db.pool, db.block_table, db.seq_lens, 500, float(b.scale),
+                                num_partitions=4, workspace=ws)
+
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    first = out.clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        step()
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(first.view(torch.int16), out.view(torch.int16))
+    check_parity(f64_of(out), want, "graph replay")
+
+
+def test_decode_config2_bagel_cfg_pairs():
+    stats = run_decode_case(W.config2_bagel_cfg_decode(), parts_list=(0, 4), check_f32=False)
+    print("cfg2", stats)
+
+
+def test_decode_config4_thinker_and_talker():
+    print("thinker", run_decode_case(W.config4_thinker(), parts_list=(0,), check_f32=False))
+    print("talker", run_decode_case(W.config4_talker(), parts_list=(0,), check_f32=False))
+
+
+def test_decode_config5_long_context_full_size():
+    """The bench configuration: 16 x 32768 tokens, 60 GiB pool, 16 partitions; all 512 rows vs the oracle."""
+    free, _ = torch.cuda.mem_get_info()
+    pages = 491520
+    if free < 70 * (1 << 30):   # smaller pool, same 2.1 GB of K/V, if the box is short of memory
+        pages = 65536
+    b = W.config5_long_context(num_pages=pages)
+    db = DeviceBatch(b)
+    db.append()
+    out, lse = db.decode(num_partitions=16)
+    k, v = compact_pool_after_append(b)
+    want, want_lse = oracle.paged_decode(b.q, k, v, b.compact_block_table, b.seq_lens, b.scale)
+    print("cfg5", check_parity(f64_of(out), want, "cfg5"))
+    assert np.abs(f64_of(lse) - want_lse).max() < 2e-3
+    # convex-hull invariant at full scale: every output lies within [min_j V, max_j V] of its kv head
+    out64 = f64_of(out)
+    V = f64_from_bf16_bits(v[b.compact_block_table[0, :1024]])      # sequence 0: [pages, Hkv, p, D]
+    vmin, vmax = V.min(axis=(0, 2)), V.max(axis=(0, 2))
+    for h in range(32):
+        assert np.all(out64[0, h] <= vmax[h // 4] + 1e-6) and np.all(out64[0, h] >= vmin[h // 4] - 1e-6)
+
+
+# ----------------------------------------------------------------------------- prefill
+
+def run_prefill_case(b, rows=None, causal=True, layout="HND"):
+    db = DeviceBatch(b, layout=layout)
+    db.append()
+    out, lse = db.prefill(causal=causal)
+    k, v = compact_pool_after_append(b)
+    want, want_lse = oracle.paged_prefill(b.q, b.cu_seqlens_q, k, v, b.compact_block_table, b.seq_lens, b.scale,
+                                          causal=causal, rows=rows)
+    got, got_lse = f64_of(out), f64_of(lse)
+    if rows is not None:
+        got, got_lse = got[rows], got_lse[rows]
+    st = check_parity(got, want, b.name)
+    assert np.abs(got_lse - want_lse).max() < 2e-3
+    return st
+
+
+@pytest.mark.parametrize("D,p", [(64, 16), (128, 16), (128, 32)])
+@pytest.mark.parametrize("G", [1, 4, 7, 8, 12])
+def test_prefill_ragged_small(D, p, G):
+    lens = [40, 17, 33, 5, 64, 200, 129, 1, 300]
+    qls = [40, 1, 16, 5, 3, 127, 129, 1, 17]
+    b = small_batch(300 + G, lens, q_lens=qls, Hq=G * 2, Hkv=2, D=D, p=p)
+    run_prefill_case(b)
+    run_prefill_case(b, causal=False)
+
+
+def test_prefill_one_token_equals_decode_semantics():
+    b = small_batch(310, [1, 17, 33, 100, 700], Hq=8, Hkv=2, D=128)
+    db = DeviceBatch(b)
+    db.append()
+    out_p, _ = db.prefill()
+    want, _ = oracle_decode(b)
+    check_parity(f64_of(out_p), want, "prefill n=1")
+
+
+def test_prefill_nhd_layout_and_empty_sequences():
+    b = small_batch(320, [50, 0, 30, 16], q_lens=[20, 0, 30, 0], Hq=4, Hkv=2, D=128)
+    run_prefill_case(b, layout="NHD")
+
+
+def test_prefill_config3_sampled_rows():
+    b = W.config3_prefill()
+    rng = np.random.default_rng(33)
+    rows = np.unique(np.concatenate([rng.integers(0, b.total_q, 96),
+                                     b.cu_seqlens_q[:-1], b.cu_seqlens_q[1:] - 1,
+                                     b.cu_seqlens_q[:-1] + 15, b.cu_seqlens_q[:-1] + 16])).astype(np.int32)
+    print("cfg3", run_prefill_case(b, rows=rows))
+
+
+# ----------------------------------------------------------------------------- errors
+
+def test_error_codes():
+    b = small_batch(400, [33, 20], Hq=4, Hkv=2, D=64)
+    db = DeviceBatch(b)
+    out = torch.empty((2, 4, 64), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(mstar.MstarError, match="WORKSPACE_TOO_SMALL"):
+        mstar.paged_attn_decode(out, db.q_decode, db.pool, db.block_table, db.seq_lens, 33, 0.125, num_partitions=4,
+                                workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
+    with pytest.raises(mstar.MstarError, match="INVALID_ARG"):   # Hq not a multiple of Hkv
+        q3 = torch.zeros((2, 3, 64), dtype=torch.bfloat16, device="cuda")
+        mstar.paged_attn_decode(torch.empty_like(q3), q3, db.pool, db.block_table, db.seq_lens, 33, 0.125,
+                                num_partitions=1)
+    with pytest.raises(mstar.MstarError, match="INVALID_ARG"):   # misaligned q
+        buf = torch.zeros(2 * 4 * 64 + 8, dtype=torch.bfloat16, device="cuda")
+        mstar.paged_attn_decode(out, buf[1:1 + 512].view(2, 4, 64), db.pool, db.block_table, db.seq_lens, 33,
+                                0.125, num_partitions=1)
+    with pytest.raises(mstar.MstarError, match="INVALID_ARG"):   # non-positive scale
+        mstar.paged_attn_decode(out, db.q_decode, db.pool, db.block_table, db.seq_lens, 33, 0.0, num_partitions=1)

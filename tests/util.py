@@ -32,6 +32,15 @@ def compact_pool_after_append(batch: PagedBatch):
     return k, v
 
 
+def decode_q(batch: PagedBatch) -> np.ndarray:
+    """One query row per sequence for decode: the sequence's new token, zeros where it has none (L = 0)."""
+    assert int(batch.q_lens.max(initial=0)) <= 1
+    q = np.zeros((batch.num_seqs, batch.num_q_heads, batch.head_dim), dtype=np.uint16)
+    has = batch.q_lens > 0
+    q[has] = batch.q[batch.cu_seqlens_q[:-1][has]]
+    return q
+
+
 def dense_kv(batch: PagedBatch, k_pool, v_pool, block_table, s):
     """Gather sequence s to dense fp64 K, V [L, Hkv, D] with numpy indexing."""
     p = batch.page_size
