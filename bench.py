@@ -1,0 +1,420 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the paged-KV attention hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A STEP is one pass of the whole hot path (rows a1..a4) over one batch of seeded
+synthetic input:
+    segment D  (BASELINE.json configs[4], the long-context decode the 70 %-of-HBM target is quoted on):
+               mstar_kv_append of the 16 newest rows -> mstar_paged_attn_decode (split-K over 16 partitions
+               + LSE combine) over 16 x 32768 tokens scattered in a 60 GiB pool;
+    segment P  (configs[2], the prefill the 50 %-of-tensor-peak target is quoted on):
+               mstar_kv_append of 8192 new rows -> mstar_paged_attn_prefill, causal over cached prefixes.
+`value` is the decode metric (algorithmic K/V GB/s of segment D, inputs resident in HBM); the prefill
+metric (TFLOP/s of segment P) rides in `prefill`.  `e2e` is the same decode metric with every per-step
+input in pinned HOST memory, copied in and the output copied out inside the timed region (the K/V pool
+is serving state and stays resident, like weights).  `roofline` / `roofline_prefill` are algorithmic
+bytes (flops) over the CUDA-event duration of the kernel's launches against MEASURED_PEAKS.json.
+`cpu_baseline` times the fp64 oracle on the host cores on a bounded sample of segment D.
+
+Multi-GPU: the path does not shard across GPUs ("replicas only"): --gpus N runs N
+independent replicas under torchrun, barrier + max-over-ranks timing, value = sum of the replicas' bytes
+over the slowest replica's time ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "paged_decode_attn_GBps"
+UNIT = "GB/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            pk = json.load(f)
+        return {"hbm_gbs": float(pk["hbm_gbs"]), "bf16_tflops": float(pk["bf16_tflops"]),
+                "bf16_tflops_sustained": float(pk.get("bf16_tflops_sustained", pk["bf16_tflops"])),
+                "source": "measured (MEASURED_PEAKS.json)"}
+    except Exception:
+        return dict(FALLBACK_PEAKS, source="fallback (B200_PROFILING.md)")
+
+
+# ----------------------------------------------------------------------------- algorithmic work
+
+def decode_bytes(b, nparts):
+    """Algorithmic bytes of one decode call: K/V once, Q in, O out, tables, split-K partials write+read."""
+    kv = b.kv_bytes_logical()
+    S, Hq, D, p = b.num_seqs, b.num_q_heads, b.head_dim, b.page_size
+    qo = 2 * S * Hq * D * 2
+    tables = 4 * int(((b.seq_lens.astype(np.int64) + p - 1) // p).sum()) + 4 * S
+    parts = 0 if nparts <= 1 else 2 * S * Hq * nparts * (D + 2) * 4
+    return kv, kv + qo + tables + parts
+
+
+def prefill_flops(b):
+    """sum_s 4 Hq D (n_s P_s + n_s (n_s + 1) / 2): QK^T and PV, 2 flops per MAC, masked triangle excluded."""
+    n = b.q_lens.astype(np.float64)
+    P = b.seq_lens.astype(np.float64) - n
+    return float((4.0 * b.num_q_heads * b.head_dim * (n * P + n * (n + 1) / 2)).sum())
+
+
+def append_bytes(b):
+    return 2 * 2 * b.total_q * b.num_kv_heads * b.head_dim * 2
+
+
+# ----------------------------------------------------------------------------- clocks
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.004):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period_s
+        self.samples, self.reason_bits = [], 0
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.reason_bits |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2.0)
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        names = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+                 0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+                 0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+        reasons = [n for bit, n in names.items() if self.reason_bits & bit and n != "gpu_idle"]
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": reasons,
+                "samples": len(self.samples)}
+
+
+# ----------------------------------------------------------------------------- distributed plumbing (replicas)
+
+def dist_setup(n_gpus: int):
+    """Returns (rank, world, local_rank, dist or None).  One process per GPU under torchrun."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world == 1:
+        return 0, 1, 0, None
+    import torch
+    import torch.distributed as dist
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    backend = "nccl" if torch.cuda.is_available() else "gloo"
+    if backend == "nccl":
+        torch.cuda.set_device(local)
+    dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return rank, world, local, dist
+
+
+def max_over_ranks(dist, value: float, device) -> float:
+    """Max of a per-rank scalar (device time in ms) over all ranks; identity for a single process."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(dist, value: float, device) -> float:
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+# ----------------------------------------------------------------------------- CPU oracle legs
+
+def oracle_sample_batch(n_seqs: int):
+    import workloads as W
+    return W.config5_long_context(num_seqs=n_seqs, num_pages=max(4096, n_seqs * 1024 * 2))
+
+
+def time_oracle_decode(b):
+    """Wall seconds of the fp64 oracle (append + decode) on batch b, as it stands."""
+    import oracle
+    k, v = b.k_store.copy(), b.v_store.copy()
+    t0 = time.perf_counter()
+    oracle.kv_append(k, v, b.k_new, b.v_new, b.compact_slot_mapping)
+    oracle.paged_decode(b.q, k, v, b.compact_block_table, b.seq_lens, b.scale)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(b):
+    """The oracle as it stands on the host cores, on the decode batch the GPU was timed on."""
+    import oracle
+    time_oracle_decode(b)                      # warm-up (page-faults the buffers)
+    dt = min(time_oracle_decode(b) for _ in range(2))
+    return {"value": b.kv_bytes_logical() / dt / 1e9, "unit": UNIT, "cores": oracle.num_threads(),
+            "kind": "oracle", "seconds": dt,
+            "sample": "all %d sequences of configs[4] (32768 tokens, 32q/8kv heads, D 128, page 32), "
+                      "append + decode, fp64, best of 2 after one warm-up" % b.num_seqs}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    n_seqs = 1
+    b = oracle_sample_batch(n_seqs)
+    for _ in range(args.warmup):
+        time_oracle_decode(b)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        time_oracle_decode(b)
+    dt = (time.perf_counter() - t0) / max(args.steps, 1)
+    val = b.kv_bytes_logical() / dt / 1e9
+    sample = ("%d of the 16 sequences of configs[4] per step (32768 tokens, 32q/8kv, D 128, page 32), append + "
+              "decode, fp64 oracle" % n_seqs)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[4] long-context decode, bounded sample", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------- the CUDA arm
+
+def run_ours(args):
+    import torch
+    rank, world, local, dist = dist_setup(args.gpus)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback; use --impl reference "
+                         "for the oracle timing)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    import paper_2606_12688_b200 as mstar
+    from paper_2606_12688_b200.harness import DeviceBatch, bf16_tensor
+    import workloads as W
+    mstar.load_library()
+    peaks = load_peaks()
+
+    # ---- inputs (seeded, host-generated, uploaded once)
+    free, _ = torch.cuda.mem_get_info()
+    pool_pages = 491520 if free > 72 * (1 << 30) else 65536
+    bd = W.config5_long_context(num_pages=pool_pages)
+    bp = W.config3_prefill()
+    D5 = DeviceBatch(bd, device=dev)
+    D3 = DeviceBatch(bp, device=dev)
+    NPARTS = 16
+    S5, Hq5, Dh = bd.num_seqs, bd.num_q_heads, bd.head_dim
+    out5 = torch.empty((S5, Hq5, Dh), dtype=torch.bfloat16, device=dev)
+    ws5 = torch.empty(mstar.decode_workspace_bytes(S5, Hq5, Dh, NPARTS), dtype=torch.uint8, device=dev)
+    out3 = torch.empty((bp.total_q, bp.num_q_heads, bp.head_dim), dtype=torch.bfloat16, device=dev)
+    ws3 = torch.empty(mstar.prefill_workspace_bytes(bp.num_seqs, bp.total_q, bp.num_q_heads, bp.head_dim),
+                      dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    msl5, msl3, mql3 = bd.max_seq_len, bp.max_seq_len, bp.max_q_len
+    sc5, sc3 = float(bd.scale), float(bp.scale)
+    launches = [0]
+
+    def seg_decode():
+        mstar.kv_append(D5.pool, D5.k_new, D5.v_new, D5.slot_mapping); launches[0] += mstar.last_launch_count()
+        mstar.paged_attn_decode(out5, D5.q_decode, D5.pool, D5.block_table, D5.seq_lens, msl5, sc5,
+                                num_partitions=NPARTS, workspace=ws5); launches[0] += mstar.last_launch_count()
+
+    def seg_prefill():
+        mstar.kv_append(D3.pool, D3.k_new, D3.v_new, D3.slot_mapping); launches[0] += mstar.last_launch_count()
+        mstar.paged_attn_prefill(out3, D3.q, D3.cu_seqlens_q, D3.pool, D3.block_table, D3.seq_lens, mql3, msl3,
+                                 sc3, causal=True, workspace=ws3); launches[0] += mstar.last_launch_count()
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        seg_decode(); flush.fill_(1); seg_prefill()
+    barrier()
+
+    # ---- timed region: K steps, CUDA events per segment and per kernel group on the launching stream
+    K = args.steps
+    sampler = ClockSampler(local)
+    sampler.start()
+    launches[0] = 0
+    marks = []
+    t_wall0 = time.perf_counter()
+    for _ in range(K):
+        e = [ev() for _ in range(6)]
+        e[0].record()
+        mstar.kv_append(D5.pool, D5.k_new, D5.v_new, D5.slot_mapping); launches[0] += mstar.last_launch_count()
+        e[1].record()
+        mstar.paged_attn_decode(out5, D5.q_decode, D5.pool, D5.block_table, D5.seq_lens, msl5, sc5,
+                                num_partitions=NPARTS, workspace=ws5); launches[0] += mstar.last_launch_count()
+        e[2].record()
+        flush.fill_(1)          # L2 flush between segments, outside the timed events
+        e[3].record()
+        mstar.kv_append(D3.pool, D3.k_new, D3.v_new, D3.slot_mapping); launches[0] += mstar.last_launch_count()
+        e[4].record()
+        mstar.paged_attn_prefill(out3, D3.q, D3.cu_seqlens_q, D3.pool, D3.block_table, D3.seq_lens, mql3, msl3,
+                                 sc3, causal=True, workspace=ws3); launches[0] += mstar.last_launch_count()
+        e[5].record()
+        marks.append(e)
+    barrier()
+    wall_ms = (time.perf_counter() - t_wall0) * 1e3 / K
+    sampler.stop()
+    timed_launches = launches[0]
+    t_app5 = sum(m[0].elapsed_time(m[1]) for m in marks) / K
+    t_dec = sum(m[1].elapsed_time(m[2]) for m in marks) / K
+    t_app3 = sum(m[3].elapsed_time(m[4]) for m in marks) / K
+    t_pre = sum(m[4].elapsed_time(m[5]) for m in marks) / K
+    t_segD = max_over_ranks(dist, t_app5 + t_dec, dev)
+    t_segP = max_over_ranks(dist, t_app3 + t_pre, dev)
+    t_dec_max = max_over_ranks(dist, t_dec, dev)
+    t_pre_max = max_over_ranks(dist, t_pre, dev)
+
+    kv_bytes, dec_bytes = decode_bytes(bd, NPARTS)
+    flops = prefill_flops(bp)
+    value = world * kv_bytes / (t_segD * 1e-3) / 1e9
+    tokens_per_s = world * S5 / (t_segD * 1e-3)
+
+    # ---- e2e: per-step inputs in pinned host memory, copied in; output copied out; same kernels
+    pin = lambda t: t.detach().cpu().pin_memory()
+    h_in = [pin(D5.q_decode), pin(D5.k_new), pin(D5.v_new), pin(D5.slot_mapping), pin(D5.block_table),
+            pin(D5.seq_lens)]
+    d_in = [D5.q_decode, D5.k_new, D5.v_new, D5.slot_mapping, D5.block_table, D5.seq_lens]
+    h_out = torch.empty(out5.shape, dtype=out5.dtype).pin_memory()
+    h2d = sum(t.numel() * t.element_size() for t in h_in)
+    d2h = h_out.numel() * h_out.element_size()
+
+    def e2e_step():
+        for h, d in zip(h_in, d_in):
+            d.copy_(h, non_blocking=True)
+        seg_decode()
+        h_out.copy_(out5, non_blocking=True)
+
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    e0, e1 = ev(), ev()
+    e0.record()
+    for _ in range(K):
+        e2e_step()
+    e1.record()
+    barrier()
+    t_e2e = max_over_ranks(dist, e0.elapsed_time(e1) / K, dev)
+    e2e_value = world * kv_bytes / (t_e2e * 1e-3) / 1e9
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    clocks = sampler.summary()
+    hbm_peak, tf_peak = peaks["hbm_gbs"], peaks["bf16_tflops"]
+    dec_gbs = dec_bytes / (t_dec_max * 1e-3) / 1e9
+    pre_tfs = flops / (t_pre_max * 1e-3) / 1e12
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
+        "warmup": max(args.warmup, 3), "ms_per_step": t_segD + t_segP, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {
+            "workload": "configs[4] long-context decode (a1 append 16 rows + a2 split-K x16 + a3 combine) then "
+                        "configs[2] causal prefill over cached prefix (a1 append 8192 rows + a4)",
+            "decode": {"seqs": S5, "seq_len": msl5, "q_heads": Hq5, "kv_heads": bd.num_kv_heads, "head_dim": Dh,
+                       "page_size": bd.page_size, "pool_pages": pool_pages, "partitions": NPARTS,
+                       "kv_bytes": kv_bytes},
+            "prefill": {"seqs": bp.num_seqs, "new_tokens": int(bp.q_lens[0]), "prefix": (bp.seq_lens - bp.q_lens).tolist(),
+                        "q_heads": bp.num_q_heads, "kv_heads": bp.num_kv_heads, "head_dim": bp.head_dim,
+                        "page_size": bp.page_size, "flops": flops},
+            "l2": "decode reads 2.1 GB per step (>> 126 MB L2); a 256 MB flush write runs before the prefill "
+                  "segment, outside the timed events",
+            "parallelism": "replicas" if world > 1 else "single GPU",
+        },
+        "ms_decode_segment": t_segD, "ms_prefill_segment": t_segP, "wall_ms_per_step": wall_ms,
+        "decode_tokens_per_s": tokens_per_s,
+        "prefill": {"metric": "paged_prefill_attn_TFLOPs", "value": world * flops / (t_segP * 1e-3) / 1e12,
+                    "unit": "TFLOP/s", "ms": t_segP, "append_GBps": append_bytes(bp) / (t_app3 * 1e-3) / 1e9},
+        "roofline": {"kernel": "decode_splitk_kernel + decode_combine_kernel (one mstar_paged_attn_decode call)",
+                     "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak, "unit": "GB/s",
+                     "frac": dec_gbs / hbm_peak, "traffic": None, "peak_source": peaks["source"],
+                     "frac_of_nominal_8TBps": dec_gbs / 8000.0, "ms": t_dec_max, "bytes": dec_bytes},
+        "roofline_prefill": {"kernel": "prefill kernel (one mstar_paged_attn_prefill call)", "bound": "tensor",
+                             "achieved": pre_tfs, "peak": tf_peak, "unit": "TFLOP/s", "frac": pre_tfs / tf_peak,
+                             "traffic": None, "peak_source": peaks["source"] + ", burst",
+                             "frac_of_sustained": pre_tfs / peaks["bf16_tflops_sustained"],
+                             "frac_of_nominal_2250": pre_tfs / 2250.0, "ms": t_pre_max, "flops": flops},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms": t_e2e, "note": "segment D with q, new K/V rows, slot mapping, block table and seq_lens in "
+                                     "pinned host memory; the K/V pool is resident serving state"},
+        "gpu_launches": timed_launches,
+        "clocks": clocks,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(bd)
+    elif not args.no_cpu_baseline:
+        line["cpu_baseline"] = {"value": None, "unit": UNIT, "cores": None, "kind": "oracle",
+                                "sample": "reported at N=1 only"}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

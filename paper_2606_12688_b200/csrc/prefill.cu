@@ -209,7 +209,9 @@ prefill_mma_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_consta
                 for (int j = 0; j < D / 8; ++j) {
                     o[j][0] *= al_a; o[j][1] *= al_a; o[j][2] *= al_b; o[j][3] *= al_b;
                 }
-                const bool tail = j0 + TOK > L;  // V rows >= L may hold NaN: zero them (0 * NaN guard)
+                // V rows >= kv_end were not loaded (stale shared memory) or hold no token (may be NaN):
+                // zero them, p = 0 there for every row (0 * NaN guard)
+                const bool tail = j0 + TOK > kv_end;
 #pragma unroll
                 for (int kt = 0; kt < TOK / 16; ++kt) {
                     const uint32_t pa0 = pack_bf16x2(sc[2 * kt][0], sc[2 * kt][1]);
@@ -219,8 +221,8 @@ prefill_mma_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_consta
                     uint32_t vm_lo = 0xffffffffu, vm_hi = 0xffffffffu;
                     if (tail) {
                         const int jt = j0 + kt * 16 + 2 * t4;
-                        vm_lo = (jt < L ? 0x0000ffffu : 0u) | (jt + 1 < L ? 0xffff0000u : 0u);
-                        vm_hi = (jt + 8 < L ? 0x0000ffffu : 0u) | (jt + 9 < L ? 0xffff0000u : 0u);
+                        vm_lo = (jt < kv_end ? 0x0000ffffu : 0u) | (jt + 1 < kv_end ? 0xffff0000u : 0u);
+                        vm_hi = (jt + 8 < kv_end ? 0x0000ffffu : 0u) | (jt + 9 < kv_end ? 0xffff0000u : 0u);
                     }
 #pragma unroll
                     for (int jj = 0; jj < D / 16; ++jj) {

@@ -271,11 +271,11 @@ def test_prefill_config3_sampled_rows():
 # ----------------------------------------------------------------------------- errors
 
 def test_error_codes():
-    b = small_batch(400, [33, 20], Hq=4, Hkv=2, D=64)
+    b = small_batch(400, [300, 20], Hq=4, Hkv=2, D=64)
     db = DeviceBatch(b)
     out = torch.empty((2, 4, 64), dtype=torch.bfloat16, device="cuda")
     with pytest.raises(mstar.MstarError, match="WORKSPACE_TOO_SMALL"):
-        mstar.paged_attn_decode(out, db.q_decode, db.pool, db.block_table, db.seq_lens, 33, 0.125, num_partitions=4,
+        mstar.paged_attn_decode(out, db.q_decode, db.pool, db.block_table, db.seq_lens, 300, 0.125, num_partitions=4,
                                 workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
     with pytest.raises(mstar.MstarError, match="INVALID_ARG"):   # Hq not a multiple of Hkv
         q3 = torch.zeros((2, 3, 64), dtype=torch.bfloat16, device="cuda")
