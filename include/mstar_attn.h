@@ -50,6 +50,8 @@ typedef enum {
 /* flags */
 #define MSTAR_FLAG_OUT_F32 1u /* `out` is fp32 instead of bf16 (diagnostic: separates kernel error from
                                  output rounding).  Unknown bits => MSTAR_ERR_INVALID_ARG. */
+#define MSTAR_FLAG_PREFILL_MMA_SYNC 2u /* prefill only, diagnostic: use the warp-level mma.sync kernel instead
+                                          of the tcgen05/TMEM kernel (head_dim 64 always uses it). */
 
 /*
  * The paged K/V pool ("a single paged KV pool").  Caller-owned device memory, bf16.

@@ -33,6 +33,12 @@ int get_pool_maps(const mstar_kv_pool* pool, PoolMaps* out);
 int make_rows_map(const void* base, int64_t rows, int32_t num_heads, int32_t head_dim, int32_t box_rows,
                   CUtensorMap* out);
 
+// tcgen05 / TMEM prefill kernel (prefill_umma.cu); head_dim 128 only
+int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, const int32_t* cu_seqlens_q,
+                        const int32_t* block_table, int64_t bt_stride, const int32_t* seq_lens, int32_t S,
+                        int32_t Hq, int32_t Hkv, int32_t page_size, int32_t max_q_len, float scale, int32_t causal,
+                        void* out, float* lse, int32_t out_f32, cudaStream_t stream);
+
 int device_sm_count();
 int device_max_smem_optin();
 

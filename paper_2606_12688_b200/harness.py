@@ -75,7 +75,7 @@ class DeviceBatch:
                                 num_partitions=num_partitions, workspace=ws, lse_out=lse)
         return out, lse
 
-    def prefill(self, causal=True, out_dtype=torch.bfloat16, want_lse=True):
+    def prefill(self, causal=True, out_dtype=torch.bfloat16, want_lse=True, mma_sync=False):
         b = self.b
         T, Hq, D = b.total_q, b.num_q_heads, b.head_dim
         out = torch.full((T, Hq, D), float("nan"), dtype=out_dtype, device=self.q.device)
@@ -84,7 +84,7 @@ class DeviceBatch:
                          device=self.q.device)
         mstar.paged_attn_prefill(out, self.q, self.cu_seqlens_q, self.pool, self.block_table, self.seq_lens,
                                  b.max_q_len, b.max_seq_len, float(b.scale), causal=causal, workspace=ws,
-                                 lse_out=lse)
+                                 lse_out=lse, mma_sync=mma_sync)
         return out, lse
 
     def store_rows_bits(self):

@@ -221,17 +221,21 @@ def test_decode_config5_long_context_full_size():
 # ----------------------------------------------------------------------------- prefill
 
 def run_prefill_case(b, rows=None, causal=True, layout="HND"):
+    """Both prefill kernels (tcgen05/TMEM default, mma.sync diagnostic) against the oracle."""
     db = DeviceBatch(b, layout=layout)
     db.append()
-    out, lse = db.prefill(causal=causal)
     k, v = compact_pool_after_append(b)
     want, want_lse = oracle.paged_prefill(b.q, b.cu_seqlens_q, k, v, b.compact_block_table, b.seq_lens, b.scale,
                                           causal=causal, rows=rows)
-    got, got_lse = f64_of(out), f64_of(lse)
-    if rows is not None:
-        got, got_lse = got[rows], got_lse[rows]
-    st = check_parity(got, want, b.name)
-    assert np.abs(got_lse - want_lse).max() < 2e-3
+    st = {}
+    for mma_sync in (False, True):
+        out, lse = db.prefill(causal=causal, mma_sync=mma_sync)
+        got, got_lse = f64_of(out), f64_of(lse)
+        if rows is not None:
+            got, got_lse = got[rows], got_lse[rows]
+        what = "%s %s" % (b.name, "mma.sync" if mma_sync else "tcgen05")
+        st[what] = check_parity(got, want, what)
+        assert np.abs(got_lse - want_lse).max() < 2e-3, what
     return st
 
 
