@@ -39,6 +39,10 @@ if ROOT not in sys.path:
 METRIC = "paged_decode_attn_GBps"
 UNIT = "GB/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/r1a_full_summary.csv); valid for the full-size workloads only.
+NCU_TRAFFIC = {"decode": 2147766000 + 5497600 + 4271000, "prefill": 88314000 + 9574912,
+               "source": "profiles/r1a_full_summary.csv"}
 
 
 def load_peaks():
@@ -379,11 +383,14 @@ def run_ours(args):
                     "unit": "TFLOP/s", "ms": t_segP, "append_GBps": append_bytes(bp) / (t_app3 * 1e-3) / 1e9},
         "roofline": {"kernel": "decode_splitk_kernel + decode_combine_kernel (one mstar_paged_attn_decode call)",
                      "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak, "unit": "GB/s",
-                     "frac": dec_gbs / hbm_peak, "traffic": None, "peak_source": peaks["source"],
+                     "frac": dec_gbs / hbm_peak,
+                     "traffic": NCU_TRAFFIC["decode"] if pool_pages == 491520 else None,
+                     "traffic_source": NCU_TRAFFIC["source"], "peak_source": peaks["source"],
                      "frac_of_nominal_8TBps": dec_gbs / 8000.0, "ms": t_dec_max, "bytes": dec_bytes},
         "roofline_prefill": {"kernel": "prefill kernel (one mstar_paged_attn_prefill call)", "bound": "tensor",
                              "achieved": pre_tfs, "peak": tf_peak, "unit": "TFLOP/s", "frac": pre_tfs / tf_peak,
-                             "traffic": None, "peak_source": peaks["source"] + ", burst",
+                             "traffic": NCU_TRAFFIC["prefill"], "traffic_source": NCU_TRAFFIC["source"],
+                             "peak_source": peaks["source"] + ", burst",
                              "frac_of_sustained": pre_tfs / peaks["bf16_tflops_sustained"],
                              "frac_of_nominal_2250": pre_tfs / 2250.0, "ms": t_pre_max, "flops": flops},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
