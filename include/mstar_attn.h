@@ -53,6 +53,10 @@ typedef enum {
 #define MSTAR_FLAG_PREFILL_MMA_SYNC 2u /* prefill only, diagnostic: use the warp-level mma.sync kernel instead
                                           of the tcgen05/TMEM kernel (head_dim 64 always uses it). */
 
+#define MSTAR_FLAG_PREFILL_REUSE_PLAN 4u /* prefill only: `workspace` still holds the plan a previous call built
+                                          for the SAME cu_seqlens_q, seq_lens, head geometry and causal flag (the
+                                          next layer of the same forward pass): skip the plan kernel. */
+
 /*
  * The paged K/V pool ("a single paged KV pool").  Caller-owned device memory, bf16.
  * Element (page, kv_head, token_in_page, d) of K lives at
@@ -124,6 +128,9 @@ int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv
  *   cu_seqlens_q   device, [S+1] int32, cu_seqlens_q[0] = 0, cu_seqlens_q[S] = total_q
  *   seq_lens       device, [S] int32, total KV length INCLUDING the new tokens (>= n_s)
  *   max_q_len, max_seq_len   host upper bounds on n_s and seq_lens
+ *   workspace      device, >= mstar_paged_attn_prefill_workspace_bytes(...) bytes, 16-B aligned.  Holds the
+ *                  device-built attention plan (PAPER.md:136 builds its plan on the CPU): work units sorted
+ *                  heaviest first plus the work counter.  Contents need no initialisation.
  */
 size_t mstar_paged_attn_prefill_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads,
                                                 int32_t head_dim);

@@ -37,7 +37,9 @@ int make_rows_map(const void* base, int64_t rows, int32_t num_heads, int32_t hea
 int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, const int32_t* cu_seqlens_q,
                         const int32_t* block_table, int64_t bt_stride, const int32_t* seq_lens, int32_t S,
                         int32_t Hq, int32_t Hkv, int32_t page_size, int32_t max_q_len, float scale, int32_t causal,
-                        void* out, float* lse, int32_t out_f32, cudaStream_t stream);
+                        void* out, float* lse, int32_t out_f32, int32_t reuse_plan, void* workspace,
+                        size_t workspace_bytes, cudaStream_t stream);
+size_t prefill_umma_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads);
 
 int device_sm_count();
 int device_max_smem_optin();

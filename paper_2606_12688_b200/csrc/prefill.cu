@@ -293,7 +293,12 @@ static int launch_prefill(const PoolMaps& maps, PrefillParams& p, cudaStream_t s
 
 }  // namespace mstar
 
-extern "C" size_t mstar_paged_attn_prefill_workspace_bytes(int32_t, int32_t, int32_t, int32_t) { return 256; }
+extern "C" size_t mstar_paged_attn_prefill_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads,
+                                                           int32_t head_dim) {
+    (void)head_dim;
+    if (num_seqs < 0 || total_q < 0 || num_q_heads <= 0) return 0;
+    return mstar::prefill_umma_workspace_bytes(num_seqs, total_q, num_q_heads);
+}
 
 extern "C" int mstar_paged_attn_prefill(void* out, float* lse_out, const void* q, const int32_t* cu_seqlens_q,
                                         const mstar_kv_pool* pool, const int32_t* block_table,
@@ -302,13 +307,12 @@ extern "C" int mstar_paged_attn_prefill(void* out, float* lse_out, const void* q
                                         float scale, int32_t causal, uint32_t flags, void* workspace,
                                         size_t workspace_bytes, void* stream) {
     using namespace mstar;
-    (void)workspace;
-    (void)workspace_bytes;
     (void)max_seq_len;
     launch_count_reset();
     int rc = check_pool(pool);
     if (rc != MSTAR_OK) return rc;
-    if (flags & ~(MSTAR_FLAG_OUT_F32 | MSTAR_FLAG_PREFILL_MMA_SYNC)) return MSTAR_ERR_INVALID_ARG;
+    if (flags & ~(MSTAR_FLAG_OUT_F32 | MSTAR_FLAG_PREFILL_MMA_SYNC | MSTAR_FLAG_PREFILL_REUSE_PLAN))
+        return MSTAR_ERR_INVALID_ARG;
     if (num_seqs < 0 || total_q < 0 || max_q_len < 0 || num_q_heads <= 0) return MSTAR_ERR_INVALID_ARG;
     if (!(scale > 0.f) || !(scale < 3.0e38f)) return MSTAR_ERR_INVALID_ARG;
     if (num_seqs == 0 || total_q == 0 || max_q_len == 0) return MSTAR_OK;
@@ -343,7 +347,8 @@ extern "C" int mstar_paged_attn_prefill(void* out, float* lse_out, const void* q
     if (D == 128 && p.G <= 128 && !(flags & MSTAR_FLAG_PREFILL_MMA_SYNC))  // tcgen05 / TMEM path
         return launch_prefill_umma(maps, q, total_q, cu_seqlens_q, block_table, block_table_stride, seq_lens, num_seqs,
                                    num_q_heads, pool->num_kv_heads, PAGE, max_q_len, scale, p.causal, out, lse_out,
-                                   p.out_f32, st);
+                                   p.out_f32, (flags & MSTAR_FLAG_PREFILL_REUSE_PLAN) ? 1 : 0, workspace,
+                                   workspace_bytes, st);
     if (D == 128 && PAGE == 16) return launch_prefill<128, 16>(maps, p, st);
     if (D == 128 && PAGE == 32) return launch_prefill<128, 32>(maps, p, st);
     if (D == 64 && PAGE == 16) return launch_prefill<64, 16>(maps, p, st);

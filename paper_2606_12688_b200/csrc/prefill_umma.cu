@@ -1,15 +1,24 @@
 // prefill_umma.cu -- step a4 on the 5th-generation tensor cores: paged prefill attention, causal over a
 // cached prefix, with tcgen05.mma, accumulators in TMEM and TMA-fed operand tiles (head_dim 128).
 //
-// Design.  Persistent CTAs (one per SM), 12 warps:
-//   warp 0      TMA producer: Q tiles (3-D boxes over [token][head][d]) and 128-token K / V stages gathered
-//               page by page through the block table (4-D boxes, 128-B swizzle), double-buffered;
-//   warp 1      MMA issuer (one elected lane): S = Q K^T (operands in shared memory) and O += P V (P read from
-//               TMEM, V MN-major from shared memory), M = 128, N = 128, K = 16 per instruction;
-//   warps 4-7   softmax warpgroup of Q tile A, warps 8-11 of Q tile B: thread = query row = TMEM lane;
-//               tcgen05.ld S, mask, max, exp2, row sum (no shuffles: a thread owns its row), P -> bf16 ->
-//               tcgen05.st into the columns S occupied; lazy rescale of O in TMEM only when the running max
-//               grows by more than 2^8; epilogue O / l -> bf16 -> global.
+// Design.  Two launches per call:
+//   prefill_plan_kernel   one CTA: the device-side attention plan (where the plan is built on
+//                         the CPU).  Enumerates the work units of the batch, counting-sorts them by cost
+//                         (KV stages), heaviest first, writes one 32-byte descriptor per unit and zeroes the
+//                         work counter.
+//   prefill_umma_kernel   persistent CTAs (one per SM), 12 warps, units pulled from the plan with an atomic
+//                         counter (longest-processing-time-first, so the tail is one light unit):
+//     warp 0      TMA producer + scheduler: Q tiles (3-D boxes over [token][head][d]) and 128-token K / V stages
+//                 gathered page by page through the block table (4-D boxes, 128-B swizzle), double-buffered;
+//     warp 1      MMA issuer (one elected lane): S = Q K^T (operands in shared memory) and O += P V (P read from
+//                 TMEM, V MN-major from shared memory), M = 128, N = 128, K = 16 per instruction;
+//     warps 4-7   softmax warpgroup of Q tile A, warps 8-11 of Q tile B: thread = query row = TMEM lane.  The
+//                 whole S row is pulled into registers once (tcgen05.ld), masked on diagonal stages only,
+//                 3-input max, packed f32x2 scale/subtract, ex2, bf16 pack, tcgen05.st over the columns S
+//                 occupied, handed to the MMA warp in two 64-column halves so P V starts while the second half
+//                 is still in the SFU; row sums are taken after the hand-off.  O is rescaled in TMEM only when
+//                 the running max grows by more than 2^8 (lazy rescale); epilogue O / l -> bf16 -> global.
+//   setmaxnreg moves registers from warps 0-3 (56) to the softmax warpgroups (224).
 // A work unit is (sequence, kv head, block of 2*tq query tokens), tq = floor(128 / G): the G grouped query
 // heads of a kv head are packed into the 128 rows of a Q tile (row = token*G + head), so one K/V stage serves
 // all of them and the causal diagonal wastes at most tq columns.  The two Q tiles of a unit ping-pong: while
@@ -28,15 +37,27 @@ constexpr int kPuTok = 128;       // KV tokens per stage
 constexpr int kPuThreads = 384;   // 12 warps
 constexpr int kPuHT = 128 * 128;  // bytes of a half tile: 128 rows x 64 bf16, 128-B swizzled
 constexpr float kPuTau = 8.0f;    // lazy-rescale threshold, log2 units
+constexpr int kPlanBuckets = 1024;
+constexpr int kPlanHeaderInts = 8;  // [0] work counter  [1] CTAs done  [2] number of units
+
+// One work unit, as the plan kernel writes it and every role reads it (32 bytes).
+struct PuDesc {
+    int s;       // sequence
+    int kvh;     // kv head
+    int t0;      // first query token of the unit within the sequence
+    int n;       // query tokens of the sequence
+    int P;       // cached prefix of the sequence (seq_len - n)
+    int r0;      // first global query row of the sequence
+    int kv_end;  // KV positions [0, kv_end) are visible to at least one row of the unit
+    int T;       // KV stages of 128 tokens; 0 terminates
+};
 
 struct PrefillUmmaParams {
-    const int32_t* cu_seqlens_q;
     const int32_t* block_table;
     int64_t bt_stride;
-    const int32_t* seq_lens;
-    int32_t S, Hq, Hkv, G;
-    int32_t tq;       // query tokens per Q tile = floor(128 / G)
-    int32_t nqb;      // query blocks (of 2*tq tokens) per sequence, from the host bound max_q_len
+    int32_t* plan;
+    int32_t Hq, G;
+    int32_t tq;  // query tokens per Q tile = floor(128 / G)
     float scale_log2;
     void* out;
     float* lse;
@@ -44,28 +65,66 @@ struct PrefillUmmaParams {
     int32_t causal;
 };
 
-struct PuUnit {
-    int s, kvh, t0, n, P, L, r0, kv_end, T;
-    bool valid;
-};
-
-__device__ __forceinline__ PuUnit pu_unit(const PrefillUmmaParams& p, int u) {
-    PuUnit x;
-    const int per = p.S * p.Hkv;
-    const int qb = p.nqb - 1 - u / per;  // heaviest (latest) query blocks first
-    const int rem = u % per;
-    x.s = rem / p.Hkv;
-    x.kvh = rem % p.Hkv;
-    x.r0 = __ldg(p.cu_seqlens_q + x.s);
-    x.n = __ldg(p.cu_seqlens_q + x.s + 1) - x.r0;
-    x.t0 = qb * 2 * p.tq;
-    x.valid = x.t0 < x.n;
-    x.L = __ldg(p.seq_lens + x.s);
-    x.P = x.L - x.n;
-    const int rows_tok = min(2 * p.tq, x.n - x.t0);
-    x.kv_end = p.causal ? x.P + x.t0 + rows_tok : x.L;
-    x.T = (x.kv_end + kPuTok - 1) / kPuTok;
-    return x;
+// ------------------------------------------------------------------------------------------------ plan
+__global__ void __launch_bounds__(kPlanBuckets)
+prefill_plan_kernel(const int32_t* __restrict__ cu_seqlens_q, const int32_t* __restrict__ seq_lens, int S, int Hkv,
+                    int tq, int nqb, int causal, int32_t* __restrict__ plan) {
+    __shared__ int hist[kPlanBuckets];
+    __shared__ int scan[kPlanBuckets];
+    const int tid = threadIdx.x;
+    hist[tid] = 0;
+    __syncthreads();
+    const int64_t total = (int64_t)nqb * S;
+    auto unit_of = [&](int64_t i, PuDesc& d) -> bool {
+        d.s = (int)(i % S);
+        const int qb = (int)(i / S);
+        d.r0 = __ldg(cu_seqlens_q + d.s);
+        d.n = __ldg(cu_seqlens_q + d.s + 1) - d.r0;
+        d.t0 = qb * 2 * tq;
+        if (d.t0 >= d.n) return false;
+        const int L = __ldg(seq_lens + d.s);
+        d.P = L - d.n;
+        const int rows_tok = min(2 * tq, d.n - d.t0);
+        d.kv_end = causal ? d.P + d.t0 + rows_tok : L;
+        d.T = (d.kv_end + kPuTok - 1) / kPuTok;
+        return d.T > 0;
+    };
+    for (int64_t i = tid; i < total; i += kPlanBuckets) {
+        PuDesc d;
+        if (unit_of(i, d)) atomicAdd(&hist[min(d.T, kPlanBuckets - 1)], Hkv);
+    }
+    __syncthreads();
+    // inclusive suffix sum: scan[b] = sum over b' >= b of hist[b']  (heaviest bucket first in the list)
+    const int mine = hist[tid];
+    scan[tid] = mine;
+    __syncthreads();
+    for (int off = 1; off < kPlanBuckets; off <<= 1) {
+        const int add = (tid + off < kPlanBuckets) ? scan[tid + off] : 0;
+        __syncthreads();
+        scan[tid] += add;
+        __syncthreads();
+    }
+    const int num_units = scan[0];
+    hist[tid] = scan[tid] - mine;  // cursor: first list position of bucket tid
+    __syncthreads();
+    PuDesc* list = reinterpret_cast<PuDesc*>(plan + kPlanHeaderInts);
+    for (int64_t i = tid; i < total; i += kPlanBuckets) {
+        PuDesc d;
+        if (unit_of(i, d)) {
+            const int pos = atomicAdd(&hist[min(d.T, kPlanBuckets - 1)], Hkv);
+            for (int h = 0; h < Hkv; ++h) {
+                d.kvh = h;
+                int4* dst = reinterpret_cast<int4*>(list + pos + h);
+                dst[0] = make_int4(d.s, d.kvh, d.t0, d.n);
+                dst[1] = make_int4(d.P, d.r0, d.kv_end, d.T);
+            }
+        }
+    }
+    if (tid == 0) {
+        plan[0] = 0;
+        plan[1] = 0;
+        plan[2] = num_units;
+    }
 }
 
 // shared memory map (offsets from the 1024-aligned base)
@@ -73,9 +132,43 @@ constexpr int kPuQ = 0;                     // 2 tiles x 2 halves
 constexpr int kPuK = 4 * kPuHT;             // 2 stages x 2 halves
 constexpr int kPuV = 8 * kPuHT;             // 2 stages x 2 halves
 constexpr int kPuBars = 12 * kPuHT;         // barriers
-constexpr int kPuSmemBytes = 12 * kPuHT + 256 + 1024;
-enum { B_QFULL = 0, B_QEMPTY, B_KFULL0, B_KFULL1, B_KEMPTY0, B_KEMPTY1, B_VFULL0, B_VFULL1, B_VEMPTY0, B_VEMPTY1,
-       B_SFULL0, B_SFULL1, B_PFULL0, B_PFULL1, B_OFULL0, B_OFULL1, B_OEMPTY0, B_OEMPTY1, B_COUNT };
+enum { B_QFULL0 = 0, B_QFULL1, B_QEMPTY0, B_QEMPTY1, B_KFULL0, B_KFULL1, B_KEMPTY0, B_KEMPTY1, B_VFULL0, B_VFULL1,
+       B_VEMPTY0, B_VEMPTY1, B_SFULL0, B_SFULL1, B_PFULL00, B_PFULL01, B_PFULL10, B_PFULL11, B_OFULL0, B_OFULL1,
+       B_OEMPTY0, B_OEMPTY1, B_UFULL0, B_UFULL1, B_UEMPTY0, B_UEMPTY1, B_COUNT };
+constexpr int kPuDesc = kPuBars + 256;      // 2 unit descriptors (32 B each)
+constexpr int kPuTmemSlot = kPuDesc + 64;
+constexpr int kPuSmemBytes = 12 * kPuHT + 512 + 1024;
+static_assert(B_COUNT * 8 <= 256, "barrier area");
+
+// packed fp32x2 helpers (FFMA2 / FADD2 on sm_100) and the 3-input max (FMNMX3)
+__device__ __forceinline__ void ffma2_bcast(float& d0, float& d1, float a0, float a1, float b, float c) {
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\t"
+        "mov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %4};\n\tmov.b64 rc, {%5, %5};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d0), "=f"(d1)
+        : "f"(a0), "f"(a1), "f"(b), "f"(c));
+}
+__device__ __forceinline__ void fadd2(float& d0, float& d1, float a0, float a1, float b0, float b1) {
+    asm("{\n\t.reg .b64 ra, rb, rd;\n\t"
+        "mov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
+        "add.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d0), "=f"(d1)
+        : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+__device__ __forceinline__ float fmax3(float a, float b, float c) {
+    float d;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
+
+__device__ __forceinline__ PuDesc pu_read_desc(const uint8_t* gbase, int uslot) {
+    const int4* src = reinterpret_cast<const int4*>(gbase + kPuDesc + uslot * 32);
+    const int4 a = src[0], b = src[1];
+    PuDesc d;
+    d.s = a.x; d.kvh = a.y; d.t0 = a.z; d.n = a.w;
+    d.P = b.x; d.r0 = b.y; d.kv_end = b.z; d.T = b.w;
+    return d;
+}
 
 template <int PAGE>
 __global__ void __launch_bounds__(kPuThreads, 1)
@@ -87,22 +180,25 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* gbase = smem_raw + (base - smem_u32(smem_raw));
     const uint32_t bars = base + kPuBars;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(gbase + kPuBars + B_COUNT * 8);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(gbase + kPuTmemSlot);
     auto bar = [&](int i) { return bars + 8u * i; };
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        mbar_init(bar(B_QFULL), 1);
-        mbar_init(bar(B_QEMPTY), 1);
         for (int i = 0; i < 2; ++i) {
+            mbar_init(bar(B_QFULL0 + i), 1);
+            mbar_init(bar(B_QEMPTY0 + i), 1);
             mbar_init(bar(B_KFULL0 + i), 1);
             mbar_init(bar(B_KEMPTY0 + i), 1);
             mbar_init(bar(B_VFULL0 + i), 1);
             mbar_init(bar(B_VEMPTY0 + i), 1);
             mbar_init(bar(B_SFULL0 + i), 1);
-            mbar_init(bar(B_PFULL0 + i), 4);
+            mbar_init(bar(B_PFULL00 + 2 * i), 4);
+            mbar_init(bar(B_PFULL00 + 2 * i + 1), 4);
             mbar_init(bar(B_OFULL0 + i), 1);
             mbar_init(bar(B_OEMPTY0 + i), 4);
+            mbar_init(bar(B_UFULL0 + i), 1);
+            mbar_init(bar(B_UEMPTY0 + i), 9);  // MMA warp + 8 softmax warps
         }
         fence_mbar_init();
     }
@@ -114,149 +210,224 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    const int total_units = p.nqb * p.S * p.Hkv;
     const int rows_used = p.tq * p.G;  // rows of a Q tile that carry (token, head) pairs
 
-    if (warp == 0) {
-        // =============================== TMA PRODUCER ===============================
-        prefetch_tensormap(&qmap);
-        prefetch_tensormap(&kmap);
-        prefetch_tensormap(&vmap);
-        const uint64_t pol_kv = policy_evict_last();   // K/V re-read by other query blocks of the sequence
-        const uint64_t pol_q = policy_evict_first();
-        // lane -> (K or V, page, half): PPS*2 ops for K on the low lanes, PPS*2 for V after them
-        constexpr int OPS1 = PPS * 2;
-        const int op_isv = lane / OPS1;
-        const int op_page = (lane % OPS1) / 2;
-        const int op_half = lane & 1;
-        const bool op_on = lane < 2 * OPS1;
-        uint32_t qph = 0, kvph = 0;
-        int slot = 0;
-        for (int u = blockIdx.x; u < total_units; u += gridDim.x) {
-            const PuUnit x = pu_unit(p, u);
-            if (!x.valid) continue;
-            mbar_wait(bar(B_QEMPTY), qph ^ 1);
-            if (lane == 0) mbar_arrive_expect_tx(bar(B_QFULL), (uint32_t)(4 * rows_used * 128));
-            __syncwarp();
-            if (lane < 4)  // (tile, half)
-                tma_load_3d(base + kPuQ + lane * kPuHT, &qmap, bar(B_QFULL), (lane & 1) * 64, x.kvh * p.G,
-                            x.r0 + x.t0 + (lane >> 1) * p.tq, pol_q);
-            qph ^= 1;
-            const int32_t* bt = p.block_table + (size_t)x.s * p.bt_stride;
-            for (int j = 0; j < x.T; ++j) {
-                const int rem = x.kv_end - j * kPuTok;
-                const int npg = min(PPS, (rem + PAGE - 1) / PAGE);
-                int pg = -1;
-                if (op_on && op_page < npg) pg = __ldg(bt + j * PPS + op_page);
-                const uint32_t bytes = (uint32_t)(npg * PAGE * D * 2);
-                mbar_wait(bar(B_KEMPTY0 + slot), kvph ^ 1);
-                if (lane == 0) mbar_arrive_expect_tx(bar(B_KFULL0 + slot), bytes);
-                __syncwarp();
-                if (pg >= 0 && !op_isv)
-                    tma_load_4d(base + kPuK + (slot * 2 + op_half) * kPuHT + op_page * (PAGE * 128), &kmap,
-                                bar(B_KFULL0 + slot), op_half * 64, 0, x.kvh, pg, pol_kv);
-                mbar_wait(bar(B_VEMPTY0 + slot), kvph ^ 1);
-                if (lane == 0) mbar_arrive_expect_tx(bar(B_VFULL0 + slot), bytes);
-                __syncwarp();
-                if (pg >= 0 && op_isv)
-                    tma_load_4d(base + kPuV + (slot * 2 + op_half) * kPuHT + op_page * (PAGE * 128), &vmap,
-                                bar(B_VFULL0 + slot), op_half * 64, 0, x.kvh, pg, pol_kv);
-                slot ^= 1;
-                if (slot == 0) kvph ^= 1;
-            }
-        }
-    } else if (warp == 1) {
-        // =============================== MMA ISSUER ===============================
-        const uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
-        const uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
-        uint32_t qph = 0, kph = 0, vph = 0, pph[2] = {0, 0}, oeph = 0;
-        int ks = 0, vs = 0;
-        auto issue_qk = [&](int t, int kslot) {
+    if (warp < 4) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        if (warp == 0) {
+            // =============================== TMA PRODUCER + SCHEDULER ===============================
+            prefetch_tensormap(&qmap);
+            prefetch_tensormap(&kmap);
+            prefetch_tensormap(&vmap);
+            const uint64_t pol_kv = policy_evict_last();   // K/V re-read by other query blocks of the sequence
+            const uint64_t pol_q = policy_evict_first();
+            // lane -> (K or V, page, half): PPS*2 ops for K on the low lanes, PPS*2 for V after them
+            constexpr int OPS1 = PPS * 2;
+            const int op_isv = lane / OPS1;
+            const int op_page = (lane % OPS1) / 2;
+            const int op_half = lane & 1;
+            const bool op_on = lane < 2 * OPS1;
+            const PuDesc* list = reinterpret_cast<const PuDesc*>(p.plan + kPlanHeaderInts);
+            // Lane 0 owns the scheduler state.  Fetches are pipelined two units deep: the atomic for unit
+            // u+2 and the descriptor load for unit u+1 are in flight while unit u's tiles are issued.
+            int num_units = 0, idx1 = 0;
+            int4 da = make_int4(0, 0, 0, 0), db = make_int4(0, 0, 0, 0);
             if (lane == 0) {
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    const uint64_t a = umma_desc_kmajor_sw128(base + kPuQ + (t * 2 + (k >> 2)) * kPuHT + (k & 3) * 32);
-                    const uint64_t b = umma_desc_kmajor_sw128(base + kPuK + (kslot * 2 + (k >> 2)) * kPuHT + (k & 3) * 32);
-                    umma_ss(tmem + t * 128, a, b, idesc_qk, k > 0);
-                }
-                umma_commit(bar(B_SFULL0 + t));
-            }
-        };
-        auto issue_pv = [&](int t, int vslot, bool acc) {
-            if (lane == 0) {
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    const uint64_t b = umma_desc_mnmajor_sw128(base + kPuV + vslot * 2 * kPuHT + k * 16 * 128, kPuHT);
-                    umma_ts(tmem + 256 + t * 128, tmem + t * 128 + k * 8, b, idesc_pv, (acc || k > 0) ? 1u : 0u);
+                num_units = *reinterpret_cast<volatile int32_t*>(p.plan + 2);
+                const int idx0 = atomicAdd(p.plan, 1);
+                idx1 = atomicAdd(p.plan, 1);
+                if (idx0 < num_units) {
+                    const int4* e = reinterpret_cast<const int4*>(list + idx0);
+                    da = __ldg(e);
+                    db = __ldg(e + 1);
                 }
             }
-        };
-        for (int u = blockIdx.x; u < total_units; u += gridDim.x) {
-            const PuUnit x = pu_unit(p, u);
-            if (!x.valid) continue;
-            const int T = x.T;
-            mbar_wait(bar(B_QFULL), qph);
-            qph ^= 1;
-            mbar_wait(bar(B_KFULL0 + ks), kph);
-            tc_fence_after();
-            issue_qk(0, ks);
-            issue_qk(1, ks);
-            if (lane == 0) {
-                umma_commit(bar(B_KEMPTY0 + ks));
-                if (T == 1) umma_commit(bar(B_QEMPTY));
-            }
-            ks ^= 1;
-            if (ks == 0) kph ^= 1;
-            for (int j = 0; j < T; ++j) {
-                mbar_wait(bar(B_VFULL0 + vs), vph);
-                if (j == T - 1) {
-                    // rows of the last V stage that hold no visible token (not loaded, or NaN poison) -> 0,
-                    // so that p = 0 there cannot produce 0 * NaN inside the MMA
-                    const int nvalid = x.kv_end - j * kPuTok;
-                    if (nvalid < kPuTok) {
-                        uint8_t* vg = gbase + kPuV + vs * 2 * kPuHT;
-                        for (int i = nvalid * 8 + lane; i < kPuTok * 8; i += 32) {  // 16-B chunks of 128-B rows
-                            *reinterpret_cast<int4*>(vg + i * 16) = make_int4(0, 0, 0, 0);
-                            *reinterpret_cast<int4*>(vg + kPuHT + i * 16) = make_int4(0, 0, 0, 0);
-                        }
-                        fence_proxy_async_smem();
-                        __syncwarp();
+            uint32_t qph[2] = {0, 0}, kvph = 0, uph = 0;
+            int slot = 0, uslot = 0;
+            while (true) {
+                mbar_wait(bar(B_UEMPTY0 + uslot), uph ^ 1);
+                if (lane == 0) {
+                    int4* dst = reinterpret_cast<int4*>(gbase + kPuDesc + uslot * 32);
+                    dst[0] = da;
+                    dst[1] = db;
+                    mbar_arrive(bar(B_UFULL0 + uslot));
+                }
+                __syncwarp();
+                const PuDesc x = pu_read_desc(gbase, uslot);
+                uslot ^= 1;
+                if (uslot == 0) uph ^= 1;
+                if (x.T == 0) break;
+                int idx2 = 0;
+                int4 na = make_int4(0, 0, 0, 0), nb = make_int4(0, 0, 0, 0);
+                if (lane == 0) {
+                    idx2 = atomicAdd(p.plan, 1);
+                    if (idx1 < num_units) {
+                        const int4* e = reinterpret_cast<const int4*>(list + idx1);
+                        na = __ldg(e);
+                        nb = __ldg(e + 1);
                     }
+                }
+                const int32_t* bt = p.block_table + (size_t)x.s * p.bt_stride;
+                int pg_next = -1;
+                {
+                    const int npg0 = min(PPS, (x.kv_end + PAGE - 1) / PAGE);
+                    if (op_on && op_page < npg0) pg_next = __ldg(bt + op_page);
                 }
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
-                    if (j == 0) mbar_wait(bar(B_OEMPTY0 + t), oeph ^ 1);
-                    mbar_wait(bar(B_PFULL0 + t), pph[t]);
-                    pph[t] ^= 1;
+                    mbar_wait(bar(B_QEMPTY0 + t), qph[t] ^ 1);
+                    qph[t] ^= 1;
+                    if (lane == 0) mbar_arrive_expect_tx(bar(B_QFULL0 + t), (uint32_t)(2 * rows_used * 128));
+                    __syncwarp();
+                    if (lane < 2)  // half
+                        tma_load_3d(base + kPuQ + (t * 2 + lane) * kPuHT, &qmap, bar(B_QFULL0 + t), lane * 64,
+                                    x.kvh * p.G, x.r0 + x.t0 + t * p.tq, pol_q);
+                }
+                for (int j = 0; j < x.T; ++j) {
+                    const int rem = x.kv_end - j * kPuTok;
+                    const int npg = min(PPS, (rem + PAGE - 1) / PAGE);
+                    const int pg = pg_next;
+                    pg_next = -1;
+                    if (j + 1 < x.T) {  // block-table entries of the next stage, one stage ahead
+                        const int npg1 = min(PPS, (rem - kPuTok + PAGE - 1) / PAGE);
+                        if (op_on && op_page < npg1) pg_next = __ldg(bt + (j + 1) * PPS + op_page);
+                    }
+                    const uint32_t bytes = (uint32_t)(npg * PAGE * D * 2);
+                    mbar_wait(bar(B_KEMPTY0 + slot), kvph ^ 1);
+                    if (lane == 0) mbar_arrive_expect_tx(bar(B_KFULL0 + slot), bytes);
+                    __syncwarp();
+                    if (pg >= 0 && !op_isv)
+                        tma_load_4d(base + kPuK + (slot * 2 + op_half) * kPuHT + op_page * (PAGE * 128), &kmap,
+                                    bar(B_KFULL0 + slot), op_half * 64, 0, x.kvh, pg, pol_kv);
+                    mbar_wait(bar(B_VEMPTY0 + slot), kvph ^ 1);
+                    if (lane == 0) mbar_arrive_expect_tx(bar(B_VFULL0 + slot), bytes);
+                    __syncwarp();
+                    if (pg >= 0 && op_isv)
+                        tma_load_4d(base + kPuV + (slot * 2 + op_half) * kPuHT + op_page * (PAGE * 128), &vmap,
+                                    bar(B_VFULL0 + slot), op_half * 64, 0, x.kvh, pg, pol_kv);
+                    slot ^= 1;
+                    if (slot == 0) kvph ^= 1;
+                }
+                da = na;
+                db = nb;
+                idx1 = idx2;
+            }
+            // Every fetch of this CTA has returned.  The last CTA out re-arms the plan (counter = 0), so the
+            // same plan serves the next launch (MSTAR_FLAG_PREFILL_REUSE_PLAN).
+            if (lane == 0) {
+                asm volatile("" ::"r"(idx1));
+                __threadfence();
+                const int done = atomicAdd(p.plan + 1, 1);
+                if (done == (int)gridDim.x - 1) {
+                    p.plan[0] = 0;
+                    p.plan[1] = 0;
+                }
+            }
+        } else if (warp == 1) {
+            // =============================== MMA ISSUER ===============================
+            const uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
+            const uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
+            uint32_t qph[2] = {0, 0}, kph = 0, vph = 0, pph[2] = {0, 0}, oeph = 0, uph = 0;
+            int ks = 0, vs = 0, uslot = 0;
+            auto issue_qk = [&](int t, int kslot) {
+                if (lane == 0) {
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const uint64_t a =
+                            umma_desc_kmajor_sw128(base + kPuQ + (t * 2 + (k >> 2)) * kPuHT + (k & 3) * 32);
+                        const uint64_t b =
+                            umma_desc_kmajor_sw128(base + kPuK + (kslot * 2 + (k >> 2)) * kPuHT + (k & 3) * 32);
+                        umma_ss(tmem + t * 128, a, b, idesc_qk, k > 0);
+                    }
+                    umma_commit(bar(B_SFULL0 + t));
+                }
+            };
+            auto issue_pv = [&](int t, int vslot, bool acc, int kbeg) {
+                if (lane == 0) {
+#pragma unroll
+                    for (int k = kbeg; k < kbeg + 4; ++k) {
+                        const uint64_t b =
+                            umma_desc_mnmajor_sw128(base + kPuV + vslot * 2 * kPuHT + k * 16 * 128, kPuHT);
+                        umma_ts(tmem + 256 + t * 128, tmem + t * 128 + k * 8, b, idesc_pv, (acc || k > 0) ? 1u : 0u);
+                    }
+                }
+            };
+            while (true) {
+                mbar_wait(bar(B_UFULL0 + uslot), uph);
+                const PuDesc x = pu_read_desc(gbase, uslot);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_UEMPTY0 + uslot));
+                uslot ^= 1;
+                if (uslot == 0) uph ^= 1;
+                if (x.T == 0) break;
+                const int T = x.T;
+                mbar_wait(bar(B_KFULL0 + ks), kph);
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    mbar_wait(bar(B_QFULL0 + t), qph[t]);
+                    qph[t] ^= 1;
                     tc_fence_after();
-                    issue_pv(t, vs, j > 0);
-                    if (lane == 0) {
-                        if (t == 1) umma_commit(bar(B_VEMPTY0 + vs));
-                        if (j == T - 1) umma_commit(bar(B_OFULL0 + t));
+                    issue_qk(t, ks);
+                    if (T == 1 && lane == 0) umma_commit(bar(B_QEMPTY0 + t));
+                }
+                if (lane == 0) umma_commit(bar(B_KEMPTY0 + ks));
+                ks ^= 1;
+                if (ks == 0) kph ^= 1;
+                for (int j = 0; j < T; ++j) {
+                    mbar_wait(bar(B_VFULL0 + vs), vph);
+                    if (j == T - 1) {
+                        // rows of the last V stage that hold no visible token (not loaded, or NaN poison) -> 0,
+                        // so that p = 0 there cannot produce 0 * NaN inside the MMA
+                        const int nvalid = x.kv_end - j * kPuTok;
+                        if (nvalid < kPuTok) {
+                            uint8_t* vg = gbase + kPuV + vs * 2 * kPuHT;
+                            for (int i = nvalid * 8 + lane; i < kPuTok * 8; i += 32) {  // 16-B chunks of 128-B rows
+                                *reinterpret_cast<int4*>(vg + i * 16) = make_int4(0, 0, 0, 0);
+                                *reinterpret_cast<int4*>(vg + kPuHT + i * 16) = make_int4(0, 0, 0, 0);
+                            }
+                            fence_proxy_async_smem();
+                            __syncwarp();
+                        }
+                    }
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        if (j == 0) mbar_wait(bar(B_OEMPTY0 + t), oeph ^ 1);
+                        mbar_wait(bar(B_PFULL00 + 2 * t), pph[t]);
+                        tc_fence_after();
+                        issue_pv(t, vs, j > 0, 0);
+                        mbar_wait(bar(B_PFULL00 + 2 * t + 1), pph[t]);
+                        pph[t] ^= 1;
+                        tc_fence_after();
+                        issue_pv(t, vs, true, 4);
+                        if (lane == 0) {
+                            if (t == 1) umma_commit(bar(B_VEMPTY0 + vs));
+                            if (j == T - 1) umma_commit(bar(B_OFULL0 + t));
+                        }
+                        if (j + 1 < T) {
+                            if (t == 0) {
+                                mbar_wait(bar(B_KFULL0 + ks), kph);
+                                tc_fence_after();
+                            }
+                            issue_qk(t, ks);
+                            if (lane == 0) {
+                                if (j + 1 == T - 1) umma_commit(bar(B_QEMPTY0 + t));
+                                if (t == 1) umma_commit(bar(B_KEMPTY0 + ks));
+                            }
+                        }
                     }
                     if (j + 1 < T) {
-                        if (t == 0) {
-                            mbar_wait(bar(B_KFULL0 + ks), kph);
-                            tc_fence_after();
-                        }
-                        issue_qk(t, ks);
-                        if (t == 1 && lane == 0) {
-                            umma_commit(bar(B_KEMPTY0 + ks));
-                            if (j + 1 == T - 1) umma_commit(bar(B_QEMPTY));
-                        }
+                        ks ^= 1;
+                        if (ks == 0) kph ^= 1;
                     }
+                    vs ^= 1;
+                    if (vs == 0) vph ^= 1;
                 }
-                if (j + 1 < T) {
-                    ks ^= 1;
-                    if (ks == 0) kph ^= 1;
-                }
-                vs ^= 1;
-                if (vs == 0) vph ^= 1;
+                oeph ^= 1;
             }
-            oeph ^= 1;
         }
-    } else if (warp >= 4) {
+    } else {
         // =============================== SOFTMAX / EPILOGUE WARPGROUPS ===============================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
         const int t = (warp - 4) >> 2;            // Q tile of this warpgroup
         const int row = ((warp & 3) << 5) | lane;  // TMEM lane = Q tile row
         const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
@@ -264,36 +435,54 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
         const uint32_t o_addr = tmem + lane_addr + 256 + t * 128;
         const int tok_l = row / p.G, head_l = row - tok_l * p.G;
         const float c = p.scale_log2;
-        uint32_t sph = 0, oph = 0;
-        for (int u = blockIdx.x; u < total_units; u += gridDim.x) {
-            const PuUnit x = pu_unit(p, u);
-            if (!x.valid) continue;
+        uint32_t sph = 0, oph = 0, uph = 0;
+        int uslot = 0;
+        while (true) {
+            mbar_wait(bar(B_UFULL0 + uslot), uph);
+            const PuDesc x = pu_read_desc(gbase, uslot);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_UEMPTY0 + uslot));
+            uslot ^= 1;
+            if (uslot == 0) uph ^= 1;
+            if (x.T == 0) break;
             const int tok = x.t0 + t * p.tq + tok_l;  // query token within the sequence
             const bool row_ok = row < rows_used && tok < x.n;
             // last visible KV position of this row (rows that are not stored follow the unit bound)
-            const int lim = min(p.causal ? x.P + tok : x.L - 1, x.kv_end - 1);
+            const int lim = p.causal ? min(x.P + tok, x.kv_end - 1) : x.kv_end - 1;
             float m_ref = -INFINITY, l = 0.f;
             for (int j = 0; j < x.T; ++j) {
                 const int j0 = j * kPuTok;
-                const bool need_mask = j0 + kPuTok - 1 > lim;
                 mbar_wait(bar(B_SFULL0 + t), sph);
                 sph ^= 1;
                 tc_fence_after();
-                // ---- pass 1: row max
-                float mx = -INFINITY;
-#pragma unroll
-                for (int cb = 0; cb < 4; ++cb) {
-                    uint32_t r[32];
-                    tmem_ld_32x32b_x32(s_addr + cb * 32, r);
+                uint32_t r[128];
+                {
+                    uint32_t(&r0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[0]);
+                    uint32_t(&r1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[32]);
+                    uint32_t(&r2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[64]);
+                    uint32_t(&r3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[96]);
+                    tmem_ld_32x32b_x32(s_addr, r0);
+                    tmem_ld_32x32b_x32(s_addr + 32, r1);
+                    tmem_ld_32x32b_x32(s_addr + 64, r2);
+                    tmem_ld_32x32b_x32(s_addr + 96, r3);
                     tmem_wait_ld();
-                    if (need_mask) {
-#pragma unroll
-                        for (int i = 0; i < 32; ++i)
-                            if (j0 + cb * 32 + i > lim) r[i] = 0xff800000u;  // -inf
-                    }
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(r[i]));
                 }
+                // ---- mask (diagonal / last stages only; warp-uniform branch)
+                if (__any_sync(0xffffffffu, j0 + kPuTok - 1 > lim)) {
+                    const int rel = lim - j0;  // columns i > rel are invisible to this row
+#pragma unroll
+                    for (int i = 0; i < 128; ++i)
+                        if (i > rel) r[i] = 0xff800000u;  // -inf
+                }
+                // ---- row max (3-input max, two chains)
+                float mxa = fmax3(__uint_as_float(r[0]), __uint_as_float(r[1]), __uint_as_float(r[2]));
+                float mxb = fmax3(__uint_as_float(r[3]), __uint_as_float(r[4]), __uint_as_float(r[5]));
+#pragma unroll
+                for (int i = 6; i < 126; i += 4) {
+                    mxa = fmax3(mxa, __uint_as_float(r[i]), __uint_as_float(r[i + 1]));
+                    mxb = fmax3(mxb, __uint_as_float(r[i + 2]), __uint_as_float(r[i + 3]));
+                }
+                const float mx = fmax3(mxa, mxb, fmaxf(__uint_as_float(r[126]), __uint_as_float(r[127])));
                 // ---- running max with lazy rescale of O (TMEM) and l
                 if (j == 0) {
                     m_ref = mx;
@@ -306,41 +495,45 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                         m_ref = m_new;
 #pragma unroll
                         for (int cb = 0; cb < 4; ++cb) {
-                            uint32_t r[32];
-                            tmem_ld_32x32b_x32(o_addr + cb * 32, r);
+                            uint32_t o[32];
+                            tmem_ld_32x32b_x32(o_addr + cb * 32, o);
                             tmem_wait_ld();
 #pragma unroll
-                            for (int i = 0; i < 32; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) * alpha);
-                            tmem_st_32x32b_x32(o_addr + cb * 32, r);
+                            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                            tmem_st_32x32b_x32(o_addr + cb * 32, o);
                         }
                         tmem_wait_st();
                     }
                 }
-                // ---- pass 2: p = 2^(s*c - m_ref*c), row sum, P -> bf16 -> TMEM (over the columns of S)
-                const float mc = m_ref * c;
+                // ---- p = 2^(s*c - m_ref*c), P -> bf16 -> TMEM (over the columns of S), two 64-column halves
+                const float nmc = -m_ref * c;
 #pragma unroll
-                for (int cb = 0; cb < 4; ++cb) {
-                    uint32_t r[32];
-                    tmem_ld_32x32b_x32(s_addr + cb * 32, r);
-                    tmem_wait_ld();
-                    uint32_t pk[16];
+                for (int h = 0; h < 2; ++h) {
+                    uint32_t pk[32];
 #pragma unroll
-                    for (int i = 0; i < 32; i += 2) {
-                        float p0 = fast_exp2(__uint_as_float(r[i]) * c - mc);
-                        float p1 = fast_exp2(__uint_as_float(r[i + 1]) * c - mc);
-                        if (need_mask) {
-                            if (j0 + cb * 32 + i > lim) p0 = 0.f;
-                            if (j0 + cb * 32 + i + 1 > lim) p1 = 0.f;
-                        }
-                        l += p0 + p1;
+                    for (int i = 0; i < 64; i += 2) {
+                        float x0, x1;
+                        ffma2_bcast(x0, x1, __uint_as_float(r[h * 64 + i]), __uint_as_float(r[h * 64 + i + 1]), c, nmc);
+                        const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
+                        r[h * 64 + i] = __float_as_uint(p0);
+                        r[h * 64 + i + 1] = __float_as_uint(p1);
                         pk[i >> 1] = pack_bf16x2(p0, p1);
                     }
-                    tmem_st_32x32b_x16(s_addr + cb * 16, pk);
+                    tmem_st_32x32b_x32(s_addr + h * 32, pk);
+                    tmem_wait_st();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(B_PFULL00 + 2 * t + h));
                 }
-                tmem_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar(B_PFULL0 + t));
+                // ---- row sum, after the hand-off (packed adds, four chains)
+                float s0 = __uint_as_float(r[0]), s1 = __uint_as_float(r[1]);
+                float s2 = __uint_as_float(r[2]), s3 = __uint_as_float(r[3]);
+#pragma unroll
+                for (int i = 4; i < 128; i += 4) {
+                    fadd2(s0, s1, s0, s1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]));
+                    fadd2(s2, s3, s2, s3, __uint_as_float(r[i + 2]), __uint_as_float(r[i + 3]));
+                }
+                l += (s0 + s1) + (s2 + s3);
             }
             // ---- epilogue: O / l -> out
             mbar_wait(bar(B_OFULL0 + t), oph);
@@ -348,39 +541,46 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             tc_fence_after();
             const float inv = 1.f / l;
             const size_t orow = ((size_t)(x.r0 + tok) * p.Hq + (size_t)x.kvh * p.G + head_l) * D;
-#pragma unroll
-            for (int cb = 0; cb < 4; ++cb) {
-                uint32_t r[32];
-                tmem_ld_32x32b_x32(o_addr + cb * 32, r);
+            uint32_t r[128];
+            {
+                uint32_t(&r0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[0]);
+                uint32_t(&r1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[32]);
+                uint32_t(&r2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[64]);
+                uint32_t(&r3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[96]);
+                tmem_ld_32x32b_x32(o_addr, r0);
+                tmem_ld_32x32b_x32(o_addr + 32, r1);
+                tmem_ld_32x32b_x32(o_addr + 64, r2);
+                tmem_ld_32x32b_x32(o_addr + 96, r3);
                 tmem_wait_ld();
-                if (row_ok) {
-                    if (p.out_f32) {
-                        float* o = reinterpret_cast<float*>(p.out) + orow + cb * 32;
-#pragma unroll
-                        for (int i = 0; i < 32; i += 4)
-                            *reinterpret_cast<float4*>(o + i) =
-                                make_float4(__uint_as_float(r[i]) * inv, __uint_as_float(r[i + 1]) * inv,
-                                            __uint_as_float(r[i + 2]) * inv, __uint_as_float(r[i + 3]) * inv);
-                    } else {
-                        uint16_t* o = reinterpret_cast<uint16_t*>(p.out) + orow + cb * 32;
-#pragma unroll
-                        for (int i = 0; i < 32; i += 8) {
-                            int4 v;
-                            v.x = (int)pack_bf16x2(__uint_as_float(r[i]) * inv, __uint_as_float(r[i + 1]) * inv);
-                            v.y = (int)pack_bf16x2(__uint_as_float(r[i + 2]) * inv, __uint_as_float(r[i + 3]) * inv);
-                            v.z = (int)pack_bf16x2(__uint_as_float(r[i + 4]) * inv, __uint_as_float(r[i + 5]) * inv);
-                            v.w = (int)pack_bf16x2(__uint_as_float(r[i + 6]) * inv, __uint_as_float(r[i + 7]) * inv);
-                            *reinterpret_cast<int4*>(o + i) = v;
-                        }
-                    }
-                }
             }
-            if (row_ok && p.lse)
-                p.lse[(size_t)(x.r0 + tok) * p.Hq + (size_t)x.kvh * p.G + head_l] =
-                    (m_ref * c + log2f(l)) * 0.6931471805599453f;
+            // O is in registers: the tensor core may start the next unit's P V on this tile
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_OEMPTY0 + t));
+            if (row_ok) {
+                if (p.out_f32) {
+                    float* o = reinterpret_cast<float*>(p.out) + orow;
+#pragma unroll
+                    for (int i = 0; i < 128; i += 4)
+                        *reinterpret_cast<float4*>(o + i) =
+                            make_float4(__uint_as_float(r[i]) * inv, __uint_as_float(r[i + 1]) * inv,
+                                        __uint_as_float(r[i + 2]) * inv, __uint_as_float(r[i + 3]) * inv);
+                } else {
+                    uint16_t* o = reinterpret_cast<uint16_t*>(p.out) + orow;
+#pragma unroll
+                    for (int i = 0; i < 128; i += 8) {
+                        int4 v;
+                        v.x = (int)pack_bf16x2(__uint_as_float(r[i]) * inv, __uint_as_float(r[i + 1]) * inv);
+                        v.y = (int)pack_bf16x2(__uint_as_float(r[i + 2]) * inv, __uint_as_float(r[i + 3]) * inv);
+                        v.z = (int)pack_bf16x2(__uint_as_float(r[i + 4]) * inv, __uint_as_float(r[i + 5]) * inv);
+                        v.w = (int)pack_bf16x2(__uint_as_float(r[i + 6]) * inv, __uint_as_float(r[i + 7]) * inv);
+                        *reinterpret_cast<int4*>(o + i) = v;
+                    }
+                }
+                if (p.lse)
+                    p.lse[(size_t)(x.r0 + tok) * p.Hq + (size_t)x.kvh * p.G + head_l] =
+                        (m_ref * c + log2f(l)) * 0.6931471805599453f;
+            }
         }
     }
     tc_fence_before();
@@ -388,53 +588,68 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
     if (warp == 1) tmem_dealloc(tmem, 512);
 }
 
+size_t prefill_umma_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads) {
+    // header + one 32-byte descriptor per unit; units <= (total_q / (2 tq) + S) * Hkv <= total_q*Hq/128 + S*Hq
+    const int64_t units = ((int64_t)total_q * num_q_heads + 127) / 128 + (int64_t)num_seqs * num_q_heads + 1;
+    return (size_t)(kPlanHeaderInts * 4 + 32 * units);
+}
+
 int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, const int32_t* cu_seqlens_q,
                         const int32_t* block_table, int64_t bt_stride, const int32_t* seq_lens, int32_t S,
                         int32_t Hq, int32_t Hkv, int32_t page_size, int32_t max_q_len, float scale, int32_t causal,
-                        void* out, float* lse, int32_t out_f32, cudaStream_t stream) {
+                        void* out, float* lse, int32_t out_f32, int32_t reuse_plan, void* workspace,
+                        size_t workspace_bytes, cudaStream_t stream) {
     PrefillUmmaParams p{};
-    p.cu_seqlens_q = cu_seqlens_q;
     p.block_table = block_table;
     p.bt_stride = bt_stride;
-    p.seq_lens = seq_lens;
-    p.S = S;
+    p.plan = reinterpret_cast<int32_t*>(workspace);
     p.Hq = Hq;
-    p.Hkv = Hkv;
     p.G = Hq / Hkv;
     p.tq = 128 / p.G;
-    p.nqb = (max_q_len + 2 * p.tq - 1) / (2 * p.tq);
     p.scale_log2 = scale * 1.4426950408889634f;
     p.out = out;
     p.lse = lse;
     p.out_f32 = out_f32;
     p.causal = causal;
+    const int nqb = (max_q_len + 2 * p.tq - 1) / (2 * p.tq);
+    const int64_t max_units = ((int64_t)total_q / (2 * p.tq) + S) * Hkv;
+    if (!workspace || !aligned(workspace, 16)) return MSTAR_ERR_INVALID_ARG;
+    if (workspace_bytes < (size_t)(kPlanHeaderInts * 4 + 32 * max_units)) return MSTAR_ERR_WORKSPACE_TOO_SMALL;
+    if (max_units > 0x7fffffffLL || (int64_t)nqb * S > 0x7fffffffLL) return MSTAR_ERR_UNSUPPORTED;
     // Q view: dims (D, Hq, total_q); box (64, G, tq): rows of a tile = token * G + head
     CUtensorMap qmap;
     {
         typedef CUresult (*Fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-        void* fp = nullptr;
-        cudaDriverEntryPointQueryResult qr;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qr) != cudaSuccess ||
-            qr != cudaDriverEntryPointSuccess) {
-            (void)cudaGetLastError();
-            return MSTAR_ERR_CUDA;
+        static Fn encode = nullptr;
+        if (!encode) {
+            void* fp = nullptr;
+            cudaDriverEntryPointQueryResult qr;
+            if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qr) != cudaSuccess ||
+                qr != cudaDriverEntryPointSuccess) {
+                (void)cudaGetLastError();
+                return MSTAR_ERR_CUDA;
+            }
+            encode = reinterpret_cast<Fn>(fp);
         }
         cuuint64_t dims[3] = {128, (cuuint64_t)Hq, (cuuint64_t)total_q};
         cuuint64_t strides[2] = {256, (cuuint64_t)Hq * 256};
         cuuint32_t box[3] = {64, (cuuint32_t)p.G, (cuuint32_t)p.tq};
         cuuint32_t es[3] = {1, 1, 1};
-        if (reinterpret_cast<Fn>(fp)(&qmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), dims, strides,
-                                     box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        if (encode(&qmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), dims, strides, box, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
             return MSTAR_ERR_INVALID_ARG;
     }
-    const int64_t units = (int64_t)p.nqb * S * Hkv;
-    if (units > 0x7fffffffLL) return MSTAR_ERR_UNSUPPORTED;
+    if (!reuse_plan) {
+        prefill_plan_kernel<<<1, kPlanBuckets, 0, stream>>>(cu_seqlens_q, seq_lens, S, Hkv, p.tq, nqb, causal, p.plan);
+        MSTAR_CUDA_OK(cudaGetLastError());
+        launch_count_add(1);
+    }
     int grid = device_sm_count();
-    if (grid > units) grid = (int)units;
+    if (grid > max_units) grid = (int)max_units;
+    if (grid < 1) grid = 1;
     auto k16 = prefill_umma_kernel<16>;
     auto k32 = prefill_umma_kernel<32>;
     static bool attr_set = false;
