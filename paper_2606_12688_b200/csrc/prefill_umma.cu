@@ -65,6 +65,24 @@ struct PrefillUmmaParams {
     int32_t causal;
 };
 
+#ifdef MSTAR_PU_TRACE
+// Debug build only (-DMSTAR_PU_TRACE): CTA 0 records (clock, event) pairs per role.
+constexpr int kTraceCap = 4096;
+__device__ unsigned long long g_pu_trace[4][kTraceCap];
+__device__ int g_pu_trace_n[4];
+__device__ __forceinline__ void pu_trace(int role, int evt) {
+    if (blockIdx.x != 0 || (threadIdx.x & 31) != 0) return;
+    const int i = g_pu_trace_n[role];
+    if (i < kTraceCap) {
+        g_pu_trace[role][i] = ((unsigned long long)clock64() << 8) | (unsigned)evt;
+        g_pu_trace_n[role] = i + 1;
+    }
+}
+#define PU_TRACE(role, evt) pu_trace(role, evt)
+#else
+#define PU_TRACE(role, evt)
+#endif
+
 // ------------------------------------------------------------------------------------------------ plan
 __global__ void __launch_bounds__(kPlanBuckets)
 prefill_plan_kernel(const int32_t* __restrict__ cu_seqlens_q, const int32_t* __restrict__ seq_lens, int S, int Hkv,
@@ -329,28 +347,37 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             const uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
             uint32_t qph[2] = {0, 0}, kph = 0, vph = 0, pph[2] = {0, 0}, oeph = 0, uph = 0;
             int ks = 0, vs = 0, uslot = 0;
+            // Descriptors differ only in the 14-bit start-address field (bytes >> 4) of their low word: the bases are
+            // built once, the per-instruction offsets are compile-time constants.
+            const uint64_t dq = umma_desc_kmajor_sw128(base + kPuQ);
+            const uint64_t dk = umma_desc_kmajor_sw128(base + kPuK);
+            const uint64_t dv = umma_desc_mnmajor_sw128(base + kPuV, kPuHT);
             auto issue_qk = [&](int t, int kslot) {
-                if (lane == 0) {
+                if (elect_one()) {
+                    const uint64_t a0 = dq + (uint64_t)(t * 2 * (kPuHT >> 4));
+                    const uint64_t b0 = dk + (uint64_t)(kslot * 2 * (kPuHT >> 4));
 #pragma unroll
                     for (int k = 0; k < 8; ++k) {
-                        const uint64_t a =
-                            umma_desc_kmajor_sw128(base + kPuQ + (t * 2 + (k >> 2)) * kPuHT + (k & 3) * 32);
-                        const uint64_t b =
-                            umma_desc_kmajor_sw128(base + kPuK + (kslot * 2 + (k >> 2)) * kPuHT + (k & 3) * 32);
-                        umma_ss(tmem + t * 128, a, b, idesc_qk, k > 0);
+                        const uint32_t off = (uint32_t)((k >> 2) * (kPuHT >> 4) + (k & 3) * 2);
+                        umma_ss(tmem + t * 128, a0 + off, b0 + off, idesc_qk, k > 0);
                     }
                     umma_commit(bar(B_SFULL0 + t));
                 }
+                __syncwarp();
             };
             auto issue_pv = [&](int t, int vslot, bool acc, int kbeg) {
-                if (lane == 0) {
+                if (elect_one()) {
+                    const uint64_t b0 = dv + (uint64_t)(vslot * 2 * (kPuHT >> 4));
 #pragma unroll
-                    for (int k = kbeg; k < kbeg + 4; ++k) {
-                        const uint64_t b =
-                            umma_desc_mnmajor_sw128(base + kPuV + vslot * 2 * kPuHT + k * 16 * 128, kPuHT);
-                        umma_ts(tmem + 256 + t * 128, tmem + t * 128 + k * 8, b, idesc_pv, (acc || k > 0) ? 1u : 0u);
-                    }
+                    for (int k = kbeg; k < kbeg + 4; ++k)
+                        umma_ts(tmem + 256 + t * 128, tmem + t * 128 + k * 8, b0 + (uint64_t)(k * 16 * 128 >> 4), idesc_pv,
+                                (acc || k > 0) ? 1u : 0u);
                 }
+                __syncwarp();
+            };
+            auto commit_if = [&](bool cond, int b) {
+                if (cond && elect_one()) umma_commit(bar(b));
+                __syncwarp();
             };
             while (true) {
                 mbar_wait(bar(B_UFULL0 + uslot), uph);
@@ -361,6 +388,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 if (uslot == 0) uph ^= 1;
                 if (x.T == 0) break;
                 const int T = x.T;
+                PU_TRACE(1, 1);
                 mbar_wait(bar(B_KFULL0 + ks), kph);
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
@@ -368,13 +396,14 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     qph[t] ^= 1;
                     tc_fence_after();
                     issue_qk(t, ks);
-                    if (T == 1 && lane == 0) umma_commit(bar(B_QEMPTY0 + t));
+                    commit_if(T == 1, B_QEMPTY0 + t);
                 }
-                if (lane == 0) umma_commit(bar(B_KEMPTY0 + ks));
+                commit_if(true, B_KEMPTY0 + ks);
                 ks ^= 1;
                 if (ks == 0) kph ^= 1;
                 for (int j = 0; j < T; ++j) {
                     mbar_wait(bar(B_VFULL0 + vs), vph);
+                    PU_TRACE(1, 17);
                     if (j == T - 1) {
                         // rows of the last V stage that hold no visible token (not loaded, or NaN poison) -> 0,
                         // so that p = 0 there cannot produce 0 * NaN inside the MMA
@@ -392,27 +421,28 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
 #pragma unroll
                     for (int t = 0; t < 2; ++t) {
                         if (j == 0) mbar_wait(bar(B_OEMPTY0 + t), oeph ^ 1);
+                        PU_TRACE(1, 10 + t);
                         mbar_wait(bar(B_PFULL00 + 2 * t), pph[t]);
+                        PU_TRACE(1, 12 + t);
                         tc_fence_after();
                         issue_pv(t, vs, j > 0, 0);
                         mbar_wait(bar(B_PFULL00 + 2 * t + 1), pph[t]);
+                        PU_TRACE(1, 14 + t);
                         pph[t] ^= 1;
                         tc_fence_after();
                         issue_pv(t, vs, true, 4);
-                        if (lane == 0) {
-                            if (t == 1) umma_commit(bar(B_VEMPTY0 + vs));
-                            if (j == T - 1) umma_commit(bar(B_OFULL0 + t));
-                        }
+                        commit_if(t == 1, B_VEMPTY0 + vs);
+                        commit_if(j == T - 1, B_OFULL0 + t);
                         if (j + 1 < T) {
                             if (t == 0) {
                                 mbar_wait(bar(B_KFULL0 + ks), kph);
                                 tc_fence_after();
+                                PU_TRACE(1, 16);
                             }
                             issue_qk(t, ks);
-                            if (lane == 0) {
-                                if (j + 1 == T - 1) umma_commit(bar(B_QEMPTY0 + t));
-                                if (t == 1) umma_commit(bar(B_KEMPTY0 + ks));
-                            }
+                            PU_TRACE(1, 18 + t);
+                            commit_if(j + 1 == T - 1, B_QEMPTY0 + t);
+                            commit_if(t == 1, B_KEMPTY0 + ks);
                         }
                     }
                     if (j + 1 < T) {
@@ -452,7 +482,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             float m_ref = -INFINITY, l = 0.f;
             for (int j = 0; j < x.T; ++j) {
                 const int j0 = j * kPuTok;
+                if ((warp & 3) == 0) PU_TRACE(2 + t, 20);
                 mbar_wait(bar(B_SFULL0 + t), sph);
+                if ((warp & 3) == 0) PU_TRACE(2 + t, 21);
                 sph ^= 1;
                 tc_fence_after();
                 uint32_t r[128];
@@ -467,6 +499,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     tmem_ld_32x32b_x32(s_addr + 96, r3);
                     tmem_wait_ld();
                 }
+                if ((warp & 3) == 0) PU_TRACE(2 + t, 22);
                 // ---- mask (diagonal / last stages only; warp-uniform branch)
                 if (__any_sync(0xffffffffu, j0 + kPuTok - 1 > lim)) {
                     const int rel = lim - j0;  // columns i > rel are invisible to this row
@@ -505,6 +538,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                         tmem_wait_st();
                     }
                 }
+                if ((warp & 3) == 0) PU_TRACE(2 + t, 23);
                 // ---- p = 2^(s*c - m_ref*c), P -> bf16 -> TMEM (over the columns of S), two 64-column halves
                 const float nmc = -m_ref * c;
 #pragma unroll
@@ -524,6 +558,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_PFULL00 + 2 * t + h));
+                    if ((warp & 3) == 0) PU_TRACE(2 + t, 24 + h);
                 }
                 // ---- row sum, after the hand-off (packed adds, four chains)
                 float s0 = __uint_as_float(r[0]), s1 = __uint_as_float(r[1]);
@@ -536,6 +571,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 l += (s0 + s1) + (s2 + s3);
             }
             // ---- epilogue: O / l -> out
+            if ((warp & 3) == 0) PU_TRACE(2 + t, 30);
             mbar_wait(bar(B_OFULL0 + t), oph);
             oph ^= 1;
             tc_fence_after();
@@ -557,6 +593,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_OEMPTY0 + t));
+            if ((warp & 3) == 0) PU_TRACE(2 + t, 31);
             if (row_ok) {
                 if (p.out_f32) {
                     float* o = reinterpret_cast<float*>(p.out) + orow;
@@ -668,3 +705,14 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
 }
 
 }  // namespace mstar
+
+#ifdef MSTAR_PU_TRACE
+extern "C" int mstar_debug_pu_trace(unsigned long long* host_out, int* host_n) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(host_out, mstar::g_pu_trace, sizeof(unsigned long long) * 4 * mstar::kTraceCap);
+    cudaMemcpyFromSymbol(host_n, mstar::g_pu_trace_n, sizeof(int) * 4);
+    int z[4] = {0, 0, 0, 0};
+    cudaMemcpyToSymbol(mstar::g_pu_trace_n, z, sizeof(z));
+    return mstar::kTraceCap;
+}
+#endif

@@ -43,6 +43,19 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     }
 }
 
+// One lane of the (converged) warp returns true.  ptxas knows that the guarded region runs on a single lane,
+// so instructions that take uniform-register operands (UTCHMMA, UTMALDG, UTCBAR) are emitted straight-line
+// instead of inside a loop over the active lanes.
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
+
 // ---------------------------------------------------------------- TMA
 // L2 eviction-priority policies for streamed (read-once) and reused data.
 __device__ __forceinline__ uint64_t policy_evict_first() {
