@@ -8,17 +8,17 @@
 //                         work counter.
 //   prefill_umma_kernel   persistent CTAs (one per SM), 12 warps, units pulled from the plan with an atomic
 //                         counter (longest-processing-time-first, so the tail is one light unit):
-//     warp 0      TMA producer + scheduler: Q tiles (3-D boxes over [token][head][d]) and 128-token K / V stages
+//     warp 8      TMA producer + scheduler: Q tiles (3-D boxes over [token][head][d]) and 128-token K / V stages
 //                 gathered page by page through the block table (4-D boxes, 128-B swizzle), double-buffered;
-//     warp 1      MMA issuer (one elected lane): S = Q K^T (operands in shared memory) and O += P V (P read from
+//     warp 9      MMA issuer (one elected lane): S = Q K^T (operands in shared memory) and O += P V (P read from
 //                 TMEM, V MN-major from shared memory), M = 128, N = 128, K = 16 per instruction;
-//     warps 4-7   softmax warpgroup of Q tile A, warps 8-11 of Q tile B: thread = query row = TMEM lane.  The
+//     warps 0-3   softmax warpgroup of Q tile A, warps 4-7 of Q tile B: thread = query row = TMEM lane.  The
 //                 whole S row is pulled into registers once (tcgen05.ld), masked on diagonal stages only,
 //                 3-input max, packed f32x2 scale/subtract, ex2, bf16 pack, tcgen05.st over the columns S
 //                 occupied, handed to the MMA warp in two 64-column halves so P V starts while the second half
 //                 is still in the SFU; row sums are taken after the hand-off.  O is rescaled in TMEM only when
 //                 the running max grows by more than 2^8 (lazy rescale); epilogue O / l -> bf16 -> global.
-//   setmaxnreg moves registers from warps 0-3 (56) to the softmax warpgroups (224).
+//   setmaxnreg moves registers from warps 8-11 (88) to the softmax warpgroups (208).
 // A work unit is (sequence, kv head, block of 2*tq query tokens), tq = floor(128 / G): the G grouped query
 // heads of a kv head are packed into the 128 rows of a Q tile (row = token*G + head), so one K/V stage serves
 // all of them and the causal diagonal wastes at most tq columns.  The two Q tiles of a unit ping-pong: while
@@ -34,7 +34,11 @@
 namespace mstar {
 
 constexpr int kPuTok = 128;       // KV tokens per stage
-constexpr int kPuThreads = 384;   // 12 warps
+constexpr int kPuThreads = 384;   // 12 warps: 0-7 softmax, 8 TMA, 9 MMA (10, 11 only hand their registers over)
+// The warp scheduler of an SM sub-partition favours the highest warp id among its eligible warps (measured), so
+// the two latency-critical single-lane roles sit above the issue-heavy softmax warps that share their schedulers.
+constexpr int kPuTmaWarp = 8;
+constexpr int kPuMmaWarp = 9;
 constexpr int kPuHT = 128 * 128;  // bytes of a half tile: 128 rows x 64 bf16, 128-B swizzled
 constexpr float kPuTau = 8.0f;    // lazy-rescale threshold, log2 units
 constexpr int kPlanBuckets = 1024;
@@ -66,21 +70,33 @@ struct PrefillUmmaParams {
 };
 
 #ifdef MSTAR_PU_TRACE
-// Debug build only (-DMSTAR_PU_TRACE): CTA 0 records (clock, event) pairs per role.
-constexpr int kTraceCap = 4096;
-__device__ unsigned long long g_pu_trace[4][kTraceCap];
+// Debug build only (-DMSTAR_PU_TRACE): CTA 0 records (clock, event) words per role in spare shared memory and
+// copies them out when it exits.
+constexpr int kTraceCap = 2048;
+__device__ unsigned int g_pu_trace[4][kTraceCap];
 __device__ int g_pu_trace_n[4];
-__device__ __forceinline__ void pu_trace(int role, int evt) {
-    if (blockIdx.x != 0 || (threadIdx.x & 31) != 0) return;
-    const int i = g_pu_trace_n[role];
-    if (i < kTraceCap) {
-        g_pu_trace[role][i] = ((unsigned long long)clock64() << 8) | (unsigned)evt;
-        g_pu_trace_n[role] = i + 1;
-    }
-}
-#define PU_TRACE(role, evt) pu_trace(role, evt)
+#define PU_TRACE(role, evt)                                                                                       \
+    do {                                                                                                          \
+        if (pu_trace_on && pu_trace_n < kTraceCap)                                                                \
+            pu_trace_buf[(role)*kTraceCap + pu_trace_n++] = ((unsigned)clock() << 6) | (unsigned)(evt);           \
+    } while (0)
+#define PU_TRACE_DECL                                                                      \
+    int pu_trace_n = 0;                                                                    \
+    const bool pu_trace_on = blockIdx.x == 0 && (threadIdx.x & 31) == 0;                   \
+    unsigned* pu_trace_buf = reinterpret_cast<unsigned*>(gbase + 12 * kPuHT + 512);
+#define PU_TRACE_FLUSH(role)                                                               \
+    do {                                                                                   \
+        if (pu_trace_on) {                                                                 \
+            for (int i = 0; i < pu_trace_n; ++i) g_pu_trace[role][i] = pu_trace_buf[(role)*kTraceCap + i]; \
+            g_pu_trace_n[role] = pu_trace_n;                                               \
+        }                                                                                  \
+    } while (0)
+constexpr int kPuTraceBytes = 4 * kTraceCap * 4;
 #else
 #define PU_TRACE(role, evt)
+#define PU_TRACE_DECL
+#define PU_TRACE_FLUSH(role)
+constexpr int kPuTraceBytes = 0;
 #endif
 
 // ------------------------------------------------------------------------------------------------ plan
@@ -155,7 +171,7 @@ enum { B_QFULL0 = 0, B_QFULL1, B_QEMPTY0, B_QEMPTY1, B_KFULL0, B_KFULL1, B_KEMPT
        B_OEMPTY0, B_OEMPTY1, B_UFULL0, B_UFULL1, B_UEMPTY0, B_UEMPTY1, B_COUNT };
 constexpr int kPuDesc = kPuBars + 256;      // 2 unit descriptors (32 B each)
 constexpr int kPuTmemSlot = kPuDesc + 64;
-constexpr int kPuSmemBytes = 12 * kPuHT + 512 + 1024;
+constexpr int kPuSmemBytes = 12 * kPuHT + 512 + 1024 + kPuTraceBytes;
 static_assert(B_COUNT * 8 <= 256, "barrier area");
 
 // packed fp32x2 helpers (FFMA2 / FADD2 on sm_100) and the 3-input max (FMNMX3)
@@ -202,6 +218,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
     auto bar = [&](int i) { return bars + 8u * i; };
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    PU_TRACE_DECL
     if (threadIdx.x == 0) {
         for (int i = 0; i < 2; ++i) {
             mbar_init(bar(B_QFULL0 + i), 1);
@@ -220,7 +237,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
         }
         fence_mbar_init();
     }
-    if (warp == 1) {
+    if (warp == kPuMmaWarp) {
         tmem_alloc(smem_u32(tmem_slot), 512);
         tmem_relinquish();
     }
@@ -230,9 +247,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
     const uint32_t tmem = *tmem_slot;
     const int rows_used = p.tq * p.G;  // rows of a Q tile that carry (token, head) pairs
 
-    if (warp < 4) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
-        if (warp == 0) {
+    if (warp >= 8) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
+        if (warp == kPuTmaWarp) {
             // =============================== TMA PRODUCER + SCHEDULER ===============================
             prefetch_tensormap(&qmap);
             prefetch_tensormap(&kmap);
@@ -341,7 +358,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     p.plan[1] = 0;
                 }
             }
-        } else if (warp == 1) {
+        } else if (warp == kPuMmaWarp) {
             // =============================== MMA ISSUER ===============================
             const uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
             const uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
@@ -402,6 +419,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 ks ^= 1;
                 if (ks == 0) kph ^= 1;
                 for (int j = 0; j < T; ++j) {
+                    PU_TRACE(1, 46);
                     mbar_wait(bar(B_VFULL0 + vs), vph);
                     PU_TRACE(1, 17);
                     if (j == T - 1) {
@@ -426,15 +444,19 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                         PU_TRACE(1, 12 + t);
                         tc_fence_after();
                         issue_pv(t, vs, j > 0, 0);
+                        PU_TRACE(1, 40 + t);
                         mbar_wait(bar(B_PFULL00 + 2 * t + 1), pph[t]);
                         PU_TRACE(1, 14 + t);
                         pph[t] ^= 1;
                         tc_fence_after();
                         issue_pv(t, vs, true, 4);
+                        PU_TRACE(1, 42 + t);
                         commit_if(t == 1, B_VEMPTY0 + vs);
                         commit_if(j == T - 1, B_OFULL0 + t);
+                        PU_TRACE(1, 44 + t);
                         if (j + 1 < T) {
                             if (t == 0) {
+                                PU_TRACE(1, 47);
                                 mbar_wait(bar(B_KFULL0 + ks), kph);
                                 tc_fence_after();
                                 PU_TRACE(1, 16);
@@ -457,8 +479,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
         }
     } else {
         // =============================== SOFTMAX / EPILOGUE WARPGROUPS ===============================
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
-        const int t = (warp - 4) >> 2;            // Q tile of this warpgroup
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
+        const int t = warp >> 2;                   // Q tile of this warpgroup
         const int row = ((warp & 3) << 5) | lane;  // TMEM lane = Q tile row
         const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
         const uint32_t s_addr = tmem + lane_addr + t * 128;
@@ -620,9 +642,12 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             }
         }
     }
+    if (warp == kPuMmaWarp) PU_TRACE_FLUSH(1);
+    if (warp == 0) PU_TRACE_FLUSH(2);
+    if (warp == 4) PU_TRACE_FLUSH(3);
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) tmem_dealloc(tmem, 512);
+    if (warp == kPuMmaWarp) tmem_dealloc(tmem, 512);
 }
 
 size_t prefill_umma_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads) {
@@ -707,9 +732,9 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
 }  // namespace mstar
 
 #ifdef MSTAR_PU_TRACE
-extern "C" int mstar_debug_pu_trace(unsigned long long* host_out, int* host_n) {
+extern "C" int mstar_debug_pu_trace(unsigned int* host_out, int* host_n) {
     cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(host_out, mstar::g_pu_trace, sizeof(unsigned long long) * 4 * mstar::kTraceCap);
+    cudaMemcpyFromSymbol(host_out, mstar::g_pu_trace, sizeof(unsigned int) * 4 * mstar::kTraceCap);
     cudaMemcpyFromSymbol(host_n, mstar::g_pu_trace_n, sizeof(int) * 4);
     int z[4] = {0, 0, 0, 0};
     cudaMemcpyToSymbol(mstar::g_pu_trace_n, z, sizeof(z));
