@@ -70,33 +70,26 @@ struct PrefillUmmaParams {
 };
 
 #ifdef MSTAR_PU_TRACE
-// Debug build only (-DMSTAR_PU_TRACE): CTA 0 records (clock, event) words per role in spare shared memory and
-// copies them out when it exits.
+// Debug build only (-DMSTAR_PU_TRACE): CTA 0 records (clock, event) words per role.
 constexpr int kTraceCap = 2048;
 __device__ unsigned int g_pu_trace[4][kTraceCap];
 __device__ int g_pu_trace_n[4];
-#define PU_TRACE(role, evt)                                                                                       \
-    do {                                                                                                          \
-        if (pu_trace_on && pu_trace_n < kTraceCap)                                                                \
-            pu_trace_buf[(role)*kTraceCap + pu_trace_n++] = ((unsigned)clock() << 6) | (unsigned)(evt);           \
+#define PU_TRACE(role, evt)                                                                                 \
+    do {                                                                                                    \
+        if (pu_trace_on && pu_trace_n < kTraceCap)                                                          \
+            g_pu_trace[role][pu_trace_n++] = ((unsigned)clock() << 6) | (unsigned)(evt);                    \
     } while (0)
-#define PU_TRACE_DECL                                                                      \
-    int pu_trace_n = 0;                                                                    \
-    const bool pu_trace_on = blockIdx.x == 0 && (threadIdx.x & 31) == 0;                   \
-    unsigned* pu_trace_buf = reinterpret_cast<unsigned*>(gbase + 12 * kPuHT + 512);
-#define PU_TRACE_FLUSH(role)                                                               \
-    do {                                                                                   \
-        if (pu_trace_on) {                                                                 \
-            for (int i = 0; i < pu_trace_n; ++i) g_pu_trace[role][i] = pu_trace_buf[(role)*kTraceCap + i]; \
-            g_pu_trace_n[role] = pu_trace_n;                                               \
-        }                                                                                  \
+#define PU_TRACE_DECL   \
+    int pu_trace_n = 0; \
+    const bool pu_trace_on = blockIdx.x == 0 && (threadIdx.x & 31) == 0;
+#define PU_TRACE_FLUSH(role)                            \
+    do {                                                \
+        if (pu_trace_on) g_pu_trace_n[role] = pu_trace_n; \
     } while (0)
-constexpr int kPuTraceBytes = 4 * kTraceCap * 4;
 #else
 #define PU_TRACE(role, evt)
 #define PU_TRACE_DECL
 #define PU_TRACE_FLUSH(role)
-constexpr int kPuTraceBytes = 0;
 #endif
 
 // ------------------------------------------------------------------------------------------------ plan
@@ -165,13 +158,14 @@ prefill_plan_kernel(const int32_t* __restrict__ cu_seqlens_q, const int32_t* __r
 constexpr int kPuQ = 0;                     // 2 tiles x 2 halves
 constexpr int kPuK = 4 * kPuHT;             // 2 stages x 2 halves
 constexpr int kPuV = 8 * kPuHT;             // 2 stages x 2 halves
-constexpr int kPuBars = 12 * kPuHT;         // barriers
+constexpr int kPuO = 12 * kPuHT;            // 2 tiles x one 64-column half of the bf16 output (TMA-store staging)
+constexpr int kPuBars = 14 * kPuHT;         // barriers
 enum { B_QFULL0 = 0, B_QFULL1, B_QEMPTY0, B_QEMPTY1, B_KFULL0, B_KFULL1, B_KEMPTY0, B_KEMPTY1, B_VFULL0, B_VFULL1,
        B_VEMPTY0, B_VEMPTY1, B_SFULL0, B_SFULL1, B_PFULL00, B_PFULL01, B_PFULL10, B_PFULL11, B_OFULL0, B_OFULL1,
        B_OEMPTY0, B_OEMPTY1, B_UFULL0, B_UFULL1, B_UEMPTY0, B_UEMPTY1, B_COUNT };
 constexpr int kPuDesc = kPuBars + 256;      // 2 unit descriptors (32 B each)
 constexpr int kPuTmemSlot = kPuDesc + 64;
-constexpr int kPuSmemBytes = 12 * kPuHT + 512 + 1024 + kPuTraceBytes;
+constexpr int kPuSmemBytes = 14 * kPuHT + 512 + 1024;
 static_assert(B_COUNT * 8 <= 256, "barrier area");
 
 // packed fp32x2 helpers (FFMA2 / FADD2 on sm_100) and the 3-input max (FMNMX3)
@@ -207,7 +201,8 @@ __device__ __forceinline__ PuDesc pu_read_desc(const uint8_t* gbase, int uslot) 
 template <int PAGE>
 __global__ void __launch_bounds__(kPuThreads, 1)
 prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUtensorMap kmap,
-                    const __grid_constant__ CUtensorMap vmap, const PrefillUmmaParams p) {
+                    const __grid_constant__ CUtensorMap vmap, const __grid_constant__ CUtensorMap omap,
+                    const PrefillUmmaParams p) {
     constexpr int D = 128;
     constexpr int PPS = kPuTok / PAGE;  // pages per stage
     extern __shared__ uint8_t smem_raw[];
@@ -616,6 +611,36 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_OEMPTY0 + t));
             if ((warp & 3) == 0) PU_TRACE(2 + t, 31);
+            // Full tiles of bf16 output leave through shared memory and one TMA store per 64-column half (the
+            // box of the Q load, so rows land at (token, head)); per-thread row stores would be 32 scattered
+            // 16-byte writes per instruction.  Ragged tail tiles and the fp32 diagnostic output go direct.
+            const bool via_tma = !p.out_f32 && x.t0 + (t + 1) * p.tq <= x.n;
+            if (via_tma) {
+                const uint32_t obuf = base + kPuO + t * kPuHT;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    // the previous store out of this buffer must have finished reading it
+                    if ((warp & 3) == 0 && lane == 0) bulk_wait_group_read0();
+                    named_bar_sync(1 + t, 128);
+                    if (row < rows_used) {
+#pragma unroll
+                        for (int c8 = 0; c8 < 8; ++c8) {
+                            const int i = h * 64 + c8 * 8;
+                            st_shared_v4(obuf + swz128(row, c8),
+                                         pack_bf16x2(__uint_as_float(r[i]) * inv, __uint_as_float(r[i + 1]) * inv),
+                                         pack_bf16x2(__uint_as_float(r[i + 2]) * inv, __uint_as_float(r[i + 3]) * inv),
+                                         pack_bf16x2(__uint_as_float(r[i + 4]) * inv, __uint_as_float(r[i + 5]) * inv),
+                                         pack_bf16x2(__uint_as_float(r[i + 6]) * inv, __uint_as_float(r[i + 7]) * inv));
+                        }
+                    }
+                    fence_proxy_async_smem();
+                    named_bar_sync(1 + t, 128);
+                    if ((warp & 3) == 0 && lane == 0) {
+                        tma_store_3d(&omap, obuf, h * 64, x.kvh * p.G, x.r0 + x.t0 + t * p.tq);
+                        bulk_commit_group();
+                    }
+                }
+            }
             if (row_ok) {
                 if (p.out_f32) {
                     float* o = reinterpret_cast<float*>(p.out) + orow;
@@ -624,7 +649,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                         *reinterpret_cast<float4*>(o + i) =
                             make_float4(__uint_as_float(r[i]) * inv, __uint_as_float(r[i + 1]) * inv,
                                         __uint_as_float(r[i + 2]) * inv, __uint_as_float(r[i + 3]) * inv);
-                } else {
+                } else if (!via_tma) {
                     uint16_t* o = reinterpret_cast<uint16_t*>(p.out) + orow;
 #pragma unroll
                     for (int i = 0; i < 128; i += 8) {
@@ -642,12 +667,40 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             }
         }
     }
+    if (warp < 8 && (warp & 3) == 0 && lane == 0) bulk_wait_group0();  // output stores issued by this thread
     if (warp == kPuMmaWarp) PU_TRACE_FLUSH(1);
     if (warp == 0) PU_TRACE_FLUSH(2);
     if (warp == 4) PU_TRACE_FLUSH(3);
     tc_fence_before();
     __syncthreads();
     if (warp == kPuMmaWarp) tmem_dealloc(tmem, 512);
+}
+
+// 3-D view (D, Hq, total_q) of a [total_q][Hq][128] bf16 tensor with box (64, G, tq) and 128-byte swizzle
+static int make_q_view_map(const void* ptr, int32_t total_q, int32_t Hq, int32_t G, int32_t tq, CUtensorMap* out) {
+    typedef CUresult (*Fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                           const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                           CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static Fn encode = nullptr;
+    if (!encode) {
+        void* fp = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qr) != cudaSuccess ||
+            qr != cudaDriverEntryPointSuccess) {
+            (void)cudaGetLastError();
+            return MSTAR_ERR_CUDA;
+        }
+        encode = reinterpret_cast<Fn>(fp);
+    }
+    cuuint64_t dims[3] = {128, (cuuint64_t)Hq, (cuuint64_t)total_q};
+    cuuint64_t strides[2] = {256, (cuuint64_t)Hq * 256};
+    cuuint32_t box[3] = {64, (cuuint32_t)G, (cuuint32_t)tq};
+    cuuint32_t es[3] = {1, 1, 1};
+    if (encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, es,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return MSTAR_ERR_INVALID_ARG;
+    return MSTAR_OK;
 }
 
 size_t prefill_umma_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads) {
@@ -681,28 +734,14 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
     // Q view: dims (D, Hq, total_q); box (64, G, tq): rows of a tile = token * G + head
     CUtensorMap qmap;
     {
-        typedef CUresult (*Fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                               const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                               CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-        static Fn encode = nullptr;
-        if (!encode) {
-            void* fp = nullptr;
-            cudaDriverEntryPointQueryResult qr;
-            if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qr) != cudaSuccess ||
-                qr != cudaDriverEntryPointSuccess) {
-                (void)cudaGetLastError();
-                return MSTAR_ERR_CUDA;
-            }
-            encode = reinterpret_cast<Fn>(fp);
-        }
-        cuuint64_t dims[3] = {128, (cuuint64_t)Hq, (cuuint64_t)total_q};
-        cuuint64_t strides[2] = {256, (cuuint64_t)Hq * 256};
-        cuuint32_t box[3] = {64, (cuuint32_t)p.G, (cuuint32_t)p.tq};
-        cuuint32_t es[3] = {1, 1, 1};
-        if (encode(&qmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), dims, strides, box, es,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-            return MSTAR_ERR_INVALID_ARG;
+        const int st = make_q_view_map(q, total_q, Hq, p.G, p.tq, &qmap);
+        if (st != MSTAR_OK) return st;
+    }
+    // output view for the TMA-store epilogue: same geometry as the Q view (bf16 output only)
+    CUtensorMap omap = qmap;
+    if (!out_f32) {
+        const int st = make_q_view_map(out, total_q, Hq, p.G, p.tq, &omap);
+        if (st != MSTAR_OK) return st;
     }
     if (!reuse_plan) {
         prefill_plan_kernel<<<1, kPlanBuckets, 0, stream>>>(cu_seqlens_q, seq_lens, S, Hkv, p.tq, nqb, causal, p.plan);
@@ -721,9 +760,9 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
         attr_set = true;
     }
     if (page_size == 16)
-        k16<<<grid, kPuThreads, kPuSmemBytes, stream>>>(qmap, maps.k, maps.v, p);
+        k16<<<grid, kPuThreads, kPuSmemBytes, stream>>>(qmap, maps.k, maps.v, omap, p);
     else
-        k32<<<grid, kPuThreads, kPuSmemBytes, stream>>>(qmap, maps.k, maps.v, p);
+        k32<<<grid, kPuThreads, kPuSmemBytes, stream>>>(qmap, maps.k, maps.v, omap, p);
     MSTAR_CUDA_OK(cudaGetLastError());
     launch_count_add(1);
     return MSTAR_OK;
