@@ -41,6 +41,10 @@ constexpr int kPuTmaWarp = 8;
 constexpr int kPuMmaWarp = 9;
 constexpr int kPuHT = 128 * 128;  // bytes of a half tile: 128 rows x 64 bf16, 128-B swizzled
 constexpr float kPuTau = 8.0f;    // lazy-rescale threshold, log2 units
+#ifndef MSTAR_PU_EMU
+#define MSTAR_PU_EMU 0
+#endif
+constexpr int kPuEmu = MSTAR_PU_EMU;  // of every 4 score pairs, this many take 2^x on the FMA pipe, the rest on the SFU
 constexpr int kPlanBuckets = 1024;
 constexpr int kPlanHeaderInts = 8;  // [0] work counter  [1] CTAs done  [2] number of units
 
@@ -74,6 +78,14 @@ struct PrefillUmmaParams {
 constexpr int kTraceCap = 2048;
 __device__ unsigned int g_pu_trace[4][kTraceCap];
 __device__ int g_pu_trace_n[4];
+// per CTA: globaltimer at entry, at the first unit, at exit; units and KV stages processed
+__device__ unsigned long long g_pu_cta[160][5];
+__device__ __forceinline__ unsigned long long pu_gtime() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+#define PU_CTA(i, v) do { if ((threadIdx.x & 31) == 0 && blockIdx.x < 160) g_pu_cta[blockIdx.x][i] = (v); } while (0)
 #define PU_TRACE(role, evt)                                                                                 \
     do {                                                                                                    \
         if (pu_trace_on && pu_trace_n < kTraceCap)                                                          \
@@ -87,6 +99,7 @@ __device__ int g_pu_trace_n[4];
         if (pu_trace_on) g_pu_trace_n[role] = pu_trace_n; \
     } while (0)
 #else
+#define PU_CTA(i, v)
 #define PU_TRACE(role, evt)
 #define PU_TRACE_DECL
 #define PU_TRACE_FLUSH(role)
@@ -183,6 +196,43 @@ __device__ __forceinline__ void fadd2(float& d0, float& d1, float a0, float a1, 
         : "=f"(d0), "=f"(d1)
         : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
 }
+// 2^x for a pair of arguments on the FMA / ALU pipes instead of the SFU (the SFU pipe, 16 ex2 per clock per SM,
+// costs as many cycles per score as the two MMAs around it): x = j + f with j = round(x), f in [-0.5, 0.5];
+// 2^f by a degree-3 minimax polynomial (relative error 7.5e-5, far below the bf16 rounding of P), 2^j by adding
+// j to the exponent field.  j is read from the low mantissa bits of x + 1.5 * 2^23.  x <= ~9 by construction
+// (running max, lazy rescale); clamped below at -126 (exponent field cannot wrap).
+__device__ __forceinline__ void exp2_poly2(float& p0, float& p1, float x0, float x1) {
+    x0 = fmaxf(x0, -126.f);
+    x1 = fmaxf(x1, -126.f);
+    uint32_t u0, u1;
+    asm("{\n\t.reg .b64 x, t, j, f, q, mg, nmg, mone, c3, c2, c1, c0;\n\t"
+        ".reg .b32 t0, t1, q0, q1;\n\t"
+        "mov.b64 x, {%2, %3};\n\t"
+        "mov.b64 mg, {%4, %4};\n\t"
+        "mov.b64 nmg, {%5, %5};\n\t"
+        "mov.b64 mone, {%6, %6};\n\t"
+        "mov.b64 c3, {%7, %7};\n\t"
+        "mov.b64 c2, {%8, %8};\n\t"
+        "mov.b64 c1, {%9, %9};\n\t"
+        "mov.b64 c0, {%10, %10};\n\t"
+        "add.rn.f32x2 t, x, mg;\n\t"
+        "add.rn.f32x2 j, t, nmg;\n\t"
+        "fma.rn.f32x2 f, j, mone, x;\n\t"
+        "fma.rn.f32x2 q, c3, f, c2;\n\t"
+        "fma.rn.f32x2 q, q, f, c1;\n\t"
+        "fma.rn.f32x2 q, q, f, c0;\n\t"
+        "mov.b64 {t0, t1}, t;\n\t"
+        "mov.b64 {q0, q1}, q;\n\t"
+        "shl.b32 t0, t0, 23;\n\t"
+        "shl.b32 t1, t1, 23;\n\t"
+        "add.u32 %0, q0, t0;\n\t"
+        "add.u32 %1, q1, t1;\n\t}"
+        : "=r"(u0), "=r"(u1)
+        : "f"(x0), "f"(x1), "f"(12582912.f), "f"(-12582912.f), "f"(-1.f), "f"(0.0551716648042202f),
+          "f"(0.2426111251115799f), "f"(0.6932609677314758f), "f"(0.9999280571937561f));
+    p0 = __uint_as_float(u0);
+    p1 = __uint_as_float(u1);
+}
 __device__ __forceinline__ float fmax3(float a, float b, float c) {
     float d;
     asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
@@ -259,13 +309,16 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             const bool op_on = lane < 2 * OPS1;
             const PuDesc* list = reinterpret_cast<const PuDesc*>(p.plan + kPlanHeaderInts);
             // Lane 0 owns the scheduler state.  Fetches are pipelined two units deep: the atomic for unit
-            // u+2 and the descriptor load for unit u+1 are in flight while unit u's tiles are issued.
+            // u+2 and the descriptor load for unit u+1 are in flight while unit u's tiles are issued.  The first
+            // two units of a CTA are fixed (list is sorted heaviest first): rank b and rank 2*grid-1-b, so the
+            // CTA that got the heaviest unit of the first round gets the lightest of the second; everything
+            // after comes from the shared counter.
             int num_units = 0, idx1 = 0;
             int4 da = make_int4(0, 0, 0, 0), db = make_int4(0, 0, 0, 0);
             if (lane == 0) {
                 num_units = *reinterpret_cast<volatile int32_t*>(p.plan + 2);
-                const int idx0 = atomicAdd(p.plan, 1);
-                idx1 = atomicAdd(p.plan, 1);
+                const int idx0 = (int)blockIdx.x;
+                idx1 = 2 * (int)gridDim.x - 1 - (int)blockIdx.x;
                 if (idx0 < num_units) {
                     const int4* e = reinterpret_cast<const int4*>(list + idx0);
                     da = __ldg(e);
@@ -290,7 +343,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 int idx2 = 0;
                 int4 na = make_int4(0, 0, 0, 0), nb = make_int4(0, 0, 0, 0);
                 if (lane == 0) {
-                    idx2 = atomicAdd(p.plan, 1);
+                    idx2 = 2 * (int)gridDim.x + atomicAdd(p.plan, 1);
                     if (idx1 < num_units) {
                         const int4* e = reinterpret_cast<const int4*>(list + idx1);
                         na = __ldg(e);
@@ -358,6 +411,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             const uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
             const uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
             uint32_t qph[2] = {0, 0}, kph = 0, vph = 0, pph[2] = {0, 0}, oeph = 0, uph = 0;
+#ifdef MSTAR_PU_TRACE
+            unsigned long long cta_units = 0, cta_stages = 0;
+            PU_CTA(0, pu_gtime());
+#endif
             int ks = 0, vs = 0, uslot = 0;
             // Descriptors differ only in the 14-bit start-address field (bytes >> 4) of their low word: the bases are
             // built once, the per-instruction offsets are compile-time constants.
@@ -401,6 +458,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 if (x.T == 0) break;
                 const int T = x.T;
                 PU_TRACE(1, 1);
+#ifdef MSTAR_PU_TRACE
+                if (cta_units == 0) PU_CTA(1, pu_gtime());
+                ++cta_units;
+                cta_stages += T;
+#endif
                 mbar_wait(bar(B_KFULL0 + ks), kph);
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
@@ -471,6 +533,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 }
                 oeph ^= 1;
             }
+#ifdef MSTAR_PU_TRACE
+            PU_CTA(2, pu_gtime());
+            PU_CTA(3, cta_units);
+            PU_CTA(4, cta_stages);
+#endif
         }
     } else {
         // =============================== SOFTMAX / EPILOGUE WARPGROUPS ===============================
@@ -565,7 +632,13 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     for (int i = 0; i < 64; i += 2) {
                         float x0, x1;
                         ffma2_bcast(x0, x1, __uint_as_float(r[h * 64 + i]), __uint_as_float(r[h * 64 + i + 1]), c, nmc);
-                        const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
+                        float p0, p1;
+                        if (((i >> 1) & 3) < kPuEmu) {
+                            exp2_poly2(p0, p1, x0, x1);
+                        } else {
+                            p0 = fast_exp2(x0);
+                            p1 = fast_exp2(x1);
+                        }
                         r[h * 64 + i] = __float_as_uint(p0);
                         r[h * 64 + i + 1] = __float_as_uint(p1);
                         pk[i >> 1] = pack_bf16x2(p0, p1);
@@ -778,5 +851,10 @@ extern "C" int mstar_debug_pu_trace(unsigned int* host_out, int* host_n) {
     int z[4] = {0, 0, 0, 0};
     cudaMemcpyToSymbol(mstar::g_pu_trace_n, z, sizeof(z));
     return mstar::kTraceCap;
+}
+extern "C" int mstar_debug_pu_cta(unsigned long long* host_out) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(host_out, mstar::g_pu_cta, sizeof(unsigned long long) * 160 * 5);
+    return 160;
 }
 #endif
