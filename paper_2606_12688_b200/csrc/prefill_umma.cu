@@ -40,6 +40,7 @@ constexpr int kPuThreads = 384;   // 12 warps: 0-7 softmax, 8 TMA, 9 MMA (10, 11
 constexpr int kPuTmaWarp = 8;
 constexpr int kPuMmaWarp = 9;
 constexpr int kPuHT = 128 * 128;  // bytes of a half tile: 128 rows x 64 bf16, 128-B swizzled
+constexpr int kPuSplit = 96;      // keys of a stage in the first P hand-off (the second carries the rest)
 constexpr float kPuTau = 8.0f;    // lazy-rescale threshold, log2 units
 #ifndef MSTAR_PU_EMU
 #define MSTAR_PU_EMU 0
@@ -434,11 +435,12 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 }
                 __syncwarp();
             };
-            auto issue_pv = [&](int t, int vslot, bool acc, int kbeg) {
+            auto issue_pv = [&](int t, int vslot, bool acc, bool second) {
                 if (elect_one()) {
                     const uint64_t b0 = dv + (uint64_t)(vslot * 2 * (kPuHT >> 4));
+                    const int kbeg = second ? kPuSplit / 16 : 0, kend = second ? 8 : kPuSplit / 16;
 #pragma unroll
-                    for (int k = kbeg; k < kbeg + 4; ++k)
+                    for (int k = kbeg; k < kend; ++k)
                         umma_ts(tmem + 256 + t * 128, tmem + t * 128 + k * 8, b0 + (uint64_t)(k * 16 * 128 >> 4), idesc_pv,
                                 (acc || k > 0) ? 1u : 0u);
                 }
@@ -500,13 +502,13 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                         mbar_wait(bar(B_PFULL00 + 2 * t), pph[t]);
                         PU_TRACE(1, 12 + t);
                         tc_fence_after();
-                        issue_pv(t, vs, j > 0, 0);
+                        issue_pv(t, vs, j > 0, false);
                         PU_TRACE(1, 40 + t);
                         mbar_wait(bar(B_PFULL00 + 2 * t + 1), pph[t]);
                         PU_TRACE(1, 14 + t);
                         pph[t] ^= 1;
                         tc_fence_after();
-                        issue_pv(t, vs, true, 4);
+                        issue_pv(t, vs, true, true);
                         PU_TRACE(1, 42 + t);
                         commit_if(t == 1, B_VEMPTY0 + vs);
                         commit_if(j == T - 1, B_OFULL0 + t);
@@ -591,15 +593,21 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     for (int i = 0; i < 128; ++i)
                         if (i > rel) r[i] = 0xff800000u;  // -inf
                 }
-                // ---- row max (3-input max, two chains)
-                float mxa = fmax3(__uint_as_float(r[0]), __uint_as_float(r[1]), __uint_as_float(r[2]));
-                float mxb = fmax3(__uint_as_float(r[3]), __uint_as_float(r[4]), __uint_as_float(r[5]));
+                // ---- row max (3-input max, four chains)
+                float mx0 = fmax3(__uint_as_float(r[0]), __uint_as_float(r[1]), __uint_as_float(r[2]));
+                float mx1 = fmax3(__uint_as_float(r[3]), __uint_as_float(r[4]), __uint_as_float(r[5]));
+                float mx2 = fmax3(__uint_as_float(r[6]), __uint_as_float(r[7]), __uint_as_float(r[8]));
+                float mx3 = fmax3(__uint_as_float(r[9]), __uint_as_float(r[10]), __uint_as_float(r[11]));
 #pragma unroll
-                for (int i = 6; i < 126; i += 4) {
-                    mxa = fmax3(mxa, __uint_as_float(r[i]), __uint_as_float(r[i + 1]));
-                    mxb = fmax3(mxb, __uint_as_float(r[i + 2]), __uint_as_float(r[i + 3]));
+                for (int i = 12; i < 124; i += 8) {
+                    mx0 = fmax3(mx0, __uint_as_float(r[i]), __uint_as_float(r[i + 1]));
+                    mx1 = fmax3(mx1, __uint_as_float(r[i + 2]), __uint_as_float(r[i + 3]));
+                    mx2 = fmax3(mx2, __uint_as_float(r[i + 4]), __uint_as_float(r[i + 5]));
+                    mx3 = fmax3(mx3, __uint_as_float(r[i + 6]), __uint_as_float(r[i + 7]));
                 }
-                const float mx = fmax3(mxa, mxb, fmaxf(__uint_as_float(r[126]), __uint_as_float(r[127])));
+                mx0 = fmax3(mx0, __uint_as_float(r[124]), __uint_as_float(r[125]));
+                mx1 = fmax3(mx1, __uint_as_float(r[126]), __uint_as_float(r[127]));
+                const float mx = fmax3(fmaxf(mx0, mx1), mx2, mx3);
                 // ---- running max with lazy rescale of O (TMEM) and l
                 if (j == 0) {
                     m_ref = mx;
@@ -623,15 +631,15 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     }
                 }
                 if ((warp & 3) == 0) PU_TRACE(2 + t, 23);
-                // ---- p = 2^(s*c - m_ref*c), P -> bf16 -> TMEM (over the columns of S), two 64-column halves
+                // ---- p = 2^(s*c - m_ref*c), P -> bf16 -> TMEM (over the columns of S), handed over in two parts:
+                // the first kPuSplit keys, then the rest, so that little P V work is left after the last hand-off
                 const float nmc = -m_ref * c;
+                {
+                    uint32_t pk[kPuSplit / 2];
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    uint32_t pk[32];
-#pragma unroll
-                    for (int i = 0; i < 64; i += 2) {
+                    for (int i = 0; i < kPuSplit; i += 2) {
                         float x0, x1;
-                        ffma2_bcast(x0, x1, __uint_as_float(r[h * 64 + i]), __uint_as_float(r[h * 64 + i + 1]), c, nmc);
+                        ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), c, nmc);
                         float p0, p1;
                         if (((i >> 1) & 3) < kPuEmu) {
                             exp2_poly2(p0, p1, x0, x1);
@@ -639,16 +647,41 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                             p0 = fast_exp2(x0);
                             p1 = fast_exp2(x1);
                         }
-                        r[h * 64 + i] = __float_as_uint(p0);
-                        r[h * 64 + i + 1] = __float_as_uint(p1);
+                        r[i] = __float_as_uint(p0);
+                        r[i + 1] = __float_as_uint(p1);
                         pk[i >> 1] = pack_bf16x2(p0, p1);
                     }
-                    tmem_st_32x32b_x32(s_addr + h * 32, pk);
+                    tmem_st_32x32b_x32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
+                    tmem_st_32x32b_x16(s_addr + 32, *reinterpret_cast<uint32_t(*)[16]>(&pk[32]));
                     tmem_wait_st();
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(bar(B_PFULL00 + 2 * t + h));
-                    if ((warp & 3) == 0) PU_TRACE(2 + t, 24 + h);
+                    if (lane == 0) mbar_arrive(bar(B_PFULL00 + 2 * t));
+                    if ((warp & 3) == 0) PU_TRACE(2 + t, 24);
+                }
+                {
+                    uint32_t pk[(128 - kPuSplit) / 2];
+#pragma unroll
+                    for (int i = kPuSplit; i < 128; i += 2) {
+                        float x0, x1;
+                        ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), c, nmc);
+                        float p0, p1;
+                        if (((i >> 1) & 3) < kPuEmu) {
+                            exp2_poly2(p0, p1, x0, x1);
+                        } else {
+                            p0 = fast_exp2(x0);
+                            p1 = fast_exp2(x1);
+                        }
+                        r[i] = __float_as_uint(p0);
+                        r[i + 1] = __float_as_uint(p1);
+                        pk[(i - kPuSplit) >> 1] = pack_bf16x2(p0, p1);
+                    }
+                    tmem_st_32x32b_x16(s_addr + kPuSplit / 2, pk);
+                    tmem_wait_st();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(B_PFULL00 + 2 * t + 1));
+                    if ((warp & 3) == 0) PU_TRACE(2 + t, 25);
                 }
                 // ---- row sum, after the hand-off (packed adds, four chains)
                 float s0 = __uint_as_float(r[0]), s1 = __uint_as_float(r[1]);
