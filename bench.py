@@ -40,9 +40,9 @@ METRIC = "paged_decode_attn_GBps"
 UNIT = "GB/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r1a_full_summary.csv); valid for the full-size workloads only.
-NCU_TRAFFIC = {"decode": 2147766000 + 5497600 + 4271000, "prefill": 88314000 + 9574912,
-               "source": "profiles/r1a_full_summary.csv"}
+# (profiles/r1b_full_summary.csv); valid for the full-size workloads only.
+NCU_TRAFFIC = {"decode": 2147741000 + 5647872 + 4270000, "prefill": 87994000 + 13260544,
+               "source": "profiles/r1b_full_summary.csv"}
 
 
 def load_peaks():
@@ -229,6 +229,74 @@ def run_reference(args):
 
 # ----------------------------------------------------------------------------- the CUDA arm
 
+def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15):
+    """configs[1] (BAGEL-like CFG-pair decode) and configs[3] (thinker + talker decode): median call time with a
+    cold L2, GB/s on logical and on unique K/V bytes (shared prefix pages counted once), sequences per second."""
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def prep(b):
+        d = DeviceBatch(b, device=dev)
+        d.append()
+        S, Hq, Dh = b.num_seqs, b.num_q_heads, b.head_dim
+        parts = mstar.decode_auto_partitions(S, b.num_kv_heads, b.max_seq_len)
+        out = torch.empty((S, Hq, Dh), dtype=torch.bfloat16, device=dev)
+        ws = torch.empty(mstar.decode_workspace_bytes(S, Hq, Dh, parts), dtype=torch.uint8, device=dev)
+        call = lambda: mstar.paged_attn_decode(out, d.q_decode, d.pool, d.block_table, d.seq_lens, b.max_seq_len,
+                                               float(b.scale), num_partitions=0, workspace=ws)
+        return d, call, parts
+
+    def median_ms(calls, streams=None):
+        ts = []
+        for _ in range(iters + 3):
+            flush.fill_(1)
+            torch.cuda.synchronize()
+            e0, e1 = ev(), ev()
+            e0.record()
+            if streams is None:
+                for c in calls:
+                    c()
+            else:
+                cur = torch.cuda.current_stream()
+                for c, st in zip(calls, streams):
+                    st.wait_stream(cur)
+                    with torch.cuda.stream(st):
+                        c()
+                for st in streams:
+                    cur.wait_stream(st)
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ts = sorted(ts[3:])
+        return ts[len(ts) // 2]
+
+    def entry(b, ms, parts):
+        lg, uq = b.kv_bytes_logical(), b.kv_bytes_unique()
+        return {"seqs": b.num_seqs, "q_heads": b.num_q_heads, "kv_heads": b.num_kv_heads, "partitions": parts,
+                "us": ms * 1e3, "kv_bytes_logical": lg, "kv_bytes_unique": uq,
+                "GBps_logical": lg / (ms * 1e-3) / 1e9, "GBps_unique": uq / (ms * 1e-3) / 1e9,
+                "frac_of_measured_hbm_unique": uq / (ms * 1e-3) / 1e9 / hbm_peak,
+                "decode_tokens_per_s": b.num_seqs / (ms * 1e-3)}
+
+    res = {"protocol": "one mstar_paged_attn_decode call (split-K + combine), auto partitions, L2 flushed before "
+                       "every call, median of %d" % iters}
+    b2 = W.config2_bagel_cfg_decode()
+    d2, c2, p2 = prep(b2)
+    res["configs[1] BAGEL-like CFG-pair decode"] = entry(b2, median_ms([c2]), p2)
+    del d2, c2
+    bt, bk = W.config4_thinker(), W.config4_talker()
+    dt, ct, pt = prep(bt)
+    dk, ck, pk = prep(bk)
+    res["configs[3] thinker decode"] = entry(bt, median_ms([ct]), pt)
+    res["configs[3] talker decode"] = entry(bk, median_ms([ck]), pk)
+    ms_both = median_ms([ct, ck], streams=[torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)])
+    tot = bt.kv_bytes_logical() + bk.kv_bytes_logical()
+    res["configs[3] thinker || talker (two streams)"] = {
+        "us": ms_both * 1e3, "kv_bytes_logical": tot, "GBps_logical": tot / (ms_both * 1e-3) / 1e9,
+        "frac_of_measured_hbm": tot / (ms_both * 1e-3) / 1e9 / hbm_peak,
+        "decode_tokens_per_s": (bt.num_seqs + bk.num_seqs) / (ms_both * 1e-3)}
+    return res
+
+
 def run_ours(args):
     import torch
     rank, world, local, dist = dist_setup(args.gpus)
@@ -351,6 +419,12 @@ def run_ours(args):
     t_e2e = max_over_ranks(dist, e0.elapsed_time(e1) / K, dev)
     e2e_value = world * kv_bytes / (t_e2e * 1e-3) / 1e9
 
+    # ---- the serving-shaped decode configs (BAGEL CFG pairs, Qwen3-Omni thinker / talker): reported beside the
+    # headline, outside the K timed steps; cold L2 (flush before every call), CUDA events, median of 15
+    other = None
+    if rank == 0 and not args.no_other:
+        other = other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak=peaks["hbm_gbs"])
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -399,6 +473,8 @@ def run_ours(args):
         "gpu_launches": timed_launches,
         "clocks": clocks,
     }
+    if other is not None:
+        line["other_workloads"] = other
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(bd)
     elif not args.no_cpu_baseline:
@@ -417,6 +493,7 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other", action="store_true", help="skip the configs[1] / configs[3] decode timings")
     args = ap.parse_args(argv)
     if args.impl == "reference":
         return run_reference(args)
