@@ -99,9 +99,13 @@ int mstar_kv_append(const mstar_kv_pool* pool, const void* k_new, const void* v_
  *                  page 0,1,...; only the first ceil(seq_lens[s]/page_size) entries are read
  *   seq_lens       device, [S] int32, KV length of each sequence (0 => out = 0, lse = -inf)
  *   max_seq_len    host upper bound on seq_lens (sizes the partition grid; may over-estimate)
- *   num_partitions split-K partitions per sequence; 0 = automatic.  Partition i of a sequence covers
- *                  tokens [i*c, (i+1)*c) with c = ceil(max_seq_len/num_partitions) rounded up to a
- *                  multiple of 64; partitions past a sequence's end are empty.  1 = no combine pass.
+ *   num_partitions split-K partitions per sequence.  P >= 1: partition i of a sequence covers tokens
+ *                  [i*c, (i+1)*c) with c = ceil(max_seq_len/P) rounded up to a multiple of 64; partitions
+ *                  past a sequence's end are empty; 1 = no combine pass.  0 = balanced: the 64-token
+ *                  tiles of all (sequence, kv head) streams are laid end to end and every CTA takes an
+ *                  equal contiguous range, so ragged batches finish together; a stream cut by range
+ *                  boundaries is merged by the combine pass (the cut points depend on seq_lens and
+ *                  the SM count only, never on page ids).
  *   workspace      device, >= mstar_paged_attn_decode_workspace_bytes(...) bytes, 16-B aligned
  * Requires Hq % Hkv == 0 and Hq/Hkv <= 16.
  */
@@ -112,7 +116,8 @@ int mstar_paged_attn_decode(void* out, float* lse_out, const void* q, const msta
                             const int32_t* seq_lens, int32_t num_seqs, int32_t num_q_heads,
                             int32_t max_seq_len, float scale, int32_t num_partitions, uint32_t flags,
                             void* workspace, size_t workspace_bytes, void* stream);
-/* The partition count the automatic choice (num_partitions = 0) would use; for sizing the workspace. */
+/* Partial slots per (sequence, head) the choice num_partitions = 0 needs; pass it as max_partitions when sizing
+ * the workspace. */
 int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv_heads,
                                                 int32_t max_seq_len);
 

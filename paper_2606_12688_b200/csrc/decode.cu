@@ -41,6 +41,13 @@ struct DecodeParams {
     int32_t out_f32;
     int32_t direct;  // nparts == 1: write the final output, no combine pass
     int32_t nstages;
+    // balanced mode (num_partitions = 0): the (sequence, kv head) streams are laid end to end in 64-token tiles and
+    // every CTA takes an equal, contiguous range of them; a stream cut by CTA boundaries yields one partial per
+    // piece.  chunk == kDecodeTok then, per_min bounds the pieces of one stream by nparts, and piece_count
+    // [S*Hkv] tells the combine pass how many partials each stream has.
+    int32_t balanced;
+    int32_t per_min;
+    int32_t* piece_count;
 };
 
 struct ItemInfo {
@@ -153,19 +160,9 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         const uint32_t op_off = op_isv * KBYTES + op_half * HT + op_page * (PAGE * 128);
 
         int st = 0, ph = 0, qs = 0, qph = 0;
-        for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
-            const int pi = item / p.Hkv, kvh = item - pi * p.Hkv;
-            int lo = 0, hi = p.S;  // cum[lo] <= pi < cum[hi]
-            while (hi - lo > 1) {
-                const int mid = (lo + hi) >> 1;
-                if (cum[mid] <= pi) lo = mid; else hi = mid;
-            }
-            const int s = lo, part = pi - cum[lo];
-            const int L = p.seq_lens[s];
-            const int tok0 = part * p.chunk;
-            const int ntok = min(L - tok0, p.chunk);
+        // hand one work item to the consumers and stream its K/V tiles into the ring
+        auto emit_item = [&](int s, int kvh, int part, int tok0, int ntok) {
             const int ntiles = (ntok + TOK - 1) / TOK;
-
             mbar_wait(qempty_bar(qs), qph ^ 1);
             if (lane == 0) {
                 info[qs] = ItemInfo{s, kvh, part, tok0, ntok};
@@ -198,6 +195,55 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     tma_load_4d(ring + st * SM::kStageBytes + op_off, op_isv ? &vmap : &kmap, full_bar(st),
                                 op_half * 64, 0, kvh, pg, pol);
                 if (++st == nstages) { st = 0; ph ^= 1; }
+            }
+        };
+        if (p.balanced) {
+            // cum[] holds tiles per sequence (chunk == TOK); flat tile id = cum[s]*Hkv + kvh*nt_s + tile
+            const int64_t N = (int64_t)carry * p.Hkv;
+            int64_t per = (N + gridDim.x - 1) / gridDim.x;
+            if (per < p.per_min) per = p.per_min;
+            const int64_t fa = (int64_t)blockIdx.x * per;
+            const int64_t fb = (fa + per < N) ? fa + per : N;
+            if (fa < N) {
+                int lo = 0, hi = p.S;  // cum[lo]*Hkv <= fa < cum[hi]*Hkv
+                while (hi - lo > 1) {
+                    const int mid = (lo + hi) >> 1;
+                    if ((int64_t)cum[mid] * p.Hkv <= fa) lo = mid; else hi = mid;
+                }
+                int s = lo;
+                int64_t f = fa;
+                while (f < fb) {
+                    const int nt = cum[s + 1] - cum[s];
+                    const int64_t F0 = (int64_t)cum[s] * p.Hkv;
+                    const int kvh = (int)((f - F0) / nt);
+                    const int tile = (int)((f - F0) - (int64_t)kvh * nt);
+                    const int64_t fs = F0 + (int64_t)kvh * nt;  // flat start of this stream
+                    const int ntl = (int)(((int64_t)(nt - tile) < fb - f) ? (nt - tile) : (fb - f));
+                    const int piece = (int)((int64_t)blockIdx.x - fs / per);
+                    if (tile == 0 && lane == 0)
+                        p.piece_count[(size_t)s * p.Hkv + kvh] = (int)((fs + nt - 1) / per - fs / per) + 1;
+                    const int L = p.seq_lens[s];
+                    const int tok0 = tile * TOK;
+                    emit_item(s, kvh, piece, tok0, min(L - tok0, ntl * TOK));
+                    f += ntl;
+                    if (tile + ntl == nt && kvh == p.Hkv - 1) {
+                        ++s;
+                        while (s < p.S && cum[s + 1] == cum[s]) ++s;  // sequences without tokens
+                    }
+                }
+            }
+        } else {
+            for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+                const int pi = item / p.Hkv, kvh = item - pi * p.Hkv;
+                int lo = 0, hi = p.S;  // cum[lo] <= pi < cum[hi]
+                while (hi - lo > 1) {
+                    const int mid = (lo + hi) >> 1;
+                    if (cum[mid] <= pi) lo = mid; else hi = mid;
+                }
+                const int s = lo, part = pi - cum[lo];
+                const int L = p.seq_lens[s];
+                const int tok0 = part * p.chunk;
+                emit_item(s, kvh, part, tok0, min(L - tok0, p.chunk));
             }
         }
         // sentinel: tell the consumers to stop
@@ -420,6 +466,7 @@ __global__ void __launch_bounds__(128) decode_combine_kernel(const float* __rest
                                                              const float* __restrict__ part_m,
                                                              const float* __restrict__ part_l,
                                                              const int32_t* __restrict__ seq_lens, int32_t chunk,
+                                                             const int32_t* __restrict__ piece_count, int32_t G,
                                                              int32_t nparts, int32_t Hq, int32_t n_rows,
                                                              void* __restrict__ out, float* __restrict__ lse,
                                                              int32_t out_f32) {
@@ -429,7 +476,9 @@ __global__ void __launch_bounds__(128) decode_combine_kernel(const float* __rest
     if (row >= n_rows) return;
     const int s = row / Hq;
     const int L = seq_lens[s];
-    const int np = (L + chunk - 1) / chunk;
+    // balanced mode: the split-K kernel recorded the number of pieces of every (sequence, kv head) stream
+    const int np = (L <= 0) ? 0 : piece_count ? piece_count[(size_t)s * (Hq / G) + (row - s * Hq) / G]
+                                              : (L + chunk - 1) / chunk;
     float acc[VEC];
 #pragma unroll
     for (int i = 0; i < VEC; ++i) acc[i] = 0.f;
@@ -478,10 +527,28 @@ static int32_t auto_chunk(int32_t S, int32_t Hkv, int32_t max_seq_len) {
     return chunk;
 }
 
+// num_partitions = 0: balanced mode when a sequence can span at least two tiles.  Slots per row = pieces a stream
+// can be cut into: a CTA range is at least per_min = ceil(max_tiles / (slots - 1)) tiles long, so a stream of
+// max_tiles tiles meets at most slots CTA ranges.
+static bool balanced_plan(int32_t max_seq_len, int32_t* nparts, int32_t* per_min) {
+    const int32_t max_tiles = (max_seq_len + kDecodeTok - 1) / kDecodeTok;
+    if (max_tiles < 2) return false;
+    int32_t slots = (max_tiles + 1) / 2 + 1;
+    if (slots > 33) slots = 33;
+    *nparts = slots;
+    *per_min = (max_tiles + slots - 2) / (slots - 1);
+    return true;
+}
+
 static void partition_plan(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t num_partitions, int32_t* chunk,
                            int32_t* nparts) {
     const int32_t msl = max_seq_len > 0 ? max_seq_len : 1;
     if (num_partitions <= 0) {
+        int32_t per_min;
+        if (balanced_plan(msl, nparts, &per_min)) {
+            *chunk = kDecodeTok;
+            return;
+        }
         *chunk = auto_chunk(S, Hkv, msl);
     } else {
         *chunk = round_up((msl + num_partitions - 1) / num_partitions, kDecodeTok);
@@ -527,7 +594,8 @@ extern "C" size_t mstar_paged_attn_decode_workspace_bytes(int32_t num_seqs, int3
                                                           int32_t max_partitions) {
     if (num_seqs <= 0 || num_q_heads <= 0 || head_dim <= 0 || max_partitions <= 1) return 256;
     const size_t rows = (size_t)num_seqs * num_q_heads * max_partitions;
-    return 256 + rows * head_dim * 4 + 2 * rows * 4 + 256;
+    // partials (O, m, l) + one piece count per (sequence, kv head) stream (bounded by the q heads)
+    return 256 + rows * head_dim * 4 + 2 * rows * 4 + 256 + (size_t)num_seqs * num_q_heads * 4;
 }
 
 extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool,
@@ -554,6 +622,7 @@ extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q,
 
     DecodeParams p{};
     partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, &p.chunk, &p.nparts);
+    if (num_partitions == 0) p.balanced = balanced_plan(max_seq_len > 0 ? max_seq_len : 1, &p.nparts, &p.per_min) ? 1 : 0;
     p.direct = (p.nparts == 1);
     if (!p.direct) {
         const size_t need = mstar_paged_attn_decode_workspace_bytes(num_seqs, num_q_heads, D, p.nparts);
@@ -563,6 +632,7 @@ extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q,
         p.part_O = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + 256);
         p.part_m = p.part_O + rows * D;
         p.part_l = p.part_m + rows;
+        p.piece_count = p.balanced ? reinterpret_cast<int32_t*>(p.part_l + rows + 64) : nullptr;
     }
     p.q = reinterpret_cast<const uint16_t*>(q);
     p.block_table = block_table;
@@ -601,10 +671,12 @@ extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q,
         const int blocks = (n_rows + 3) / 4;
         if (D == 128)
             decode_combine_kernel<128><<<blocks, 128, 0, st>>>(p.part_O, p.part_m, p.part_l, seq_lens, p.chunk,
-                                                              p.nparts, num_q_heads, n_rows, out, lse_out, p.out_f32);
+                                                              p.piece_count, G, p.nparts, num_q_heads, n_rows, out,
+                                                              lse_out, p.out_f32);
         else
             decode_combine_kernel<64><<<blocks, 128, 0, st>>>(p.part_O, p.part_m, p.part_l, seq_lens, p.chunk,
-                                                             p.nparts, num_q_heads, n_rows, out, lse_out, p.out_f32);
+                                                             p.piece_count, G, p.nparts, num_q_heads, n_rows, out,
+                                                             lse_out, p.out_f32);
         MSTAR_CUDA_OK(cudaGetLastError());
         launch_count_add(1);
     }
