@@ -3,7 +3,7 @@
 // Design.  The path is an HBM stream: every K/V byte of every sequence is read
 // exactly once, 4*G*D flops per 2*D*2 bytes.  One persistent CTA per SM; work items are
 // (sequence, split-K partition, kv head).  Inside a CTA
-//   * one PRODUCER warp walks the block table and issues TMA tensor copies (cp.async.bulk.tensor,
+//   * two PRODUCER warps (K half / V half of every stage) walk the block table and issues TMA tensor copies (cp.async.bulk.tensor,
 //     128-B swizzle) of whole (page, kv head) slabs into a deep shared-memory ring of 64-token stages,
 //     running ahead across work items so the stream never drains between items;
 //   * four CONSUMER warps each own 16 tokens of every stage: S = Q K^T with warp-level bf16 MMA
@@ -21,7 +21,7 @@ namespace mstar {
 
 constexpr int kDecodeConsumerWarps = 4;
 constexpr int kDecodeTok = 16 * kDecodeConsumerWarps;  // tokens per ring stage
-constexpr int kDecodeThreads = 32 * (kDecodeConsumerWarps + 1);
+constexpr int kDecodeThreads = 32 * (kDecodeConsumerWarps + 2);  // 4 consumer warps, K producer, V producer
 constexpr int kMaxStages = 16;
 
 struct DecodeParams {
@@ -115,7 +115,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < nstages; ++i) {
-            mbar_init(full_bar(i), 1);
+            mbar_init(full_bar(i), 2);  // K producer + V producer (each with its own transaction bytes)
             mbar_init(empty_bar(i), NW);
         }
         for (int i = 0; i < 2; ++i) {
@@ -129,7 +129,11 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
     fence_proxy_async_smem();
     __syncthreads();
 
-    if (warp == NW) {
+    if (warp >= NW) {
+        // Two producer warps walk the same item list: warp NW loads the K half of every stage (and Q and the item
+        // record), warp NW + 1 the V half.  Each TMA issue with per-lane coordinates is serialised by the hardware
+        // interface, so two warps halve the issue time per stage (16 operations per stage at page size 16).
+        const int op_isv = warp - NW;
         // =============================== PRODUCER ===============================
         prefetch_tensormap(&kmap);
         prefetch_tensormap(&vmap);
@@ -153,9 +157,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         const uint64_t pol = policy_evict_first();
 
         // this lane's TMA op within a stage: (page i, K or V, 64-column half)
-        constexpr int OPS = PPS * 2 * NH;
-        const int op_page = lane / (2 * NH);
-        const int op_isv = (lane % (2 * NH)) / NH;
+        constexpr int OPS = PPS * NH;
+        const int op_page = lane / NH;
         const int op_half = lane % NH;
         const uint32_t op_off = op_isv * KBYTES + op_half * HT + op_page * (PAGE * 128);
 
@@ -163,8 +166,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         // hand one work item to the consumers and stream its K/V tiles into the ring
         auto emit_item = [&](int s, int kvh, int part, int tok0, int ntok) {
             const int ntiles = (ntok + TOK - 1) / TOK;
-            mbar_wait(qempty_bar(qs), qph ^ 1);
-            if (lane == 0) {
+            if (!op_isv) mbar_wait(qempty_bar(qs), qph ^ 1);
+            if (lane == 0 && !op_isv) {
                 info[qs] = ItemInfo{s, kvh, part, tok0, ntok};
                 mbar_arrive_expect_tx(qfull_bar(qs), (uint32_t)(p.G * D * 2));
                 bulk_load_1d(qbuf + qs * SM::kQBytes, p.q + ((size_t)s * p.Hq + (size_t)kvh * p.G) * D,
@@ -189,7 +192,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     if (lane < OPS && op_page < npg1) pg_next = __ldg(bt + (t + 1) * PPS + op_page);
                 }
                 mbar_wait(empty_bar(st), ph ^ 1);
-                if (lane == 0) mbar_arrive_expect_tx(full_bar(st), (uint32_t)(npg * PAGE * D * 2 * 2));
+                if (lane == 0) mbar_arrive_expect_tx(full_bar(st), (uint32_t)(npg * PAGE * D * 2));
                 __syncwarp();
                 if (pg >= 0)
                     tma_load_4d(ring + st * SM::kStageBytes + op_off, op_isv ? &vmap : &kmap, full_bar(st),
@@ -220,7 +223,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     const int64_t fs = F0 + (int64_t)kvh * nt;  // flat start of this stream
                     const int ntl = (int)(((int64_t)(nt - tile) < fb - f) ? (nt - tile) : (fb - f));
                     const int piece = (int)((int64_t)blockIdx.x - fs / per);
-                    if (tile == 0 && lane == 0)
+                    if (tile == 0 && lane == 0 && !op_isv)
                         p.piece_count[(size_t)s * p.Hkv + kvh] = (int)((fs + nt - 1) / per - fs / per) + 1;
                     const int L = p.seq_lens[s];
                     const int tok0 = tile * TOK;
@@ -247,8 +250,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
             }
         }
         // sentinel: tell the consumers to stop
-        mbar_wait(qempty_bar(qs), qph ^ 1);
-        if (lane == 0) {
+        if (!op_isv) mbar_wait(qempty_bar(qs), qph ^ 1);
+        if (lane == 0 && !op_isv) {
             info[qs].ntok = -1;
             mbar_arrive(qfull_bar(qs));
         }
