@@ -110,6 +110,17 @@ def test_decode_many_sequences_and_nhd_layout():
     run_decode_case(b, parts_list=(0, 2), layout="NHD", check_f32=False)
 
 
+@pytest.mark.parametrize("S", [1, 2, 3, 148, 149])
+def test_decode_sequence_counts_and_balanced_cuts(S):
+    """Batch sizes around the SM count; one long sequence among short ones makes the balanced mode
+    (num_partitions = 0) cut a stream into many pieces (per = per_min) while other CTAs take whole streams."""
+    rng = np.random.default_rng(230 + S)
+    lens = rng.integers(1, 400, S).tolist()
+    lens[S // 2] = 5000
+    b = small_batch(230 + S, lens, Hq=14, Hkv=2, D=128, p=16)
+    run_decode_case(b, parts_list=(0, 4), check_f32=False)
+
+
 def test_decode_len1_bit_exact_and_unit_values():
     """Closed forms on the GPU: L = 1 => out = V row bit-for-bit; V == 1 => out == 1 exactly."""
     b = small_batch(220, [1, 1, 1, 200, 1000], Hq=8, Hkv=2, D=128, p=16)
@@ -247,6 +258,28 @@ def test_prefill_ragged_small(D, p, G):
     b = small_batch(300 + G, lens, q_lens=qls, Hq=G * 2, Hkv=2, D=D, p=p)
     run_prefill_case(b)
     run_prefill_case(b, causal=False)
+
+
+def test_prefill_new_tokens_times_prefix_matrix():
+    """n in {1, 2, 127, 128, 129} x P in {0, 1, p-1, p, 2047, 2048} as one ragged batch (SURVEY 8(c) matrix);
+    G = 7 packs 18 tokens per Q tile, so full tiles (TMA-store epilogue) and ragged tail tiles both occur."""
+    p = 16
+    lens, qls = [], []
+    for n in (1, 2, 127, 128, 129):
+        for P in (0, 1, p - 1, p, 2047, 2048):
+            lens.append(P + n)
+            qls.append(n)
+    b = small_batch(305, lens, q_lens=qls, Hq=14, Hkv=2, D=128, p=p)
+    run_prefill_case(b)
+
+
+def test_prefill_long_block_with_and_without_prefix():
+    """n = 1024 with P = 0 and P = 2048 (config-3 extremes), sampled rows incl. first / last rows and tile edges."""
+    b = small_batch(306, [1024, 3072], q_lens=[1024, 1024], Hq=14, Hkv=2, D=128, p=16)
+    rows = np.unique(np.concatenate([np.arange(0, 40), np.arange(1000, 1064), np.arange(2008, 2048),
+                                     np.random.default_rng(5).integers(0, 2048, 64)])).astype(np.int32)
+    run_prefill_case(b, rows=rows)
+    run_prefill_case(b, rows=rows, causal=False)
 
 
 def test_prefill_one_token_equals_decode_semantics():
