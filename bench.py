@@ -296,6 +296,27 @@ def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15
         "us": ms_both * 1e3, "kv_bytes_logical": tot, "GBps_logical": tot / (ms_both * 1e-3) / 1e9,
         "frac_of_measured_hbm": tot / (ms_both * 1e-3) / 1e9 / hbm_peak,
         "decode_tokens_per_s": (bt.num_seqs + bk.num_seqs) / (ms_both * 1e-3)}
+    del dt, dk, ct, ck
+    # the BAGEL-like denoise (flow) step, 4 requests x 3 CFG labels x 4096 latent tokens,
+    # bidirectional block over the cached label context (causal = 0), appended to scratch pages first
+    bf = W.flow_step_bagel()
+    df = DeviceBatch(bf, device=dev)
+    outf = torch.empty((bf.total_q, bf.num_q_heads, bf.head_dim), dtype=torch.bfloat16, device=dev)
+    wsf = torch.empty(mstar.prefill_workspace_bytes(bf.num_seqs, bf.total_q, bf.num_q_heads, bf.head_dim),
+                      dtype=torch.uint8, device=dev)
+
+    def flow_call():
+        mstar.kv_append(df.pool, df.k_new, df.v_new, df.slot_mapping)
+        mstar.paged_attn_prefill(outf, df.q, df.cu_seqlens_q, df.pool, df.block_table, df.seq_lens, bf.max_q_len,
+                                 bf.max_seq_len, float(bf.scale), causal=False, workspace=wsf)
+
+    ms_f = median_ms([flow_call])
+    n = bf.q_lens.astype(np.float64)
+    fl = float((4.0 * bf.num_q_heads * bf.head_dim * n * bf.seq_lens.astype(np.float64)).sum())
+    res["flow step (SURVEY 8(f) rank 1): 4 requests x 3 CFG labels x 4096 latent tokens, causal = 0"] = {
+        "seqs": bf.num_seqs, "new_tokens": int(bf.q_lens[0]), "context": (bf.seq_lens - bf.q_lens).tolist(),
+        "ms": ms_f, "flops": fl, "TFLOPs": fl / (ms_f * 1e-3) / 1e12,
+        "note": "append of the block's K/V + prefill call; flops = sum 4 Hq D n (context + n)"}
     return res
 
 

@@ -282,6 +282,25 @@ def test_prefill_long_block_with_and_without_prefix():
     run_prefill_case(b, rows=rows, causal=False)
 
 
+def test_prefill_flow_step_bidirectional_block_over_cfg_labels():
+    """the denoise step -- a block of latent tokens attends bidirectionally to itself and to
+    the cached context of its CFG label (causal = 0); the cfg_img label reads the cond label's context pages by
+    reference.  Sampled rows incl. block edges; both kernels."""
+    b = W.flow_step_bagel(num_requests=2, n_latent=1024)
+    rng = np.random.default_rng(61)
+    rows = np.unique(np.concatenate([rng.integers(0, b.total_q, 128), b.cu_seqlens_q[:-1],
+                                     b.cu_seqlens_q[1:] - 1])).astype(np.int32)
+    run_prefill_case(b, rows=rows, causal=False)
+    # labels that share context pages and have equal context length see identical K/V for the context; their
+    # outputs differ only through their own latent block, so nothing is bit-identical here -- but the shared
+    # pages must not have been written by the append of either label
+    db = DeviceBatch(b)
+    before = bits_of(db.k_pool[torch.from_numpy(b.block_table[0, :4].astype(np.int64)).cuda()])
+    db.append()
+    after = bits_of(db.k_pool[torch.from_numpy(b.block_table[0, :4].astype(np.int64)).cuda()])
+    assert np.array_equal(before, after)
+
+
 def test_prefill_one_token_equals_decode_semantics():
     b = small_batch(310, [1, 17, 33, 100, 700], Hq=8, Hkv=2, D=128)
     db = DeviceBatch(b)

@@ -23,5 +23,6 @@ from .generators import (  # noqa: F401
     config4_thinker,
     config4_talker,
     config5_long_context,
+    flow_step_bagel,
     CONFIG_SEED_BASE,
 )

@@ -288,3 +288,25 @@ def config5_long_context(num_seqs: int = 16, seq_len: int = 32768, num_pages: in
     """configs[4]: 16 x 32768, 32q/8kv, D 128, page 32, pages scattered over a 60 GiB pool (491520 pages)."""
     return make_batch(_rng(5), "cfg5_long_context", [seq_len] * num_seqs, [1] * num_seqs,
                       32, 8, 128, 32, num_pages)
+
+
+def flow_step_bagel(num_requests: int = 4, n_latent: int = 4096, n_labels: int = 3) -> PagedBatch:
+    """SURVEY 8(f) rank 1, the denoise ("flow") step of BAGEL-like text-to-image: every
+    request has ``n_labels`` CFG labels (cond, cfg_text, cfg_img); each label is one sequence whose ``n_latent``
+    new latent-image tokens attend bidirectionally among themselves and to the label's cached context
+    (``causal = 0`` over seq_len = context + n_latent).  The paper gives no lengths: context of the cond label
+    U{64..512} prompt tokens, cfg_text label 1 token (no text), cfg_img label = the cond context, by reference
+    (same physical pages for its first 64 tokens).  n_latent = 4096 is a 1024 x 1024 image at 16 x 16 pixels per
+    latent token.  28 q / 4 kv heads, head_dim 128, page 16 (the BAGEL-like geometry of configs[1])."""
+    rng = np.random.default_rng(CONFIG_SEED_BASE + 61)
+    ctx = rng.integers(64, 513, num_requests)
+    lens, share = [], []
+    for r in range(num_requests):
+        for lab in range(n_labels):
+            c = 1 if lab == 1 else int(ctx[r])
+            lens.append(c + n_latent)
+            share.append(r * n_labels if lab == 2 else -1)
+    if n_labels < 3:
+        share = [-1] * len(lens)
+    return make_batch(rng, "flow_step_bagel", lens, [n_latent] * len(lens), 28, 4, 128, 16,
+                      2 * _pages(lens, 16), share_with=share, shared_tokens=64 if n_labels >= 3 else 0)
