@@ -113,6 +113,8 @@ prefill_plan_kernel(const int32_t* __restrict__ cu_seqlens_q, const int32_t* __r
     __shared__ int hist[kPlanBuckets];
     __shared__ int scan[kPlanBuckets];
     const int tid = threadIdx.x;
+    // let the attention grid start its prologue now; it waits (griddepcontrol.wait) for this grid to finish
+    asm volatile("griddepcontrol.launch_dependents;");
     hist[tid] = 0;
     __syncthreads();
     const int64_t total = (int64_t)nqb * S;
@@ -300,6 +302,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             prefetch_tensormap(&qmap);
             prefetch_tensormap(&kmap);
             prefetch_tensormap(&vmap);
+            // Programmatic dependent launch: everything above (barriers, TMEM, descriptor prefetch) overlapped the
+            // tail of the previous grid in the stream (the plan kernel, or the K/V append); every read and write
+            // of global memory in this kernel happens after this warp has seen that grid complete, because all
+            // other roles only start on barriers this warp's loads complete.
+            asm volatile("griddepcontrol.wait;" ::: "memory");
             const uint64_t pol_kv = policy_evict_last();   // K/V re-read by other query blocks of the sequence
             const uint64_t pol_q = policy_evict_first();
             // lane -> (K or V, page, half): PPS*2 ops for K on the low lanes, PPS*2 for V after them
@@ -613,7 +620,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     m_ref = mx;
                 } else {
                     const float m_new = fmaxf(m_ref, mx);
-                    const bool need = (m_new - m_ref) * c > kPuTau;
+                    // only rows that are stored vote: tile rows past rows_used hold whatever the previous kernel
+                    // left in shared memory, and a rescale they triggered would change the rounding of the whole
+                    // warp from run to run (results must be bit-identical across runs, R20)
+                    const bool need = row_ok && (m_new - m_ref) * c > kPuTau;
                     if (__any_sync(0xffffffffu, need)) {
                         const float alpha = fast_exp2((m_ref - m_new) * c);
                         l *= alpha;
@@ -865,10 +875,17 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
         MSTAR_CUDA_OK(cudaFuncSetAttribute(k32, cudaFuncAttributeMaxDynamicSharedMemorySize, kPuSmemBytes));
         attr_set = true;
     }
-    if (page_size == 16)
-        k16<<<grid, kPuThreads, kPuSmemBytes, stream>>>(qmap, maps.k, maps.v, omap, p);
-    else
-        k32<<<grid, kPuThreads, kPuSmemBytes, stream>>>(qmap, maps.k, maps.v, omap, p);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(kPuThreads);
+    cfg.dynamicSmemBytes = kPuSmemBytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, page_size == 16 ? k16 : k32, qmap, maps.k, maps.v, omap, p));
     MSTAR_CUDA_OK(cudaGetLastError());
     launch_count_add(1);
     return MSTAR_OK;
