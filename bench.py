@@ -296,7 +296,7 @@ def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15
         "us": ms_both * 1e3, "kv_bytes_logical": tot, "GBps_logical": tot / (ms_both * 1e-3) / 1e9,
         "frac_of_measured_hbm": tot / (ms_both * 1e-3) / 1e9 / hbm_peak,
         "decode_tokens_per_s": (bt.num_seqs + bk.num_seqs) / (ms_both * 1e-3)}
-    del dt, dk, ct, ck
+    del dk, ct, ck
     # the BAGEL-like denoise (flow) step, 4 requests x 3 CFG labels x 4096 latent tokens,
     # bidirectional block over the cached label context (causal = 0), appended to scratch pages first
     bf = W.flow_step_bagel()
@@ -317,6 +317,27 @@ def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15
         "seqs": bf.num_seqs, "new_tokens": int(bf.q_lens[0]), "context": (bf.seq_lens - bf.q_lens).tolist(),
         "ms": ms_f, "flops": fl, "TFLOPs": fl / (ms_f * 1e-3) / 1e12,
         "note": "append of the block's K/V + prefill call; flops = sum 4 Hq D n (context + n)"}
+    # page moves (offload / transfer): gather the thinker batch to contiguous rows and copy its
+    # pages into the free half of its own pool
+    dt2 = DeviceBatch(bt, device=dev)
+    cu = np.zeros(bt.num_seqs + 1, dtype=np.int32)
+    cu[1:] = np.cumsum(bt.seq_lens)
+    cu_d = torch.from_numpy(cu).to(dev)
+    kg = torch.empty((int(cu[-1]), bt.num_kv_heads, bt.head_dim), dtype=torch.bfloat16, device=dev)
+    vg = torch.empty_like(kg)
+    used = np.zeros(bt.num_pages, dtype=bool)
+    used[bt.used_pages] = True
+    src = torch.from_numpy(bt.used_pages.astype(np.int64)).to(dev)
+    dstp = torch.from_numpy(np.flatnonzero(~used)[:len(bt.used_pages)].astype(np.int64)).to(dev)
+    ms_g = median_ms([lambda: mstar.kv_gather(kg, vg, dt2.pool, dt2.block_table, dt2.seq_lens, cu_d)])
+    ms_c = median_ms([lambda: mstar.kv_copy_pages(dt2.pool, dt2.pool, dstp, src)])
+    gb = 2 * bt.kv_bytes_logical()
+    cb = 2 * len(bt.used_pages) * 2 * bt.num_kv_heads * bt.page_size * bt.head_dim * 2
+    res["page moves (SURVEY 8(f) rank 4) on the thinker pool"] = {
+        "gather_us": ms_g * 1e3, "gather_GBps_read_plus_write": gb / (ms_g * 1e-3) / 1e9,
+        "copy_pages_us": ms_c * 1e3, "copy_pages": int(len(bt.used_pages)),
+        "copy_GBps_read_plus_write": cb / (ms_c * 1e-3) / 1e9,
+        "frac_of_measured_copy_rate": cb / (ms_c * 1e-3) / 1e9 / hbm_peak}
     return res
 
 

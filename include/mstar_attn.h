@@ -90,6 +90,26 @@ int mstar_kv_append(const mstar_kv_pool* pool, const void* k_new, const void* v_
                     const int64_t* slot_mapping, int64_t num_tokens, void* stream);
 
 /*
+ * mstar_kv_copy_pages / mstar_kv_gather: the page moves behind "paging, offload,
+ * by-reference transfer" and prefill/decode disaggregation.  Bit copies.
+ *   copy_pages: for i in 0..num_pairs-1, all heads and slots of page src_pages[i] of src_pool (K and V) are
+ *               written to page dst_pages[i] of dst_pool.  The pools must agree in page_size, num_kv_heads and
+ *               head_dim (strides may differ; they may be the same pool; a pool may live in pinned host memory
+ *               that is mapped into the device address space).  dst_pages, src_pages: device, int64; a negative
+ *               id skips the pair.  A page that is written by one pair and read or written by another pair of the
+ *               same call: undefined.
+ *   gather:     k_out/v_out [total_tokens][Hkv][D] bf16 contiguous, 16-B aligned; row cu_seqlens_out[s] + j gets
+ *               token j of sequence s, j < seq_lens[s], read through block_table (the inverse of append).
+ *               cu_seqlens_out: device, [S+1] int32, non-decreasing, cu[s+1]-cu[s] >= seq_lens[s]; rows of a
+ *               sequence's range past seq_lens[s] are not written.
+ */
+int mstar_kv_copy_pages(const mstar_kv_pool* dst_pool, const mstar_kv_pool* src_pool, const int64_t* dst_pages,
+                        const int64_t* src_pages, int64_t num_pairs, void* stream);
+int mstar_kv_gather(void* k_out, void* v_out, const mstar_kv_pool* pool, const int32_t* block_table,
+                    int64_t block_table_stride, const int32_t* seq_lens, const int32_t* cu_seqlens_out,
+                    int32_t num_seqs, int64_t total_tokens, void* stream);
+
+/*
  * mstar_paged_attn_decode (steps a2 + a3): one query token per sequence over block-table K/V, as a
  * split-K ("flash-decoding") pass plus a log-sum-exp combine.
  *   out            device, [S][Hq][D] bf16 (fp32 with MSTAR_FLAG_OUT_F32)

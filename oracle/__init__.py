@@ -76,6 +76,36 @@ def kv_append(k_pool, v_pool, k_new, v_new, slot_mapping):
                          ctypes.c_int32(D), _p(k_new), _p(v_new), _p(slot), ctypes.c_int64(T))
 
 
+def kv_gather(k_pool, v_pool, block_table, seq_lens):
+    """GATHER.  -> (k uint16 [sum L, Hkv, D], v the same, cu int32 [S+1])."""
+    lib = _load()
+    Hkv, p, D = _geom(k_pool)
+    k_pool, v_pool = _c(k_pool, np.uint16), _c(v_pool, np.uint16)
+    bt, sl = _c(block_table, np.int32), _c(seq_lens, np.int32)
+    S = sl.shape[0]
+    cu = np.zeros(S + 1, dtype=np.int32)
+    cu[1:] = np.cumsum(sl)
+    k_out = np.zeros((int(cu[-1]), Hkv, D), dtype=np.uint16)
+    v_out = np.zeros_like(k_out)
+    lib.oracle_kv_gather(_p(k_out), _p(v_out), _p(k_pool), _p(v_pool), _p(bt),
+                         ctypes.c_int64(bt.shape[1] if bt.ndim == 2 else 0), _p(sl), _p(cu), ctypes.c_int32(S),
+                         ctypes.c_int32(Hkv), ctypes.c_int32(p), ctypes.c_int32(D))
+    return k_out, v_out, cu
+
+
+def kv_copy_pages(k_dst, v_dst, k_src, v_src, dst_pages, src_pages):
+    """COPY_PAGES in place on ``k_dst`` / ``v_dst`` (uint16, C-contiguous)."""
+    lib = _load()
+    assert k_dst.dtype == np.uint16 and k_dst.flags.c_contiguous and v_dst.flags.c_contiguous
+    Hkv, p, D = _geom(k_dst)
+    assert _geom(k_src) == (Hkv, p, D)
+    k_src, v_src = _c(k_src, np.uint16), _c(v_src, np.uint16)
+    dp, sp = _c(dst_pages, np.int64), _c(src_pages, np.int64)
+    assert dp.shape == sp.shape
+    lib.oracle_kv_copy_pages(_p(k_dst), _p(v_dst), _p(k_src), _p(v_src), _p(dp), _p(sp),
+                             ctypes.c_int64(dp.shape[0]), ctypes.c_int32(Hkv), ctypes.c_int32(p), ctypes.c_int32(D))
+
+
 def paged_decode(q, k_pool, v_pool, block_table, seq_lens, scale):
     """DECODE.  q uint16 [S,Hq,D] -> (out fp64 [S,Hq,D], lse fp64 [S,Hq])."""
     lib = _load()

@@ -17,6 +17,10 @@
  *               (bottom-right aligned causal mask, "causal masking over a cached prefix",
  *               BASELINE.json north_star; reading R6)
  *   APPEND:     pool[slot div p][h][slot mod p][:] = new[t][h][:] as 16-bit words; slot < 0 skipped
+ *   GATHER (as an operation of its own) and COPY_PAGES (the page moves behind
+ *               "paging, offload, by-reference transfer", and prefill/decode disaggregation, :116):
+ *               out[cu[s] + j][h][:] = pool[block_table[s][j div p]][h][j mod p][:];
+ *               dst_pool[dst_pages[i]] = src_pool[src_pages[i]] (all heads and slots), in order of i, id < 0 skipped
  *   COMBINE:    M = max_i m_i; out = sum_i e^{m_i-M} O_i / sum_i e^{m_i-M} l_i; lse = M + ln(sum_i ...)
  *               (split-K merge, BASELINE.json north_star "log-sum-exp combine pass")
  *
@@ -284,4 +288,39 @@ void oracle_lse_combine(double* out, double* lse, const double* m, const double*
     }
     for (int32_t d = 0; d < D; ++d) out[d] /= Z;
     if (lse) *lse = M + log(Z);
+}
+
+
+/* GATHER: pool -> contiguous [total][Hkv][D], 16-bit words. */
+void oracle_kv_gather(uint16_t* k_out, uint16_t* v_out, const uint16_t* k_pool, const uint16_t* v_pool,
+                      const int32_t* block_table, int64_t bt_stride, const int32_t* seq_lens,
+                      const int32_t* cu_out, int32_t S, int32_t Hkv, int32_t p, int32_t D) {
+    for (int32_t s = 0; s < S; ++s) {
+        for (int32_t j = 0; j < seq_lens[s]; ++j) {
+            int64_t page = block_table[(int64_t)s * bt_stride + j / p];
+            int32_t off = j % p;
+            for (int32_t h = 0; h < Hkv; ++h) {
+                size_t src = (((size_t)page * Hkv + h) * p + off) * D;
+                size_t dst = (((size_t)cu_out[s] + j) * Hkv + h) * D;
+                for (int32_t d = 0; d < D; ++d) {
+                    k_out[dst + d] = k_pool[src + d];
+                    v_out[dst + d] = v_pool[src + d];
+                }
+            }
+        }
+    }
+}
+
+/* COPY_PAGES: whole pages between two pools of the same geometry (may be the same pool), sequential in i. */
+void oracle_kv_copy_pages(uint16_t* k_dst, uint16_t* v_dst, const uint16_t* k_src, const uint16_t* v_src,
+                          const int64_t* dst_pages, const int64_t* src_pages, int64_t n, int32_t Hkv, int32_t p,
+                          int32_t D) {
+    size_t page_elems = (size_t)Hkv * p * D;
+    for (int64_t i = 0; i < n; ++i) {
+        if (dst_pages[i] < 0 || src_pages[i] < 0) continue;
+        for (size_t e = 0; e < page_elems; ++e) {
+            k_dst[(size_t)dst_pages[i] * page_elems + e] = k_src[(size_t)src_pages[i] * page_elems + e];
+            v_dst[(size_t)dst_pages[i] * page_elems + e] = v_src[(size_t)src_pages[i] * page_elems + e];
+        }
+    }
 }

@@ -7,6 +7,8 @@ Python binding.  Names mirror the C entry points:
     paged_attn_decode    <- mstar_paged_attn_decode   (split-K + LSE combine)
     paged_attn_prefill   <- mstar_paged_attn_prefill  (causal over a cached prefix)
     build_slot_mapping   <- mstar_build_slot_mapping
+    kv_copy_pages        <- mstar_kv_copy_pages       (page moves pool -> pool)
+    kv_gather            <- mstar_kv_gather           (pool -> contiguous rows)
 
 There is no CPU fallback: without the built library every call raises ``MstarError``.
 """
@@ -20,6 +22,8 @@ from .binding import (  # noqa: F401
     decode_auto_partitions,
     decode_workspace_bytes,
     kv_append,
+    kv_copy_pages,
+    kv_gather,
     last_launch_count,
     load_library,
     paged_attn_decode,

@@ -22,6 +22,8 @@ MSTAR_FLAG_PREFILL_MMA_SYNC = 2
 
 EXPORTS = (
     "mstar_kv_append",
+    "mstar_kv_copy_pages",
+    "mstar_kv_gather",
     "mstar_paged_attn_decode_workspace_bytes",
     "mstar_paged_attn_decode",
     "mstar_paged_attn_decode_auto_partitions",
@@ -69,6 +71,12 @@ def load_library() -> ctypes.CDLL:
     lib.mstar_kv_append.restype = c.c_int
     lib.mstar_kv_append.argtypes = [c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p, c.c_void_p, c.c_int64,
                                     c.c_void_p]
+    lib.mstar_kv_copy_pages.restype = c.c_int
+    lib.mstar_kv_copy_pages.argtypes = [c.POINTER(_KvPoolStruct), c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p,
+                                        c.c_int64, c.c_void_p]
+    lib.mstar_kv_gather.restype = c.c_int
+    lib.mstar_kv_gather.argtypes = [c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_int64,
+                                    c.c_void_p, c.c_void_p, c.c_int32, c.c_int64, c.c_void_p]
     lib.mstar_paged_attn_decode_workspace_bytes.restype = c.c_size_t
     lib.mstar_paged_attn_decode_workspace_bytes.argtypes = [c.c_int32] * 4
     lib.mstar_paged_attn_decode_auto_partitions.restype = c.c_int32
@@ -158,6 +166,31 @@ def kv_append(pool: KVPool, k_new: torch.Tensor, v_new: torch.Tensor, slot_mappi
     lib = load_library()
     _check(lib.mstar_kv_append(ctypes.byref(pool.c), _ptr(k_new), _ptr(v_new), _ptr(slot_mapping), T, _stream()),
            "mstar_kv_append")
+
+
+def kv_copy_pages(dst_pool: KVPool, src_pool: KVPool, dst_pages: torch.Tensor, src_pages: torch.Tensor) -> None:
+    """mstar_kv_copy_pages: page src_pages[i] of src_pool -> page dst_pages[i] of dst_pool (int64, device)."""
+    _want(dst_pages, torch.int64, "dst_pages"); _want(src_pages, torch.int64, "src_pages")
+    if dst_pages.shape != src_pages.shape or dst_pages.dim() != 1:
+        raise MstarError("dst_pages and src_pages must be 1-D and of equal length")
+    lib = load_library()
+    _check(lib.mstar_kv_copy_pages(ctypes.byref(dst_pool.c), ctypes.byref(src_pool.c), _ptr(dst_pages),
+                                   _ptr(src_pages), int(dst_pages.shape[0]), _stream()), "mstar_kv_copy_pages")
+
+
+def kv_gather(k_out: torch.Tensor, v_out: torch.Tensor, pool: KVPool, block_table: torch.Tensor,
+              seq_lens: torch.Tensor, cu_seqlens_out: torch.Tensor) -> None:
+    """mstar_kv_gather: pool -> contiguous k_out / v_out [total, Hkv, D] bf16 through the block table."""
+    _want(k_out, torch.bfloat16, "k_out"); _want(v_out, torch.bfloat16, "v_out")
+    _want(block_table, torch.int32, "block_table"); _want(seq_lens, torch.int32, "seq_lens")
+    _want(cu_seqlens_out, torch.int32, "cu_seqlens_out")
+    S = int(seq_lens.shape[0])
+    if k_out.shape != v_out.shape or tuple(k_out.shape[1:]) != (pool.num_kv_heads, pool.head_dim):
+        raise MstarError("k_out / v_out must be [total, Hkv, D]")
+    lib = load_library()
+    _check(lib.mstar_kv_gather(_ptr(k_out), _ptr(v_out), ctypes.byref(pool.c), _ptr(block_table),
+                               int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens),
+                               _ptr(cu_seqlens_out), S, int(k_out.shape[0]), _stream()), "mstar_kv_gather")
 
 
 def decode_auto_partitions(num_seqs: int, num_kv_heads: int, max_seq_len: int) -> int:

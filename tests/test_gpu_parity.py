@@ -87,6 +87,44 @@ def test_build_slot_mapping_matches_generator():
     assert np.array_equal(out.cpu().numpy(), b.slot_mapping)
 
 
+@pytest.mark.parametrize("layout", ["HND", "NHD"])
+def test_gather_and_copy_pages_bit_exact(layout):
+    """SURVEY 8(f) rank 4 page moves against the oracle: GATHER rows, COPY_PAGES into a second pool with the other
+    layout and back into free pages of the same pool; whole pools compared bit for bit."""
+    b = small_batch(150, [1, 17, 33, 100, 0, 257], q_lens=[1, 5, 33, 40, 0, 1], Hq=4, Hkv=2, D=128, p=16)
+    db = DeviceBatch(b, layout=layout)
+    db.append()
+    k, v = b.full_pool()
+    oracle.kv_append(k, v, b.k_new, b.v_new, b.slot_mapping)
+    want_k, want_v, cu = oracle.kv_gather(k, v, b.block_table, b.seq_lens)
+    k_out = torch.zeros((int(cu[-1]) + 3, 2, 128), dtype=torch.bfloat16, device="cuda")
+    v_out = torch.zeros_like(k_out)
+    mstar.kv_gather(k_out, v_out, db.pool, db.block_table, db.seq_lens, torch.from_numpy(cu).cuda())
+    assert np.array_equal(bits_of(k_out)[:cu[-1]], want_k) and np.array_equal(bits_of(v_out)[:cu[-1]], want_v)
+    assert not bits_of(k_out)[cu[-1]:].any()
+    # pool -> other pool (other layout), sequence 5's pages to ids 0.., one skipped pair
+    other = DeviceBatch(b, layout="NHD" if layout == "HND" else "HND")
+    src = b.block_table[5, :17].astype(np.int64)
+    dst = np.arange(17, dtype=np.int64) * 3 % b.num_pages
+    src_s, dst_s = np.append(src, [2, -1]), np.append(dst, [-1, 2])
+    k2, v2 = b.full_pool()
+    oracle.kv_copy_pages(k2, v2, k, v, dst_s, src_s)
+    mstar.kv_copy_pages(other.pool, db.pool, torch.from_numpy(dst_s).cuda(), torch.from_numpy(src_s).cuda())
+    assert np.array_equal(bits_of(other.k_pool.contiguous()), k2)
+    assert np.array_equal(bits_of(other.v_pool.contiguous()), v2)
+    # same pool: to free pages, then attention through the relabelled block table is bit-identical
+    used = set(b.used_pages.tolist())
+    free = np.array([pg for pg in range(b.num_pages) if pg not in used][:17][::-1], dtype=np.int64)
+    out0, _ = db.prefill()
+    mstar.kv_copy_pages(db.pool, db.pool, torch.from_numpy(free).cuda(), torch.from_numpy(src).cuda())
+    k3, v3 = k.copy(), v.copy()
+    oracle.kv_copy_pages(k3, v3, k, v, free, src)
+    assert np.array_equal(bits_of(db.k_pool.contiguous()), k3) and np.array_equal(bits_of(db.v_pool.contiguous()), v3)
+    db.block_table[5, :17] = torch.from_numpy(free.astype(np.int32)).cuda()
+    out1, _ = db.prefill()
+    assert torch.equal(out0.view(torch.int16), out1.view(torch.int16))
+
+
 # ----------------------------------------------------------------------------- decode
 
 def test_decode_config1_tiny():

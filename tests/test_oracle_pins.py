@@ -56,6 +56,45 @@ def test_append_matches_numpy_scatter_whole_pool_and_roundtrip():
         assert np.array_equal(v1[pages, :, j % b.page_size, :], b.v_new[t0:t0 + n])
 
 
+def test_gather_and_copy_pages_pins():
+    """GATHER == numpy fancy indexing through the block table; GATHER(APPEND(x)) returns x for the new rows;
+    COPY_PAGES == numpy page assignment, other pages keep their bits, negative ids skipped; copying a sequence's
+    pages to fresh ids and pointing the block table at them leaves GATHER (and decode) bit-identical."""
+    b = small_batch(3, [1, 17, 33, 100, 0], q_lens=[1, 5, 33, 40, 0], Hq=4, Hkv=2, D=64, p=16)
+    k, v = b.full_pool()
+    oracle.kv_append(k, v, b.k_new, b.v_new, b.slot_mapping)
+    kg, vg, cu = oracle.kv_gather(k, v, b.block_table, b.seq_lens)
+    assert cu.tolist() == [0, 1, 18, 51, 151, 151]
+    for s in range(b.num_seqs):
+        L, n = int(b.seq_lens[s]), int(b.q_lens[s])
+        j = np.arange(L)
+        pages = b.block_table[s, j // b.page_size]
+        assert np.array_equal(kg[cu[s]:cu[s + 1]], k[pages, :, j % b.page_size, :])
+        assert np.array_equal(vg[cu[s]:cu[s + 1]], v[pages, :, j % b.page_size, :])
+        t0 = int(b.cu_seqlens_q[s])
+        assert np.array_equal(kg[cu[s + 1] - n:cu[s + 1]], b.k_new[t0:t0 + n])
+    # copy pages: sequence 3's pages to unused ids (in reverse order), one skipped pair
+    used = set(b.used_pages.tolist())
+    free = [pg for pg in range(b.num_pages) if pg not in used]
+    src = b.block_table[3, :7].astype(np.int64)
+    dst = np.array(free[:7][::-1], dtype=np.int64)
+    src_s, dst_s = np.append(src, [5, -1]), np.append(dst, [-1, 5])
+    k2, v2 = k.copy(), v.copy()
+    oracle.kv_copy_pages(k2, v2, k, v, dst_s, src_s)
+    k3, v3 = k.copy(), v.copy()
+    k3[dst] = k[src]
+    v3[dst] = v[src]
+    assert np.array_equal(k2, k3) and np.array_equal(v2, v3)
+    bt2 = b.block_table.copy()
+    bt2[3, :7] = dst
+    kg2, vg2, _ = oracle.kv_gather(k2, v2, bt2, b.seq_lens)
+    assert np.array_equal(kg2, kg) and np.array_equal(vg2, vg)
+    q = np.ascontiguousarray(b.q[:b.num_seqs])   # any S query rows
+    o1, l1 = oracle.paged_decode(q, k, v, b.block_table, b.seq_lens, b.scale)
+    o2, l2 = oracle.paged_decode(q, k2, v2, bt2, b.seq_lens, b.scale)
+    assert np.array_equal(o1, o2) and np.array_equal(l1, l2)
+
+
 def test_append_negative_slot_skipped():
     b = small_batch(2, [20, 9], q_lens=[3, 2], Hq=2, Hkv=1, D=64)
     k0, v0 = b.full_pool()
