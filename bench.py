@@ -297,6 +297,19 @@ def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15
         "frac_of_measured_hbm": tot / (ms_both * 1e-3) / 1e9 / hbm_peak,
         "decode_tokens_per_s": (bt.num_seqs + bk.num_seqs) / (ms_both * 1e-3)}
     del dk, ct, ck
+    # shared-prefix cascade on configs[1] (prefix pass with stacked heads + suffix pass + merge)
+    from paper_2606_12688_b200.harness import CascadeDecode
+    d2c = DeviceBatch(b2, device=dev)
+    d2c.append()
+    casc = CascadeDecode(d2c, n_branches=2, shared_tokens=256)
+    ms_c2 = median_ms([casc.run])
+    res["configs[1] as shared-prefix cascade (SURVEY 8(f) rank 3)"] = {
+        "us": ms_c2 * 1e3, "kv_bytes_unique": b2.kv_bytes_unique(),
+        "GBps_unique": b2.kv_bytes_unique() / (ms_c2 * 1e-3) / 1e9,
+        "note": "3 calls: decode over the 256 shared tokens with both branches' queries stacked as grouped heads, "
+                "decode over the private suffixes, mstar_merge_attn_states; shared pages are 5 % of the bytes, so "
+                "the extra launches outweigh the saving at this shape"}
+    del d2c, casc
     # the BAGEL-like denoise (flow) step, 4 requests x 3 CFG labels x 4096 latent tokens,
     # bidirectional block over the cached label context (causal = 0), appended to scratch pages first
     bf = W.flow_step_bagel()

@@ -142,6 +142,23 @@ int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv
                                                 int32_t max_seq_len);
 
 /*
+ * mstar_merge_attn_states: log-sum-exp merge of two normalised attention states over
+ * disjoint key sets, row by row -- the last step of a shared-prefix ("cascade") decode for CFG branches whose
+ * labels reference the same prefix pages:
+ *     M = max(lse_a, lse_b);  out = (e^{lse_a-M} out_a + e^{lse_b-M} out_b) / (e^{lse_a-M} + e^{lse_b-M});
+ *     lse = M + ln(e^{lse_a-M} + e^{lse_b-M})           (natural log; a state with lse = -inf has weight 0)
+ *   out        device, [num_rows][D] bf16 (fp32 with MSTAR_FLAG_OUT_F32); lse_out [num_rows] fp32 or NULL
+ *   out_a      device, [*][D] fp32, lse_a [*] fp32; row r of the result reads row row_map_a[r] of state A
+ *              (row_map_a: device int32 [num_rows], or NULL for the identity)
+ *   out_b      device, [num_rows][D] fp32, lse_b [num_rows] fp32
+ * The two states are the fp32 outputs (MSTAR_FLAG_OUT_F32) and LSEs of two mstar_paged_attn_decode calls: one over
+ * the shared prefix with the branches' queries stacked as grouped heads, one over the private suffixes.
+ */
+int mstar_merge_attn_states(void* out, float* lse_out, const float* out_a, const float* lse_a,
+                            const int32_t* row_map_a, const float* out_b, const float* lse_b, int64_t num_rows,
+                            int32_t head_dim, uint32_t flags, void* stream);
+
+/*
  * mstar_paged_attn_prefill (step a4): many query tokens per sequence, causal over a cached prefix.
  * Query row i (0-based within sequence s, n_s = cu_seqlens_q[s+1]-cu_seqlens_q[s] rows) attends to
  * KV positions j <= (seq_lens[s] - n_s) + i when causal != 0 (bottom-right aligned mask), to all

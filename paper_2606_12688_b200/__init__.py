@@ -9,6 +9,7 @@ Python binding.  Names mirror the C entry points:
     build_slot_mapping   <- mstar_build_slot_mapping
     kv_copy_pages        <- mstar_kv_copy_pages       (page moves pool -> pool)
     kv_gather            <- mstar_kv_gather           (pool -> contiguous rows)
+    merge_attn_states    <- mstar_merge_attn_states   (LSE merge for shared-prefix cascade decode)
 
 There is no CPU fallback: without the built library every call raises ``MstarError``.
 """
@@ -26,6 +27,7 @@ from .binding import (  # noqa: F401
     kv_gather,
     last_launch_count,
     load_library,
+    merge_attn_states,
     paged_attn_decode,
     paged_attn_prefill,
     prefill_workspace_bytes,

@@ -24,6 +24,7 @@ EXPORTS = (
     "mstar_kv_append",
     "mstar_kv_copy_pages",
     "mstar_kv_gather",
+    "mstar_merge_attn_states",
     "mstar_paged_attn_decode_workspace_bytes",
     "mstar_paged_attn_decode",
     "mstar_paged_attn_decode_auto_partitions",
@@ -77,6 +78,9 @@ def load_library() -> ctypes.CDLL:
     lib.mstar_kv_gather.restype = c.c_int
     lib.mstar_kv_gather.argtypes = [c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_int64,
                                     c.c_void_p, c.c_void_p, c.c_int32, c.c_int64, c.c_void_p]
+    lib.mstar_merge_attn_states.restype = c.c_int
+    lib.mstar_merge_attn_states.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
+                                            c.c_void_p, c.c_int64, c.c_int32, c.c_uint32, c.c_void_p]
     lib.mstar_paged_attn_decode_workspace_bytes.restype = c.c_size_t
     lib.mstar_paged_attn_decode_workspace_bytes.argtypes = [c.c_int32] * 4
     lib.mstar_paged_attn_decode_auto_partitions.restype = c.c_int32
@@ -191,6 +195,28 @@ def kv_gather(k_out: torch.Tensor, v_out: torch.Tensor, pool: KVPool, block_tabl
     _check(lib.mstar_kv_gather(_ptr(k_out), _ptr(v_out), ctypes.byref(pool.c), _ptr(block_table),
                                int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens),
                                _ptr(cu_seqlens_out), S, int(k_out.shape[0]), _stream()), "mstar_kv_gather")
+
+
+def merge_attn_states(out: torch.Tensor, out_a: torch.Tensor, lse_a: torch.Tensor, out_b: torch.Tensor,
+                      lse_b: torch.Tensor, row_map_a: Optional[torch.Tensor] = None,
+                      lse_out: Optional[torch.Tensor] = None) -> None:
+    """mstar_merge_attn_states: LSE merge of two fp32 attention states [.., D] into out [N, D] (bf16 or fp32)."""
+    for t, nm in ((out_a, "out_a"), (lse_a, "lse_a"), (out_b, "out_b"), (lse_b, "lse_b")):
+        _want(t, torch.float32, nm)
+    if row_map_a is not None:
+        _want(row_map_a, torch.int32, "row_map_a")
+    if lse_out is not None:
+        _want(lse_out, torch.float32, "lse_out")
+    D = int(out.shape[-1])
+    N = out.numel() // D
+    flags = MSTAR_FLAG_OUT_F32 if out.dtype == torch.float32 else 0
+    if out.dtype not in (torch.float32, torch.bfloat16) or not out.is_contiguous():
+        raise MstarError("out must be contiguous bf16 or fp32")
+    if out_b.numel() != N * D or lse_b.numel() != N:
+        raise MstarError("state B must have the rows of out")
+    lib = load_library()
+    _check(lib.mstar_merge_attn_states(_ptr(out), _ptr(lse_out), _ptr(out_a), _ptr(lse_a), _ptr(row_map_a),
+                                       _ptr(out_b), _ptr(lse_b), N, D, flags, _stream()), "mstar_merge_attn_states")
 
 
 def decode_auto_partitions(num_seqs: int, num_kv_heads: int, max_seq_len: int) -> int:

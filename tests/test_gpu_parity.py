@@ -10,7 +10,7 @@ import torch
 import oracle
 import paper_2606_12688_b200 as mstar
 import workloads as W
-from tests.gpu_util import DeviceBatch, bf16_tensor, bits_of, f64_of
+from tests.gpu_util import CascadeDecode, DeviceBatch, bf16_tensor, bits_of, f64_of
 from tests.util import check_parity, compact_pool_after_append, decode_q, f64_from_bf16_bits
 
 pytestmark = pytest.mark.gpu
@@ -238,6 +238,41 @@ def test_decode_deterministic_and_graph_capturable():
 def test_decode_config2_bagel_cfg_pairs():
     stats = run_decode_case(W.config2_bagel_cfg_decode(), parts_list=(0, 4), check_f32=False)
     print("cfg2", stats)
+
+
+def test_cascade_decode_cfg_branches_and_merge_states():
+    """shared-prefix cascade (stacked-head prefix pass + suffix pass + mstar_merge_attn_states)
+    on configs[1] against the oracle's plain decode; the merge kernel alone against COMBINE incl. empty states."""
+    b = W.config2_bagel_cfg_decode()
+    db = DeviceBatch(b)
+    db.append()
+    want, want_lse = oracle_decode(b)
+    out, lse = CascadeDecode(db, n_branches=2, shared_tokens=256).run()
+    check_parity(f64_of(out), want, "cascade cfg2")
+    assert np.abs(f64_of(lse) - want_lse).max() < 2e-3
+    # merge kernel alone: random states, -inf on either or both sides, row map
+    rng = np.random.default_rng(9)
+    N, D = 37, 128
+    oa, ob = rng.standard_normal((N + 5, D)).astype(np.float32), rng.standard_normal((N, D)).astype(np.float32)
+    la, lb = rng.standard_normal(N + 5).astype(np.float32) * 3, rng.standard_normal(N).astype(np.float32) * 3
+    rmap = rng.permutation(N + 5)[:N].astype(np.int32)
+    la[rmap[0]] = -np.inf
+    lb[1] = -np.inf
+    la[rmap[2]] = lb[2] = -np.inf
+    o = torch.empty((N, D), dtype=torch.float32, device="cuda")
+    l = torch.empty(N, dtype=torch.float32, device="cuda")
+    cu = lambda a: torch.from_numpy(a).cuda()
+    mstar.merge_attn_states(o, cu(oa), cu(la), cu(ob), cu(lb), row_map_a=cu(rmap), lse_out=l)
+    got, got_l = f64_of(o), f64_of(l)
+    for r in range(N):
+        m = np.array([la[rmap[r]], lb[r]], dtype=np.float64)
+        if np.isneginf(m).all():
+            assert not got[r].any() and np.isneginf(got_l[r])
+            continue
+        keep = ~np.isneginf(m)
+        w_out, w_lse = oracle.lse_combine(m[keep], np.ones(int(keep.sum())),
+                                          np.stack([oa[rmap[r]], ob[r]]).astype(np.float64)[keep])
+        assert np.abs(got[r] - w_out).max() < 1e-5 and abs(got_l[r] - w_lse) < 1e-5
 
 
 def test_decode_config4_thinker_and_talker():

@@ -11,7 +11,7 @@ import pytest
 
 import oracle
 import workloads as W
-from tests.util import (brute_force_attention, compact_pool_after_append, dense_kv,
+from tests.util import (brute_force_attention, compact_pool_after_append, decode_q, dense_kv,
                         f64_from_bf16_bits, bf16_bits_from_f32, numpy_scatter)
 
 TOL = 1e-12
@@ -93,6 +93,38 @@ def test_gather_and_copy_pages_pins():
     o1, l1 = oracle.paged_decode(q, k, v, b.block_table, b.seq_lens, b.scale)
     o2, l2 = oracle.paged_decode(q, k2, v2, bt2, b.seq_lens, b.scale)
     assert np.array_equal(o1, o2) and np.array_equal(l1, l2)
+
+
+def test_cascade_identity_stacked_prefix_plus_suffix_merge():
+    """SURVEY 8(f) rank 3 in fp64: decode over the shared prefix with the branches' queries stacked as grouped
+    heads gives each branch's prefix state; merged with its private-suffix state by COMBINE (l = 1) it equals the
+    plain decode over the whole sequence."""
+    B, shared, p = 2, 32, 16
+    lens = [40, 40, 33, 33, 100, 100]
+    rng = np.random.default_rng(77)
+    b = W.make_batch(rng, "cfg", lens, [1] * 6, 4, 2, 64, p, 64, share_with=[-1, 0, -1, 2, -1, 4],
+                     shared_tokens=shared)
+    k, v = compact_pool_after_append(b)
+    q = decode_q(b)
+    full, full_lse = oracle.paged_decode(q, k, v, b.compact_block_table, b.seq_lens, b.scale)
+    S, Hq, Hkv, D = 6, 4, 2, 64
+    G, R = Hq // Hkv, S // B
+    qa = np.zeros((R, Hq * B, D), dtype=np.uint16)
+    for r in range(R):
+        for kvh in range(Hkv):
+            for br in range(B):
+                for g in range(G):
+                    qa[r, kvh * B * G + br * G + g] = q[r * B + br, kvh * G + g]
+    pa, pa_lse = oracle.paged_decode(qa, k, v, b.compact_block_table[::B], np.full(R, shared, np.int32), b.scale)
+    sb, sb_lse = oracle.paged_decode(q, k, v, np.ascontiguousarray(b.compact_block_table[:, shared // p:]),
+                                     b.seq_lens - shared, b.scale)
+    for s in range(S):
+        for h in range(Hq):
+            r, br, kvh, g = s // B, s % B, h // G, h % G
+            ra = kvh * B * G + br * G + g
+            out, lse = oracle.lse_combine(np.array([pa_lse[r, ra], sb_lse[s, h]]), np.ones(2),
+                                          np.stack([pa[r, ra], sb[s, h]]))
+            assert np.abs(out - full[s, h]).max() < 1e-12 and abs(lse - full_lse[s, h]) < 1e-12
 
 
 def test_append_negative_slot_skipped():
