@@ -128,6 +128,9 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
     for (int i = threadIdx.x; i < 2 * SM::kQBytes / 4; i += blockDim.x) reinterpret_cast<uint32_t*>(qbuf_g)[i] = 0u;
     fence_proxy_async_smem();
     __syncthreads();
+    // let the combine grid (launched with programmatic stream serialization) become resident now; it blocks in
+    // griddepcontrol.wait until this grid has completed
+    asm volatile("griddepcontrol.launch_dependents;");
 
     if (warp >= NW) {
         // Two producer warps walk the same item list: warp NW loads the K half of every stage (and Q and the item
@@ -476,6 +479,9 @@ __global__ void __launch_bounds__(128) decode_combine_kernel(const float* __rest
     constexpr int VEC = D / 32;
     const int lane = threadIdx.x & 31;
     const int row = blockIdx.x * 4 + (threadIdx.x >> 5);
+    // programmatic dependent launch: this grid may be resident before the split-K grid has finished; nothing it
+    // reads (partials, piece counts) is valid before this returns
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (row >= n_rows) return;
     const int s = row / Hq;
     const int L = seq_lens[s];
@@ -672,14 +678,28 @@ extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q,
     if (!p.direct) {
         const int n_rows = num_seqs * num_q_heads;
         const int blocks = (n_rows + 3) / 4;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)blocks);
+        cfg.blockDim = dim3(128);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        const float* cO = p.part_O;
+        const float* cm = p.part_m;
+        const float* cl = p.part_l;
+        const int32_t* cpc = p.piece_count;
         if (D == 128)
-            decode_combine_kernel<128><<<blocks, 128, 0, st>>>(p.part_O, p.part_m, p.part_l, seq_lens, p.chunk,
-                                                              p.piece_count, G, p.nparts, num_q_heads, n_rows, out,
-                                                              lse_out, p.out_f32);
+            MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, decode_combine_kernel<128>, cO, cm, cl, seq_lens, p.chunk, cpc,
+                                             (int32_t)G, p.nparts, num_q_heads, (int32_t)n_rows, out, lse_out,
+                                             p.out_f32));
         else
-            decode_combine_kernel<64><<<blocks, 128, 0, st>>>(p.part_O, p.part_m, p.part_l, seq_lens, p.chunk,
-                                                             p.piece_count, G, p.nparts, num_q_heads, n_rows, out,
-                                                             lse_out, p.out_f32);
+            MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, decode_combine_kernel<64>, cO, cm, cl, seq_lens, p.chunk, cpc,
+                                             (int32_t)G, p.nparts, num_q_heads, (int32_t)n_rows, out, lse_out,
+                                             p.out_f32));
         MSTAR_CUDA_OK(cudaGetLastError());
         launch_count_add(1);
     }
