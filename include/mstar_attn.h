@@ -142,6 +142,34 @@ int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv
                                                 int32_t max_seq_len);
 
 /*
+ * Quantised pool ("fp8 K/V pages with per-page scales"; the KV-cache state of
+ * PAPER.md:134 at half the bytes per token).  The pool holds one byte per element: an OCP E4M3 ("fn") code
+ * (sign, 4 exponent bits of bias 7, 3 mantissa bits; 0x7F / 0xFF = NaN, no infinities, largest magnitude 448).
+ * An element's value is  e4m3(code) * scale[page][kv head]  with caller-owned fp32 scales
+ *   k_scale, v_scale   device, [num_pages][Hkv] fp32, positive and finite (not validated).
+ * The pool is described by an mstar_kv_pool whose k_pool / v_pool point at the bytes and whose strides count
+ * elements (= bytes); head_dim 128 only (a token row is one 128-byte line), page_size 16 or 32, strides
+ * multiples of 16.
+ *
+ * mstar_kv_append_fp8: quantise and scatter the step's new rows.  For every element x (bf16) of a row that goes to
+ * (page, h):  y = fp32(x) / scale[page][h]  in IEEE fp32 (round to nearest even);  code = y rounded to nearest
+ * E4M3 value, ties to the even code, magnitudes above 448 (and infinities) saturate to +-448, NaN -> 0x7F.
+ * Arguments as mstar_kv_append; bit-exact by definition (R24-R25).
+ *
+ * mstar_paged_attn_decode_fp8: mstar_paged_attn_decode on the dequantised K and V; all other arguments, the
+ * partition rules and the workspace size are those of mstar_paged_attn_decode.  Codes are converted to bf16
+ * exactly in the kernel; k_scale multiplies the logits of a page, v_scale its probabilities (fp32).  Slots at or
+ * past seq_len may hold any byte.  NaN codes inside a sequence give undefined output.
+ */
+int mstar_kv_append_fp8(const mstar_kv_pool* pool8, const float* k_scale, const float* v_scale, const void* k_new,
+                        const void* v_new, const int64_t* slot_mapping, int64_t num_tokens, void* stream);
+int mstar_paged_attn_decode_fp8(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool8,
+                                const float* k_scale, const float* v_scale, const int32_t* block_table,
+                                int64_t block_table_stride, const int32_t* seq_lens, int32_t num_seqs,
+                                int32_t num_q_heads, int32_t max_seq_len, float scale, int32_t num_partitions,
+                                uint32_t flags, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * mstar_merge_attn_states: log-sum-exp merge of two normalised attention states over
  * disjoint key sets, row by row -- the last step of a shared-prefix ("cascade") decode for CFG branches whose
  * labels reference the same prefix pages:

@@ -69,13 +69,15 @@ def kv_append_fp8(k_pool8, v_pool8, k_scale, v_scale, k_new, v_new, slot_mapping
     _, Hkv, p, D = k_pool8.shape
     kf, vf = bf16_bits_to_f32(k_new), bf16_bits_to_f32(v_new)
     ks, vs = np.asarray(k_scale, dtype=np.float32), np.asarray(v_scale, dtype=np.float32)
-    for t, slot in enumerate(np.asarray(slot_mapping, dtype=np.int64)):
-        if slot < 0:
-            continue
-        page, off = int(slot) // p, int(slot) % p
-        for h in range(Hkv):
-            k_pool8[page, h, off, :] = e4m3_encode(kf[t, h, :] / ks[page, h])  # fp32 / fp32 -> fp32, IEEE RN
-            v_pool8[page, h, off, :] = e4m3_encode(vf[t, h, :] / vs[page, h])
+    slot = np.asarray(slot_mapping, dtype=np.int64)
+    ok = slot >= 0
+    page, off = slot[ok] // p, slot[ok] % p
+    # fp32 / fp32 -> fp32, IEEE round to nearest even, element by element (the scale of the row's page and head)
+    yk = kf[ok] / ks[page][:, :, None]
+    yv = vf[ok] / vs[page][:, :, None]
+    assert yk.dtype == np.float32 and yv.dtype == np.float32
+    k_pool8[page, :, off, :] = e4m3_encode(yk)  # slots are unique within a call (duplicates: caller error, R19)
+    v_pool8[page, :, off, :] = e4m3_encode(yv)
 
 
 def dequant_gather(pool8, scale, block_table_row, L):

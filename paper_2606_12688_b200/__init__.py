@@ -4,6 +4,8 @@ The product is the C-ABI library ``libmstar_attn.so`` (``include/mstar_attn.h``)
 Python binding.  Names mirror the C entry points:
 
     kv_append            <- mstar_kv_append
+    kv_append_fp8        <- mstar_kv_append_fp8        (quantising append into an E4M3 pool)
+    paged_attn_decode_fp8 <- mstar_paged_attn_decode_fp8 (decode over the E4M3 pool)
     paged_attn_decode    <- mstar_paged_attn_decode   (split-K + LSE combine)
     paged_attn_prefill   <- mstar_paged_attn_prefill  (causal over a cached prefix)
     build_slot_mapping   <- mstar_build_slot_mapping
@@ -16,6 +18,7 @@ There is no CPU fallback: without the built library every call raises ``MstarErr
 from .binding import (  # noqa: F401
     EXPORTS,
     KVPool,
+    KVPoolFp8,
     LIB_PATH,
     MSTAR_FLAG_OUT_F32,
     MstarError,
@@ -23,12 +26,14 @@ from .binding import (  # noqa: F401
     decode_auto_partitions,
     decode_workspace_bytes,
     kv_append,
+    kv_append_fp8,
     kv_copy_pages,
     kv_gather,
     last_launch_count,
     load_library,
     merge_attn_states,
     paged_attn_decode,
+    paged_attn_decode_fp8,
     paged_attn_prefill,
     prefill_workspace_bytes,
     status_string,

@@ -22,6 +22,8 @@ MSTAR_FLAG_PREFILL_MMA_SYNC = 2
 
 EXPORTS = (
     "mstar_kv_append",
+    "mstar_kv_append_fp8",
+    "mstar_paged_attn_decode_fp8",
     "mstar_kv_copy_pages",
     "mstar_kv_gather",
     "mstar_merge_attn_states",
@@ -72,6 +74,14 @@ def load_library() -> ctypes.CDLL:
     lib.mstar_kv_append.restype = c.c_int
     lib.mstar_kv_append.argtypes = [c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p, c.c_void_p, c.c_int64,
                                     c.c_void_p]
+    lib.mstar_kv_append_fp8.restype = c.c_int
+    lib.mstar_kv_append_fp8.argtypes = [c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
+                                        c.c_void_p, c.c_int64, c.c_void_p]
+    lib.mstar_paged_attn_decode_fp8.restype = c.c_int
+    lib.mstar_paged_attn_decode_fp8.argtypes = [
+        c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p, c.c_void_p, c.c_int64,
+        c.c_void_p, c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_uint32, c.c_void_p, c.c_size_t,
+        c.c_void_p]
     lib.mstar_kv_copy_pages.restype = c.c_int
     lib.mstar_kv_copy_pages.argtypes = [c.POINTER(_KvPoolStruct), c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p,
                                         c.c_int64, c.c_void_p]
@@ -158,6 +168,65 @@ class KVPool:
         self.c = _KvPoolStruct(
             k_pool.data_ptr(), v_pool.data_ptr(), self.num_pages, self.page_size, self.num_kv_heads,
             self.head_dim, int(k_pool.stride(0)), int(k_pool.stride(1)), int(k_pool.stride(2)))
+
+
+class KVPoolFp8:
+    """The quantised pool: two uint8 tensors of E4M3 codes viewed as [num_pages, Hkv, page_size, 128] plus fp32
+    scales [num_pages, Hkv] (value = e4m3(code) * scale[page][head])."""
+
+    def __init__(self, k_pool: torch.Tensor, v_pool: torch.Tensor, k_scale: torch.Tensor, v_scale: torch.Tensor):
+        for t, nm in ((k_pool, "k_pool"), (v_pool, "v_pool")):
+            if not t.is_cuda or t.dtype != torch.uint8 or t.dim() != 4 or t.stride(3) != 1:
+                raise MstarError("%s must be a CUDA uint8 tensor [num_pages, Hkv, page_size, D] with unit inner stride" % nm)
+        if k_pool.shape != v_pool.shape or k_pool.stride() != v_pool.stride():
+            raise MstarError("k_pool and v_pool must share shape and strides")
+        self.k_pool, self.v_pool = k_pool, v_pool
+        self.num_pages, self.num_kv_heads, self.page_size, self.head_dim = (int(x) for x in k_pool.shape)
+        for t, nm in ((k_scale, "k_scale"), (v_scale, "v_scale")):
+            _want(t, torch.float32, nm)
+            if tuple(t.shape) != (self.num_pages, self.num_kv_heads):
+                raise MstarError("%s must be [num_pages, Hkv]" % nm)
+        self.k_scale, self.v_scale = k_scale, v_scale
+        self.c = _KvPoolStruct(
+            k_pool.data_ptr(), v_pool.data_ptr(), self.num_pages, self.page_size, self.num_kv_heads,
+            self.head_dim, int(k_pool.stride(0)), int(k_pool.stride(1)), int(k_pool.stride(2)))
+
+
+def kv_append_fp8(pool: KVPoolFp8, k_new: torch.Tensor, v_new: torch.Tensor, slot_mapping: torch.Tensor) -> None:
+    """mstar_kv_append_fp8: quantise k_new/v_new [T,Hkv,D] bf16 to E4M3 codes at slot_mapping [T] int64."""
+    _want(k_new, torch.bfloat16, "k_new"); _want(v_new, torch.bfloat16, "v_new")
+    _want(slot_mapping, torch.int64, "slot_mapping")
+    T = int(slot_mapping.shape[0])
+    if tuple(k_new.shape) != (T, pool.num_kv_heads, pool.head_dim) or k_new.shape != v_new.shape:
+        raise MstarError("k_new/v_new must be [T, Hkv, D]")
+    lib = load_library()
+    _check(lib.mstar_kv_append_fp8(ctypes.byref(pool.c), _ptr(pool.k_scale), _ptr(pool.v_scale), _ptr(k_new),
+                                   _ptr(v_new), _ptr(slot_mapping), T, _stream()), "mstar_kv_append_fp8")
+
+
+def paged_attn_decode_fp8(out: torch.Tensor, q: torch.Tensor, pool: KVPoolFp8, block_table: torch.Tensor,
+                          seq_lens: torch.Tensor, max_seq_len: int, scale: float, num_partitions: int = 0,
+                          workspace: Optional[torch.Tensor] = None, lse_out: Optional[torch.Tensor] = None) -> None:
+    """mstar_paged_attn_decode_fp8: decode over the quantised pool; arguments as paged_attn_decode."""
+    _want(q, torch.bfloat16, "q"); _want(block_table, torch.int32, "block_table")
+    _want(seq_lens, torch.int32, "seq_lens")
+    S, Hq, D = (int(x) for x in q.shape)
+    flags = 0
+    if out.dtype == torch.float32:
+        flags |= MSTAR_FLAG_OUT_F32
+    elif out.dtype != torch.bfloat16:
+        raise MstarError("out must be bf16 or fp32")
+    if not out.is_cuda or not out.is_contiguous() or tuple(out.shape) != (S, Hq, D):
+        raise MstarError("out must be a contiguous CUDA tensor [S, Hq, D]")
+    if lse_out is not None:
+        _want(lse_out, torch.float32, "lse_out")
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    lib = load_library()
+    _check(lib.mstar_paged_attn_decode_fp8(
+        _ptr(out), _ptr(lse_out), _ptr(q), ctypes.byref(pool.c), _ptr(pool.k_scale), _ptr(pool.v_scale),
+        _ptr(block_table), int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens), S, Hq,
+        int(max_seq_len), float(scale), int(num_partitions), flags, _ptr(workspace), ws_bytes, _stream()),
+        "mstar_paged_attn_decode_fp8")
 
 
 def kv_append(pool: KVPool, k_new: torch.Tensor, v_new: torch.Tensor, slot_mapping: torch.Tensor) -> None:

@@ -48,19 +48,23 @@ struct DecodeParams {
     int32_t balanced;
     int32_t per_min;
     int32_t* piece_count;
+    // quantised pool (FP8 instantiations): value = e4m3(code) * scale[page][kv head]
+    const float* k_scale;
+    const float* v_scale;
 };
 
 struct ItemInfo {
     int32_t s, kvh, part, tok0, ntok;
 };
 
-template <int D, int GH>
+template <int D, int GH, int EB>  // EB = bytes per pool element (2 = bf16, 1 = e4m3)
 struct DecodeSmem {
-    static constexpr int kStageBytes = 2 * kDecodeTok * D * 2;
+    static constexpr int kStageBytes = 2 * kDecodeTok * D * EB;
+    static constexpr int kScaleBytes = EB == 1 ? kMaxStages * 2 * 4 * 4 : 0;  // [stage][K|V][page of the stage] fp32
     static constexpr int kQBytes = GH * D * 2;
     static constexpr int kMergeBytes = kDecodeConsumerWarps * GH * (D + 2) * 4;
     // fixed part after the ring: Q slots, merge buffer, barriers, item info
-    static constexpr int kFixed = 2 * kQBytes + kMergeBytes + (2 * kMaxStages + 4) * 8 + 2 * 32;
+    static constexpr int kFixed = 2 * kQBytes + kMergeBytes + (2 * kMaxStages + 4) * 8 + 2 * 32 + kScaleBytes;
     static size_t bytes(int nstages, int S) {
         return 1024 + (size_t)nstages * kStageBytes + kFixed + (size_t)(S + 1) * 4 + 16;
     }
@@ -78,17 +82,30 @@ __device__ __forceinline__ void store_out_vec(void* out, int out_f32, size_t idx
     }
 }
 
-template <int D, int PAGE, int GH>
+// two E4M3 codes (bytes of w picked by the PRMT selector into the high byte of each 16-bit lane) -> two bf16,
+// exactly: sign to bit 15, the 7 exponent/mantissa bits to bits [10:4] (a bf16 with exponent bias 127 instead of
+// 7, subnormal codes land on bf16 subnormals), then one packed multiply by 2^120 fixes the bias.
+template <uint32_t SEL>
+__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t w) {
+    const uint32_t y = __byte_perm(w, 0u, SEL);
+    uint32_t x = (y & 0x80008000u) | ((y >> 4) & 0x07f007f0u);
+    asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(x) : "r"(x), "r"(0x7B807B80u));
+    return x;
+}
+
+template <int D, int PAGE, int GH, bool FP8>
 __global__ void __launch_bounds__(kDecodeThreads, 1)
 decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_constant__ CUtensorMap vmap,
                      const DecodeParams p) {
     constexpr int NW = kDecodeConsumerWarps;
     constexpr int TOK = kDecodeTok;
     constexpr int PPS = TOK / PAGE;  // pages per stage
-    constexpr int NH = D / 64;       // 64-column halves per row
-    constexpr int HT = TOK * 128;    // bytes of one half tile (TOK rows x 128 B)
-    constexpr int KBYTES = NH * HT;  // K part of a stage
-    using SM = DecodeSmem<D, GH>;
+    constexpr int EB = FP8 ? 1 : 2;    // bytes per pool element
+    constexpr int NH = D * EB / 128;   // 128-byte column slices per row (bf16: 64-column halves)
+    constexpr int HT = TOK * 128;      // bytes of one slice tile (TOK rows x 128 B)
+    constexpr int KBYTES = NH * HT;    // K part of a stage
+    using SM = DecodeSmem<D, GH, EB>;
+    static_assert(!FP8 || D == 128, "fp8 pool: one 128-byte line per token row");
     constexpr int VEC = D / 32;
 
     extern __shared__ uint8_t smem_raw[];
@@ -105,7 +122,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
     uint64_t* bars_g = reinterpret_cast<uint64_t*>(g_after + 2 * SM::kQBytes + SM::kMergeBytes);
     const uint32_t bars = smem_u32(bars_g);
     ItemInfo* info = reinterpret_cast<ItemInfo*>(bars_g + 2 * kMaxStages + 4);
-    int32_t* cum = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(info) + 2 * 32);
+    float* sc_ring = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(info) + 2 * 32);  // FP8 only
+    int32_t* cum = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(info) + 2 * 32 + SM::kScaleBytes);
     auto full_bar = [&](int st) { return bars + 8u * st; };
     auto empty_bar = [&](int st) { return bars + 8u * (kMaxStages + st); };
     auto qfull_bar = [&](int qs) { return bars + 8u * (2 * kMaxStages + qs); };
@@ -194,8 +212,14 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     const int npg1 = min(PPS, (rem - TOK + PAGE - 1) / PAGE);
                     if (lane < OPS && op_page < npg1) pg_next = __ldg(bt + (t + 1) * PPS + op_page);
                 }
+                float pg_scale = 0.f;  // FP8: requested before the ring wait, which hides its latency
+                if (FP8 && pg >= 0) pg_scale = __ldg((op_isv ? p.v_scale : p.k_scale) + (size_t)pg * p.Hkv + kvh);
                 mbar_wait(empty_bar(st), ph ^ 1);
-                if (lane == 0) mbar_arrive_expect_tx(full_bar(st), (uint32_t)(npg * PAGE * D * 2));
+                if (FP8) {
+                    if (pg >= 0) sc_ring[(st * 2 + op_isv) * 4 + op_page] = pg_scale;
+                    __syncwarp();  // the scales are ordered before lane 0's (releasing) arrive
+                }
+                if (lane == 0) mbar_arrive_expect_tx(full_bar(st), (uint32_t)(npg * PAGE * D * EB));
                 __syncwarp();
                 if (pg >= 0)
                     tma_load_4d(ring + st * SM::kStageBytes + op_off, op_isv ? &vmap : &kmap, full_bar(st),
@@ -278,6 +302,9 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         const uint32_t k_csel = (lane >> 3) & 1;
         const uint32_t v_row = w * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
         const uint32_t v_csel = lane >> 4;
+        // FP8: one 16-byte chunk = 16 d values of a token; ldmatrix.x4 = (tokens 0-7 | 8-15) x (chunk c | c + 1)
+        const uint32_t f_row = w * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
+        const uint32_t f_csel = lane >> 4;
 
         int st = 0, ph = 0, qs = 0, qph = 0;
         while (true) {
@@ -290,11 +317,15 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 const uint16_t* qb = qbuf_g + qs * (SM::kQBytes / 2);
 #pragma unroll
                 for (int ks = 0; ks < D / 16; ++ks) {
-                    qa[ks][0] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + 2 * t4);
-                    qa[ks][2] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + 8 + 2 * t4);
+                    // FP8: this lane's K bytes of a 16-wide d block are d = 4*t4 .. 4*t4+3 (one ldmatrix word), so
+                    // the contraction index is permuted: MMA k-slots (2t4, 2t4+1 | 2t4+8, 2t4+9) <-> d (4t4, 4t4+1 |
+                    // 4t4+2, 4t4+3); Q takes the same permutation
+                    const int c0 = FP8 ? 4 * t4 : 2 * t4, c1 = FP8 ? 4 * t4 + 2 : 8 + 2 * t4;
+                    qa[ks][0] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + c0);
+                    qa[ks][2] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + c1);
                     if (GH == 16) {
-                        qa[ks][1] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + 2 * t4);
-                        qa[ks][3] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + 8 + 2 * t4);
+                        qa[ks][1] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + c0);
+                        qa[ks][3] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + c1);
                     } else {
                         qa[ks][1] = 0u;
                         qa[ks][3] = 0u;
@@ -322,13 +353,35 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     float sc[2][4];
 #pragma unroll
                     for (int b = 0; b < 2; ++b) sc[b][0] = sc[b][1] = sc[b][2] = sc[b][3] = 0.f;
+                    if constexpr (FP8) {
 #pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks) {
-                        const uint32_t chunk = 2 * ks + k_csel;
-                        uint32_t b0, b1, b2, b3;
-                        ldsm_x4(kb + (chunk >> 3) * HT + swz128(k_row, chunk & 7), b0, b1, b2, b3);
-                        mma_bf16_16816(sc[0], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b0, b1);
-                        mma_bf16_16816(sc[1], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b2, b3);
+                        for (int c2 = 0; c2 < D / 32; ++c2) {
+                            uint32_t r0, r1, r2, r3;
+                            ldsm_x4(kb + swz128(f_row, 2 * c2 + f_csel), r0, r1, r2, r3);
+                            const int ka = 2 * c2, kc = 2 * c2 + 1;
+                            mma_bf16_16816(sc[0], qa[ka][0], qa[ka][1], qa[ka][2], qa[ka][3],
+                                           e4m3x2_to_bf16x2<0x1404>(r0), e4m3x2_to_bf16x2<0x3424>(r0));
+                            mma_bf16_16816(sc[1], qa[ka][0], qa[ka][1], qa[ka][2], qa[ka][3],
+                                           e4m3x2_to_bf16x2<0x1404>(r1), e4m3x2_to_bf16x2<0x3424>(r1));
+                            mma_bf16_16816(sc[0], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
+                                           e4m3x2_to_bf16x2<0x1404>(r2), e4m3x2_to_bf16x2<0x3424>(r2));
+                            mma_bf16_16816(sc[1], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
+                                           e4m3x2_to_bf16x2<0x1404>(r3), e4m3x2_to_bf16x2<0x3424>(r3));
+                        }
+                        const float ksc = sc_ring[(st * 2 + 0) * 4 + (w * 16) / PAGE];  // this warp's page
+#pragma unroll
+                        for (int b = 0; b < 2; ++b) {
+                            sc[b][0] *= ksc; sc[b][1] *= ksc; sc[b][2] *= ksc; sc[b][3] *= ksc;
+                        }
+                    } else {
+#pragma unroll
+                        for (int ks = 0; ks < D / 16; ++ks) {
+                            const uint32_t chunk = 2 * ks + k_csel;
+                            uint32_t b0, b1, b2, b3;
+                            ldsm_x4(kb + (chunk >> 3) * HT + swz128(k_row, chunk & 7), b0, b1, b2, b3);
+                            mma_bf16_16816(sc[0], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b0, b1);
+                            mma_bf16_16816(sc[1], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b2, b3);
+                        }
                     }
                     // ---- mask the ragged tail (slots >= seq_len may hold anything, incl. NaN)
                     uint32_t vmask_lo = 0xffffffffu, vmask_hi = 0xffffffffu;
@@ -355,9 +408,11 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     const float p10 = fast_exp2(sc[1][0] * p.scale_log2 - ms0);
                     const float p11 = fast_exp2(sc[1][1] * p.scale_log2 - ms0);
                     l0 = l0 * a0 + (p00 + p01) + (p10 + p11);
+                    // FP8: the page's V scale goes into P (the row sum l keeps the unscaled probabilities)
+                    const float vsc = FP8 ? sc_ring[(st * 2 + 1) * 4 + (w * 16) / PAGE] : 1.f;
                     uint32_t pa[4];
-                    pa[0] = pack_bf16x2(p00, p01);
-                    pa[2] = pack_bf16x2(p10, p11);
+                    pa[0] = pack_bf16x2(p00 * vsc, p01 * vsc);
+                    pa[2] = pack_bf16x2(p10 * vsc, p11 * vsc);
                     pa[1] = 0u;
                     pa[3] = 0u;
                     float a1 = 1.f;
@@ -374,15 +429,27 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                         const float q10 = fast_exp2(sc[1][2] * p.scale_log2 - ms1);
                         const float q11 = fast_exp2(sc[1][3] * p.scale_log2 - ms1);
                         l1 = l1 * a1 + (q00 + q01) + (q10 + q11);
-                        pa[1] = pack_bf16x2(q00, q01);
-                        pa[3] = pack_bf16x2(q10, q11);
+                        pa[1] = pack_bf16x2(q00 * vsc, q01 * vsc);
+                        pa[3] = pack_bf16x2(q10 * vsc, q11 * vsc);
                     }
                     // ---- O = O * alpha + P V
+                    uint32_t fr[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
                     for (int jj = 0; jj < D / 16; ++jj) {
-                        const uint32_t chunk = 2 * jj + v_csel;
                         uint32_t b0, b1, b2, b3;
-                        ldsm_x4_trans(vb + (chunk >> 3) * HT + swz128(v_row, chunk & 7), b0, b1, b2, b3);
+                        if constexpr (FP8) {
+                            // transposed 8x8 b16 matrices = byte pairs: this lane gets V[2t4 | 2t4+1][2g | 2g+1] of
+                            // a 16-wide d block; n-block 2jj takes the even d (n = g <-> d = 2g), 2jj+1 the odd d
+                            if ((jj & 1) == 0) ldsm_x4_trans(vb + swz128(f_row, jj + f_csel), fr[0], fr[1], fr[2], fr[3]);
+                            const uint32_t lo = fr[(jj & 1) * 2], hi = fr[(jj & 1) * 2 + 1];
+                            b0 = e4m3x2_to_bf16x2<0x2404>(lo);
+                            b1 = e4m3x2_to_bf16x2<0x2404>(hi);
+                            b2 = e4m3x2_to_bf16x2<0x3414>(lo);
+                            b3 = e4m3x2_to_bf16x2<0x3414>(hi);
+                        } else {
+                            const uint32_t chunk = 2 * jj + v_csel;
+                            ldsm_x4_trans(vb + (chunk >> 3) * HT + swz128(v_row, chunk & 7), b0, b1, b2, b3);
+                        }
                         if (nv < 16) {  // 0 * NaN guard: zero V rows that hold no token
                             b0 &= vmask_lo; b1 &= vmask_hi; b2 &= vmask_lo; b3 &= vmask_hi;
                         }
@@ -410,9 +477,19 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 float* mo = merge_O + (size_t)w * GH * D;
 #pragma unroll
                 for (int j = 0; j < D / 8; ++j) {
-                    *reinterpret_cast<float2*>(mo + g * D + j * 8 + 2 * t4) = make_float2(o[j][0], o[j][1]);
-                    if (GH == 16)
-                        *reinterpret_cast<float2*>(mo + (g + 8) * D + j * 8 + 2 * t4) = make_float2(o[j][2], o[j][3]);
+                    if constexpr (FP8) {  // n-blocks 2c | 2c+1 hold the even | odd d of block c: d = 16c + 4t4 + 0..3
+                        if (j & 1) continue;
+                        *reinterpret_cast<float4*>(mo + g * D + j * 8 + 4 * t4) =
+                            make_float4(o[j][0], o[j + 1][0], o[j][1], o[j + 1][1]);
+                        if (GH == 16)
+                            *reinterpret_cast<float4*>(mo + (g + 8) * D + j * 8 + 4 * t4) =
+                                make_float4(o[j][2], o[j + 1][2], o[j][3], o[j + 1][3]);
+                    } else {
+                        *reinterpret_cast<float2*>(mo + g * D + j * 8 + 2 * t4) = make_float2(o[j][0], o[j][1]);
+                        if (GH == 16)
+                            *reinterpret_cast<float2*>(mo + (g + 8) * D + j * 8 + 2 * t4) =
+                                make_float2(o[j][2], o[j][3]);
+                    }
                 }
                 if (t4 == 0) {
                     merge_m[w * GH + g] = m0 * p.scale_log2;
@@ -566,16 +643,16 @@ static void partition_plan(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t 
     if (num_partitions > 0 && *nparts > num_partitions) *nparts = num_partitions;
 }
 
-template <int D, int PAGE, int GH>
+template <int D, int PAGE, int GH, bool FP8>
 static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, cudaStream_t stream) {
-    using SM = DecodeSmem<D, GH>;
+    using SM = DecodeSmem<D, GH, FP8 ? 1 : 2>;
     const int max_smem = device_max_smem_optin();
     int nstages = (int)(((int64_t)max_smem - 1024 - SM::kFixed - (int64_t)(p.S + 1) * 4 - 16) / SM::kStageBytes);
     if (nstages > kMaxStages) nstages = kMaxStages;
     if (nstages < 2) return MSTAR_ERR_UNSUPPORTED;
     p.nstages = nstages;
     const size_t smem = SM::bytes(nstages, p.S);
-    auto kern = decode_splitk_kernel<D, PAGE, GH>;
+    auto kern = decode_splitk_kernel<D, PAGE, GH, FP8>;
     static bool attr_set = false;  // per instantiation
     if (!attr_set) {
         MSTAR_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
@@ -607,15 +684,17 @@ extern "C" size_t mstar_paged_attn_decode_workspace_bytes(int32_t num_seqs, int3
     return 256 + rows * head_dim * 4 + 2 * rows * 4 + 256 + (size_t)num_seqs * num_q_heads * 4;
 }
 
-extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool,
-                                       const int32_t* block_table, int64_t block_table_stride,
-                                       const int32_t* seq_lens, int32_t num_seqs, int32_t num_q_heads,
-                                       int32_t max_seq_len, float scale, int32_t num_partitions, uint32_t flags,
-                                       void* workspace, size_t workspace_bytes, void* stream) {
+// bf16 pool (k_scale == v_scale == NULL, fp8 false) or quantised pool
+static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, void* out, float* lse_out,
+                        const void* q, const mstar_kv_pool* pool, const int32_t* block_table,
+                        int64_t block_table_stride, const int32_t* seq_lens, int32_t num_seqs, int32_t num_q_heads,
+                        int32_t max_seq_len, float scale, int32_t num_partitions, uint32_t flags, void* workspace,
+                        size_t workspace_bytes, void* stream) {
     using namespace mstar;
     launch_count_reset();
-    int rc = check_pool(pool);
+    int rc = fp8 ? check_pool_fp8(pool) : check_pool(pool);
     if (rc != MSTAR_OK) return rc;
+    if (fp8 && (!k_scale || !v_scale || !aligned(k_scale, 4) || !aligned(v_scale, 4))) return MSTAR_ERR_INVALID_ARG;
     if (flags & ~MSTAR_FLAG_OUT_F32) return MSTAR_ERR_INVALID_ARG;
     if (num_seqs < 0 || num_q_heads <= 0 || max_seq_len < 0 || num_partitions < 0) return MSTAR_ERR_INVALID_ARG;
     if (!(scale > 0.f) || !(scale < 3.0e38f)) return MSTAR_ERR_INVALID_ARG;  // positive and finite
@@ -655,23 +734,28 @@ extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q,
     p.out = out;
     p.lse = lse_out;
     p.out_f32 = (flags & MSTAR_FLAG_OUT_F32) ? 1 : 0;
+    p.k_scale = k_scale;
+    p.v_scale = v_scale;
 
     PoolMaps maps;
-    rc = get_pool_maps(pool, &maps);
+    rc = fp8 ? get_pool_maps_fp8(pool, &maps) : get_pool_maps(pool, &maps);
     if (rc != MSTAR_OK) return rc;
 
     const int64_t max_items64 = (int64_t)num_seqs * p.nparts * pool->num_kv_heads;
     const int max_items = max_items64 > (1 << 30) ? (1 << 30) : (int)max_items64;
     cudaStream_t st = (cudaStream_t)stream;
     const bool g16 = G > 8;
-#define MSTAR_DECODE_CASE(DD, PP)                                                                  \
-    if (D == DD && PAGE == PP)                                                                     \
-        rc = g16 ? launch_decode<DD, PP, 16>(maps, p, max_items, st) : launch_decode<DD, PP, 8>(maps, p, max_items, st);
+#define MSTAR_DECODE_CASE(DD, PP, F8)                                                    \
+    if (D == DD && PAGE == PP && fp8 == F8)                                              \
+        rc = g16 ? launch_decode<DD, PP, 16, F8>(maps, p, max_items, st)                 \
+                 : launch_decode<DD, PP, 8, F8>(maps, p, max_items, st);
     rc = MSTAR_ERR_UNSUPPORTED;
-    MSTAR_DECODE_CASE(128, 16)
-    MSTAR_DECODE_CASE(128, 32)
-    MSTAR_DECODE_CASE(64, 16)
-    MSTAR_DECODE_CASE(64, 32)
+    MSTAR_DECODE_CASE(128, 16, false)
+    MSTAR_DECODE_CASE(128, 32, false)
+    MSTAR_DECODE_CASE(64, 16, false)
+    MSTAR_DECODE_CASE(64, 32, false)
+    MSTAR_DECODE_CASE(128, 16, true)
+    MSTAR_DECODE_CASE(128, 32, true)
 #undef MSTAR_DECODE_CASE
     if (rc != MSTAR_OK) return rc;
 
@@ -704,4 +788,25 @@ extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q,
         launch_count_add(1);
     }
     return MSTAR_OK;
+}
+
+extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool,
+                                       const int32_t* block_table, int64_t block_table_stride,
+                                       const int32_t* seq_lens, int32_t num_seqs, int32_t num_q_heads,
+                                       int32_t max_seq_len, float scale, int32_t num_partitions, uint32_t flags,
+                                       void* workspace, size_t workspace_bytes, void* stream) {
+    return decode_entry(false, nullptr, nullptr, out, lse_out, q, pool, block_table, block_table_stride, seq_lens,
+                        num_seqs, num_q_heads, max_seq_len, scale, num_partitions, flags, workspace,
+                        workspace_bytes, stream);
+}
+
+extern "C" int mstar_paged_attn_decode_fp8(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool8,
+                                           const float* k_scale, const float* v_scale, const int32_t* block_table,
+                                           int64_t block_table_stride, const int32_t* seq_lens, int32_t num_seqs,
+                                           int32_t num_q_heads, int32_t max_seq_len, float scale,
+                                           int32_t num_partitions, uint32_t flags, void* workspace,
+                                           size_t workspace_bytes, void* stream) {
+    return decode_entry(true, k_scale, v_scale, out, lse_out, q, pool8, block_table, block_table_stride, seq_lens,
+                        num_seqs, num_q_heads, max_seq_len, scale, num_partitions, flags, workspace,
+                        workspace_bytes, stream);
 }

@@ -24,6 +24,20 @@ int check_pool(const mstar_kv_pool* pool) {
     return MSTAR_OK;
 }
 
+int check_pool_fp8(const mstar_kv_pool* pool) {
+    if (!pool || !pool->k_pool || !pool->v_pool) return MSTAR_ERR_INVALID_ARG;
+    if (pool->num_pages <= 0 || pool->num_kv_heads <= 0) return MSTAR_ERR_INVALID_ARG;
+    if (pool->page_size != 16 && pool->page_size != 32) return MSTAR_ERR_UNSUPPORTED;
+    if (pool->head_dim != 128) return MSTAR_ERR_UNSUPPORTED;
+    if (!aligned(pool->k_pool, 128) || !aligned(pool->v_pool, 128)) return MSTAR_ERR_INVALID_ARG;
+    if (pool->stride_page <= 0 || pool->stride_head <= 0 || pool->stride_token < pool->head_dim)
+        return MSTAR_ERR_INVALID_ARG;
+    if (pool->stride_page % 16 || pool->stride_head % 16 || pool->stride_token % 16) return MSTAR_ERR_INVALID_ARG;
+    if (pool->num_pages * (int64_t)pool->num_kv_heads * pool->page_size >= (int64_t(1) << 31))
+        return MSTAR_ERR_UNSUPPORTED;
+    return MSTAR_OK;
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -43,9 +57,21 @@ static EncodeTiledFn encode_fn() {
     return fn;
 }
 
-static int encode_pool_map(void* base, const mstar_kv_pool* pool, CUtensorMap* out) {
+static int encode_pool_map(void* base, const mstar_kv_pool* pool, int elem_bytes, CUtensorMap* out) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return MSTAR_ERR_CUDA;
+    if (elem_bytes == 1) {
+        cuuint64_t dims[4] = {(cuuint64_t)pool->head_dim, (cuuint64_t)pool->page_size,
+                              (cuuint64_t)pool->num_kv_heads, (cuuint64_t)pool->num_pages};
+        cuuint64_t strides[3] = {(cuuint64_t)pool->stride_token, (cuuint64_t)pool->stride_head,
+                                 (cuuint64_t)pool->stride_page};
+        cuuint32_t box[4] = {128, (cuuint32_t)pool->page_size, 1, 1};
+        cuuint32_t estr[4] = {1, 1, 1, 1};
+        CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, base, dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        return r == CUDA_SUCCESS ? MSTAR_OK : MSTAR_ERR_INVALID_ARG;
+    }
     cuuint64_t dims[4] = {(cuuint64_t)pool->head_dim, (cuuint64_t)pool->page_size, (cuuint64_t)pool->num_kv_heads,
                           (cuuint64_t)pool->num_pages};
     cuuint64_t strides[3] = {(cuuint64_t)pool->stride_token * 2, (cuuint64_t)pool->stride_head * 2,
@@ -60,6 +86,7 @@ static int encode_pool_map(void* base, const mstar_kv_pool* pool, CUtensorMap* o
 
 struct CacheEntry {
     mstar_kv_pool key;
+    int elem_bytes;
     PoolMaps maps;
 };
 static std::mutex g_cache_mu;
@@ -71,18 +98,23 @@ static bool same_pool(const mstar_kv_pool& a, const mstar_kv_pool& b) {
            a.stride_page == b.stride_page && a.stride_head == b.stride_head && a.stride_token == b.stride_token;
 }
 
-int get_pool_maps(const mstar_kv_pool* pool, PoolMaps* out) {
+static int pool_maps(const mstar_kv_pool* pool, int elem_bytes, PoolMaps* out);
+int get_pool_maps(const mstar_kv_pool* pool, PoolMaps* out) { return pool_maps(pool, 2, out); }
+int get_pool_maps_fp8(const mstar_kv_pool* pool, PoolMaps* out) { return pool_maps(pool, 1, out); }
+
+static int pool_maps(const mstar_kv_pool* pool, int elem_bytes, PoolMaps* out) {
     std::lock_guard<std::mutex> lock(g_cache_mu);
     for (const CacheEntry& e : g_cache)
-        if (same_pool(e.key, *pool)) {
+        if (e.elem_bytes == elem_bytes && same_pool(e.key, *pool)) {
             *out = e.maps;
             return MSTAR_OK;
         }
     CacheEntry e;
     e.key = *pool;
-    int rc = encode_pool_map(pool->k_pool, pool, &e.maps.k);
+    e.elem_bytes = elem_bytes;
+    int rc = encode_pool_map(pool->k_pool, pool, elem_bytes, &e.maps.k);
     if (rc != MSTAR_OK) return rc;
-    rc = encode_pool_map(pool->v_pool, pool, &e.maps.v);
+    rc = encode_pool_map(pool->v_pool, pool, elem_bytes, &e.maps.v);
     if (rc != MSTAR_OK) return rc;
     if (g_cache.size() >= 64) g_cache.erase(g_cache.begin());
     g_cache.push_back(e);

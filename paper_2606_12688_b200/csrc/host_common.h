@@ -17,6 +17,8 @@ inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_
 
 // Validates the pool geometry common to all entry points.  Returns MSTAR_OK or a negative status.
 int check_pool(const mstar_kv_pool* pool);
+// The same for a quantised (one byte per element) pool: head_dim 128 only, strides multiples of 16.
+int check_pool_fp8(const mstar_kv_pool* pool);
 
 // One tensor map per pool tensor: 4-D view (D, page_size, Hkv, num_pages) of bf16 with a
 // (64, page_size, 1, 1) box and 128-B swizzle, so that a (page, kv head, 64-column half) slab lands in
@@ -27,6 +29,9 @@ struct PoolMaps {
     CUtensorMap v;
 };
 int get_pool_maps(const mstar_kv_pool* pool, PoolMaps* out);
+// Quantised pool: 4-D view (D, page_size, Hkv, num_pages) of bytes with a (128, page_size, 1, 1) box and 128-B
+// swizzle: a (page, kv head) slab lands as page_size rows of 128 B, one row per token.
+int get_pool_maps_fp8(const mstar_kv_pool* pool, PoolMaps* out);
 
 // 3-D view (D, Hq, total_rows) of a contiguous [rows][Hq][D] bf16 tensor with a (64, 1, box_rows) box,
 // 128-B swizzle.  Not cached (cheap, pointer changes every call).

@@ -1,0 +1,133 @@
+"""GPU parity of the quantised (fp8 E4M3) K/V pool against oracle/fp8.py: the quantising
+append bit-exact over the whole pool, decode within the gates of DESIGN.md R11 on the same codes.  Needs a B200."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_12688_b200 as mstar
+import workloads as W
+from oracle import fp8 as ofp8
+from tests.gpu_util import DeviceBatchFp8, bf16_tensor, f64_of
+from tests.util import check_parity, decode_q
+
+pytestmark = pytest.mark.gpu
+
+
+def small_batch(seed, lens, Hq=8, Hkv=2, p=16, pool=None, **kw):
+    rng = np.random.default_rng(seed)
+    q_lens = [min(1, l) for l in lens]
+    pages = sum((l + p - 1) // p for l in lens)
+    return W.make_batch(rng, "t8", lens, q_lens, Hq, Hkv, 128, p, pool or max(2 * pages, 4), **kw)
+
+
+def oracle_pool(b, k_scale, v_scale):
+    """The oracle's quantised compact store after the step: store rows, then the new rows, through APPEND_FP8."""
+    U, Hkv, p, D = b.k_store.shape
+    k8 = np.full((U, Hkv, p, D), 0x7F, dtype=np.uint8)
+    v8 = np.full((U, Hkv, p, D), 0x7F, dtype=np.uint8)
+    ks, vs = k_scale[b.used_pages], v_scale[b.used_pages]  # scales of the compact store's pages
+    rows_k = b.k_store.transpose(0, 2, 1, 3).reshape(-1, Hkv, D)
+    rows_v = b.v_store.transpose(0, 2, 1, 3).reshape(-1, Hkv, D)
+    ofp8.kv_append_fp8(k8, v8, ks, vs, rows_k, rows_v, np.arange(U * p, dtype=np.int64))
+    ofp8.kv_append_fp8(k8, v8, ks, vs, b.k_new, b.v_new, b.compact_slot_mapping)
+    return k8, v8, ks, vs
+
+
+def run_case(b, parts_list=(0,), layout="HND", seed=1):
+    k_scale, v_scale = W.fp8_page_scales(seed, b.num_pages, b.num_kv_heads)
+    db = DeviceBatchFp8(b, k_scale, v_scale, layout=layout)
+    db.quantise_store()
+    db.append()
+    k8, v8, ks, vs = oracle_pool(b, k_scale, v_scale)
+    gk, gv = db.store_codes()
+    assert np.array_equal(gk, k8) and np.array_equal(gv, v8), "quantised codes differ from the oracle"
+    # pages no sequence uses keep their poison
+    unused = np.setdiff1d(np.arange(b.num_pages), b.used_pages)
+    if unused.size:
+        idx = torch.from_numpy(unused[:64]).to(db.k_pool.device)
+        assert bool((db.k_pool[idx] == 0x7F).all()) and bool((db.v_pool[idx] == 0x7F).all())
+    want, want_lse = ofp8.paged_decode_fp8(decode_q(b), k8, v8, ks, vs, b.compact_block_table, b.seq_lens, b.scale)
+    stats = {}
+    for parts in parts_list:
+        out, lse = db.decode(num_partitions=parts)
+        stats[parts] = check_parity(f64_of(out), want, "%s fp8 parts=%d" % (b.name, parts))
+        got_lse = f64_of(lse)
+        fin = np.isfinite(want_lse)
+        assert np.array_equal(np.isneginf(got_lse), np.isneginf(want_lse))
+        assert np.abs(got_lse[fin] - want_lse[fin]).max(initial=0.0) < 2e-3
+    out32, _ = db.decode(num_partitions=parts_list[0], out_dtype=torch.float32)
+    _, r = check_parity(f64_of(out32), want, "%s fp8 f32" % b.name)
+    assert r <= 6e-3
+    return stats
+
+
+@pytest.mark.parametrize("layout", ["HND", "NHD"])
+def test_append_fp8_bit_exact_with_skips_and_special_values(layout):
+    b = small_batch(31, [0, 1, 15, 16, 17, 100, 257], Hq=8, Hkv=2, p=16)
+    # special inputs in the new rows: huge, tiny, zero, negative zero, NaN, inf
+    b.k_new[0, 0, :6] = W.bf16_bits_from_f32(np.array([1e30, -1e30, 1e-30, 0.0, -0.0, np.inf], dtype=np.float32))
+    b.v_new[0, 0, 0] = W.BF16_NAN
+    b.slot_mapping[2] = -1
+    b.compact_slot_mapping[2] = -1
+    k_scale, v_scale = W.fp8_page_scales(2, b.num_pages, b.num_kv_heads)
+    db = DeviceBatchFp8(b, k_scale, v_scale, layout=layout)
+    db.quantise_store()
+    db.append()
+    k8, v8, _, _ = oracle_pool(b, k_scale, v_scale)
+    gk, gv = db.store_codes()
+    assert np.array_equal(gk, k8) and np.array_equal(gv, v8)
+
+
+@pytest.mark.parametrize("p", [16, 32])
+@pytest.mark.parametrize("G", [1, 4, 7, 8, 16])
+def test_decode_fp8_edge_lengths(p, G):
+    lens = [0, 1, p - 1, p, p + 1, 2 * p - 1, 63, 64, 65, 127, 128, 129, 191, 257, 300]
+    b = small_batch(300 + G, lens, Hq=G * 2, Hkv=2, p=p, table_width=40)
+    run_case(b, parts_list=(0, 1, 3, 9))
+
+
+def test_decode_fp8_many_sequences_nhd_and_long_stream():
+    rng = np.random.default_rng(17)
+    lens = rng.integers(1, 500, 149).tolist()
+    lens[70] = 5000
+    b = small_batch(310, lens, Hq=8, Hkv=4, p=16)
+    run_case(b, parts_list=(0, 4), layout="NHD")
+
+
+def test_decode_fp8_len1_is_the_dequantised_v_row():
+    b = small_batch(320, [1, 1, 1], Hq=8, Hkv=2, p=16)
+    k_scale, v_scale = W.fp8_page_scales(3, b.num_pages, b.num_kv_heads)
+    db = DeviceBatchFp8(b, k_scale, v_scale)
+    db.append()
+    out32, _ = db.decode(num_partitions=1, out_dtype=torch.float32)
+    k8, v8, ks, vs = oracle_pool(b, k_scale, v_scale)
+    t = ofp8.e4m3_decode_table()
+    got = f64_of(out32)
+    for s in range(3):
+        pg = int(b.compact_block_table[s, 0])
+        for h in range(8):
+            g = h // 4
+            # p = 1, l = 1: out = bf16(v_scale) ... the kernel folds v_scale into P (rounded to bf16), so the row is the
+            # code values times bf16(v_scale)
+            vs_b = float(torch.tensor(float(vs[pg, g])).to(torch.bfloat16).to(torch.float64))
+            assert np.array_equal(got[s, h], (t[v8[pg, g, 0]] * vs_b).astype(np.float32).astype(np.float64))
+
+
+def test_decode_fp8_config2_bagel_cfg_pairs():
+    b = W.config2_bagel_cfg_decode()
+    stats = run_case(b, parts_list=(0,))
+    print("config 2 fp8", stats)
+
+
+def test_fp8_error_codes():
+    b = small_batch(330, [5], Hq=8, Hkv=2, p=16)
+    dev = "cuda"
+    k = torch.zeros((4, 2, 16, 64), dtype=torch.uint8, device=dev)
+    sc = torch.ones((4, 2), dtype=torch.float32, device=dev)
+    pool64 = mstar.KVPoolFp8(k, k.clone(), sc, sc)
+    q = torch.zeros((1, 8, 64), dtype=torch.bfloat16, device=dev)
+    out = torch.zeros_like(q)
+    bt = torch.zeros((1, 1), dtype=torch.int32, device=dev)
+    sl = torch.ones(1, dtype=torch.int32, device=dev)
+    with pytest.raises(mstar.MstarError, match="UNSUPPORTED"):
+        mstar.paged_attn_decode_fp8(out, q, pool64, bt, sl, 1, 0.125, num_partitions=1)

@@ -24,5 +24,6 @@ from .generators import (  # noqa: F401
     config4_talker,
     config5_long_context,
     flow_step_bagel,
+    fp8_page_scales,
     CONFIG_SEED_BASE,
 )

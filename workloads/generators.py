@@ -310,3 +310,13 @@ def flow_step_bagel(num_requests: int = 4, n_latent: int = 4096, n_labels: int =
         share = [-1] * len(lens)
     return make_batch(rng, "flow_step_bagel", lens, [n_latent] * len(lens), 28, 4, 128, 16,
                       2 * _pages(lens, 16), share_with=share, shared_tokens=64 if n_labels >= 3 else 0)
+
+
+def fp8_page_scales(seed: int, num_pages: int, num_kv_heads: int, lo: float = 0.006, hi: float = 0.02):
+    """Caller-owned scales of a quantised pool: fp32 [num_pages, Hkv] for K and for V, uniform
+    in [lo, hi).  With N(0,1) rows the quotient x / scale spans subnormal codes, the normal range and, at the low
+    end of the interval (448 * 0.006 = 2.7 sigma), saturation.  Inputs only: no arithmetic of the method."""
+    rng = np.random.default_rng(seed)
+    k = rng.uniform(lo, hi, (num_pages, num_kv_heads)).astype(np.float32)
+    v = rng.uniform(lo, hi, (num_pages, num_kv_heads)).astype(np.float32)
+    return k, v
