@@ -229,7 +229,7 @@ def run_reference(args):
 
 # ----------------------------------------------------------------------------- the CUDA arm
 
-def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15):
+def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15, b_long=None):
     """configs[1] (BAGEL-like CFG-pair decode) and configs[3] (thinker + talker decode): median call time with a
     cold L2, GB/s on logical and on unique K/V bytes (shared prefix pages counted once), sequences per second."""
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -351,6 +351,36 @@ def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15
         "copy_pages_us": ms_c * 1e3, "copy_pages": int(len(bt.used_pages)),
         "copy_GBps_read_plus_write": cb / (ms_c * 1e-3) / 1e9,
         "frac_of_measured_copy_rate": cb / (ms_c * 1e-3) / 1e9 / hbm_peak}
+    del dt2, kg, vg
+    # the quantised pool.  Same batches, K/V as E4M3 codes with per-(page, head) scales written
+    # by mstar_kv_append_fp8; one mstar_paged_attn_decode_fp8 call.  Bytes = one byte per element (+ the scales).
+    from paper_2606_12688_b200.harness import DeviceBatchFp8
+
+    def fp8_entry(b, parts_arg, seed):
+        ks, vs = W.fp8_page_scales(seed, b.num_pages, b.num_kv_heads)
+        d = DeviceBatchFp8(b, ks, vs, device=dev)
+        d.quantise_store()
+        d.append()
+        S, Hq, Dh = b.num_seqs, b.num_q_heads, b.head_dim
+        parts = parts_arg if parts_arg > 0 else mstar.decode_auto_partitions(S, b.num_kv_heads, b.max_seq_len)
+        out = torch.empty((S, Hq, Dh), dtype=torch.bfloat16, device=dev)
+        ws = torch.empty(mstar.decode_workspace_bytes(S, Hq, Dh, parts), dtype=torch.uint8, device=dev)
+        call = lambda: mstar.paged_attn_decode_fp8(out, d.q_decode, d.pool, d.block_table, d.seq_lens, b.max_seq_len,
+                                                   float(b.scale), num_partitions=parts_arg, workspace=ws)
+        ms = median_ms([call])
+        uq = b.kv_bytes_unique() // 2
+        n_pages = int(sum((int(L) + b.page_size - 1) // b.page_size for L in b.seq_lens))
+        byt = uq + n_pages * b.num_kv_heads * 8
+        return {"seqs": S, "partitions": parts, "us": ms * 1e3, "kv_bytes_unique_fp8": uq,
+                "bytes_with_scales": byt, "GBps": byt / (ms * 1e-3) / 1e9,
+                "frac_of_measured_hbm": byt / (ms * 1e-3) / 1e9 / hbm_peak,
+                "bf16_equivalent_GBps": b.kv_bytes_unique() / (ms * 1e-3) / 1e9,
+                "decode_tokens_per_s": S / (ms * 1e-3)}
+
+    res["fp8 pool (SURVEY 8(f) rank 4): configs[1] decode"] = fp8_entry(b2, 0, 81)
+    res["fp8 pool (SURVEY 8(f) rank 4): configs[3] thinker decode"] = fp8_entry(bt, 0, 82)
+    if b_long is not None:
+        res["fp8 pool (SURVEY 8(f) rank 4): configs[4] long-context decode, 16 partitions"] = fp8_entry(b_long, 16, 83)
     return res
 
 
@@ -480,7 +510,7 @@ def run_ours(args):
     # headline, outside the K timed steps; cold L2 (flush before every call), CUDA events, median of 15
     other = None
     if rank == 0 and not args.no_other:
-        other = other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak=peaks["hbm_gbs"])
+        other = other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak=peaks["hbm_gbs"], b_long=bd)
 
     if rank != 0:
         if dist is not None:

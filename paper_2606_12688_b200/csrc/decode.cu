@@ -19,9 +19,11 @@
 
 namespace mstar {
 
-constexpr int kDecodeConsumerWarps = 4;
-constexpr int kDecodeTok = 16 * kDecodeConsumerWarps;  // tokens per ring stage
-constexpr int kDecodeThreads = 32 * (kDecodeConsumerWarps + 2);  // 4 consumer warps, K producer, V producer
+// Consumer warps (16 tokens of every ring stage each): 4 for a bf16 pool; 8 for an fp8 pool, where the byte -> bf16
+// conversion is ALU work that two warps per scheduler overlap and a 128-token stage has the bytes of a bf16 one.
+constexpr int decode_consumer_warps(bool fp8) { return fp8 ? 8 : 4; }
+constexpr int decode_tok(bool fp8) { return 16 * decode_consumer_warps(fp8); }          // tokens per ring stage
+constexpr int decode_threads(bool fp8) { return 32 * (decode_consumer_warps(fp8) + 2); }  // + K and V producer
 constexpr int kMaxStages = 16;
 
 struct DecodeParams {
@@ -30,7 +32,7 @@ struct DecodeParams {
     int64_t bt_stride;
     const int32_t* seq_lens;
     int32_t S, Hq, Hkv, G;
-    int32_t chunk;   // tokens per partition, multiple of kDecodeTok
+    int32_t chunk;   // tokens per partition, multiple of the stage size (decode_tok)
     int32_t nparts;  // partition slots per (sequence, head) in the workspace
     float scale_log2;
     float* part_O;  // [S*Hq][nparts][D]
@@ -43,7 +45,7 @@ struct DecodeParams {
     int32_t nstages;
     // balanced mode (num_partitions = 0): the (sequence, kv head) streams are laid end to end in 64-token tiles and
     // every CTA takes an equal, contiguous range of them; a stream cut by CTA boundaries yields one partial per
-    // piece.  chunk == kDecodeTok then, per_min bounds the pieces of one stream by nparts, and piece_count
+    // piece.  chunk == decode_tok then, per_min bounds the pieces of one stream by nparts, and piece_count
     // [S*Hkv] tells the combine pass how many partials each stream has.
     int32_t balanced;
     int32_t per_min;
@@ -59,10 +61,11 @@ struct ItemInfo {
 
 template <int D, int GH, int EB>  // EB = bytes per pool element (2 = bf16, 1 = e4m3)
 struct DecodeSmem {
-    static constexpr int kStageBytes = 2 * kDecodeTok * D * EB;
-    static constexpr int kScaleBytes = EB == 1 ? kMaxStages * 2 * 4 * 4 : 0;  // [stage][K|V][page of the stage] fp32
+    static constexpr int kWarps = decode_consumer_warps(EB == 1);
+    static constexpr int kStageBytes = 2 * 16 * kWarps * D * EB;
+    static constexpr int kScaleBytes = EB == 1 ? kMaxStages * 2 * 8 * 4 : 0;  // [stage][K|V][page of the stage] fp32
     static constexpr int kQBytes = GH * D * 2;
-    static constexpr int kMergeBytes = kDecodeConsumerWarps * GH * (D + 2) * 4;
+    static constexpr int kMergeBytes = kWarps * GH * (D + 2) * 4;
     // fixed part after the ring: Q slots, merge buffer, barriers, item info
     static constexpr int kFixed = 2 * kQBytes + kMergeBytes + (2 * kMaxStages + 4) * 8 + 2 * 32 + kScaleBytes;
     static size_t bytes(int nstages, int S) {
@@ -82,23 +85,28 @@ __device__ __forceinline__ void store_out_vec(void* out, int out_f32, size_t idx
     }
 }
 
-// two E4M3 codes (bytes of w picked by the PRMT selector into the high byte of each 16-bit lane) -> two bf16,
-// exactly: sign to bit 15, the 7 exponent/mantissa bits to bits [10:4] (a bf16 with exponent bias 127 instead of
-// 7, subnormal codes land on bf16 subnormals), then one packed multiply by 2^120 fixes the bias.
+// Two E4M3 codes -> two bf16, exactly.  PRMT picks the two bytes of w into the low byte of each 16-bit lane and
+// replicates their sign bit over the high byte (selector nibbles 8..11); times 16 moves the 7 exponent / mantissa
+// bits to bits [10:4]; the mask keeps them and one copy of the sign (bit 15).  That is the bf16 of the code's value
+// with exponent bias 127 instead of 7 (subnormal codes land on bf16 subnormals); one packed multiply by 2^120 fixes
+// the bias.  Two ALU-pipe and two FMA-pipe instructions per pair.
 template <uint32_t SEL>
 __device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t w) {
-    const uint32_t y = __byte_perm(w, 0u, SEL);
-    uint32_t x = (y & 0x80008000u) | ((y >> 4) & 0x07f007f0u);
+    uint32_t y;  // prmt in its default mode: selector nibbles 8..15 replicate the sign of byte (nibble & 7)
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(y) : "r"(w), "r"(0u), "n"(SEL));
+    uint32_t x = (y * 16u) & 0x87f087f0u;
     asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(x) : "r"(x), "r"(0x7B807B80u));
     return x;
 }
+constexpr uint32_t kSelK01 = 0x9180, kSelK23 = 0xB3A2;  // bytes (0, 1) | (2, 3) of a word: 4 consecutive d of a token
+constexpr uint32_t kSelV02 = 0xA280, kSelV13 = 0xB391;  // bytes (0, 2) | (1, 3): one d of two consecutive tokens
 
 template <int D, int PAGE, int GH, bool FP8>
-__global__ void __launch_bounds__(kDecodeThreads, 1)
+__global__ void __launch_bounds__(decode_threads(FP8), 1)
 decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_constant__ CUtensorMap vmap,
                      const DecodeParams p) {
-    constexpr int NW = kDecodeConsumerWarps;
-    constexpr int TOK = kDecodeTok;
+    constexpr int NW = decode_consumer_warps(FP8);
+    constexpr int TOK = decode_tok(FP8);
     constexpr int PPS = TOK / PAGE;  // pages per stage
     constexpr int EB = FP8 ? 1 : 2;    // bytes per pool element
     constexpr int NH = D * EB / 128;   // 128-byte column slices per row (bf16: 64-column halves)
@@ -216,7 +224,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 if (FP8 && pg >= 0) pg_scale = __ldg((op_isv ? p.v_scale : p.k_scale) + (size_t)pg * p.Hkv + kvh);
                 mbar_wait(empty_bar(st), ph ^ 1);
                 if (FP8) {
-                    if (pg >= 0) sc_ring[(st * 2 + op_isv) * 4 + op_page] = pg_scale;
+                    if (pg >= 0) sc_ring[(st * 2 + op_isv) * 8 + op_page] = pg_scale;
                     __syncwarp();  // the scales are ordered before lane 0's (releasing) arrive
                 }
                 if (lane == 0) mbar_arrive_expect_tx(full_bar(st), (uint32_t)(npg * PAGE * D * EB));
@@ -360,15 +368,15 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                             ldsm_x4(kb + swz128(f_row, 2 * c2 + f_csel), r0, r1, r2, r3);
                             const int ka = 2 * c2, kc = 2 * c2 + 1;
                             mma_bf16_16816(sc[0], qa[ka][0], qa[ka][1], qa[ka][2], qa[ka][3],
-                                           e4m3x2_to_bf16x2<0x1404>(r0), e4m3x2_to_bf16x2<0x3424>(r0));
+                                           e4m3x2_to_bf16x2<kSelK01>(r0), e4m3x2_to_bf16x2<kSelK23>(r0));
                             mma_bf16_16816(sc[1], qa[ka][0], qa[ka][1], qa[ka][2], qa[ka][3],
-                                           e4m3x2_to_bf16x2<0x1404>(r1), e4m3x2_to_bf16x2<0x3424>(r1));
+                                           e4m3x2_to_bf16x2<kSelK01>(r1), e4m3x2_to_bf16x2<kSelK23>(r1));
                             mma_bf16_16816(sc[0], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
-                                           e4m3x2_to_bf16x2<0x1404>(r2), e4m3x2_to_bf16x2<0x3424>(r2));
+                                           e4m3x2_to_bf16x2<kSelK01>(r2), e4m3x2_to_bf16x2<kSelK23>(r2));
                             mma_bf16_16816(sc[1], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
-                                           e4m3x2_to_bf16x2<0x1404>(r3), e4m3x2_to_bf16x2<0x3424>(r3));
+                                           e4m3x2_to_bf16x2<kSelK01>(r3), e4m3x2_to_bf16x2<kSelK23>(r3));
                         }
-                        const float ksc = sc_ring[(st * 2 + 0) * 4 + (w * 16) / PAGE];  // this warp's page
+                        const float ksc = sc_ring[(st * 2 + 0) * 8 + (w * 16) / PAGE];  // this warp's page
 #pragma unroll
                         for (int b = 0; b < 2; ++b) {
                             sc[b][0] *= ksc; sc[b][1] *= ksc; sc[b][2] *= ksc; sc[b][3] *= ksc;
@@ -409,7 +417,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     const float p11 = fast_exp2(sc[1][1] * p.scale_log2 - ms0);
                     l0 = l0 * a0 + (p00 + p01) + (p10 + p11);
                     // FP8: the page's V scale goes into P (the row sum l keeps the unscaled probabilities)
-                    const float vsc = FP8 ? sc_ring[(st * 2 + 1) * 4 + (w * 16) / PAGE] : 1.f;
+                    const float vsc = FP8 ? sc_ring[(st * 2 + 1) * 8 + (w * 16) / PAGE] : 1.f;
                     uint32_t pa[4];
                     pa[0] = pack_bf16x2(p00 * vsc, p01 * vsc);
                     pa[2] = pack_bf16x2(p10 * vsc, p11 * vsc);
@@ -433,6 +441,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                         pa[3] = pack_bf16x2(q10 * vsc, q11 * vsc);
                     }
                     // ---- O = O * alpha + P V
+                    // FP8 (issue-bound): skip the multiplies of a stage in which no row's running max moved
+                    const bool rescale = !FP8 || __any_sync(0xffffffffu, a0 != 1.f || a1 != 1.f);
                     uint32_t fr[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
                     for (int jj = 0; jj < D / 16; ++jj) {
@@ -442,10 +452,10 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                             // a 16-wide d block; n-block 2jj takes the even d (n = g <-> d = 2g), 2jj+1 the odd d
                             if ((jj & 1) == 0) ldsm_x4_trans(vb + swz128(f_row, jj + f_csel), fr[0], fr[1], fr[2], fr[3]);
                             const uint32_t lo = fr[(jj & 1) * 2], hi = fr[(jj & 1) * 2 + 1];
-                            b0 = e4m3x2_to_bf16x2<0x2404>(lo);
-                            b1 = e4m3x2_to_bf16x2<0x2404>(hi);
-                            b2 = e4m3x2_to_bf16x2<0x3414>(lo);
-                            b3 = e4m3x2_to_bf16x2<0x3414>(hi);
+                            b0 = e4m3x2_to_bf16x2<kSelV02>(lo);
+                            b1 = e4m3x2_to_bf16x2<kSelV02>(hi);
+                            b2 = e4m3x2_to_bf16x2<kSelV13>(lo);
+                            b3 = e4m3x2_to_bf16x2<kSelV13>(hi);
                         } else {
                             const uint32_t chunk = 2 * jj + v_csel;
                             ldsm_x4_trans(vb + (chunk >> 3) * HT + swz128(v_row, chunk & 7), b0, b1, b2, b3);
@@ -453,9 +463,11 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                         if (nv < 16) {  // 0 * NaN guard: zero V rows that hold no token
                             b0 &= vmask_lo; b1 &= vmask_hi; b2 &= vmask_lo; b3 &= vmask_hi;
                         }
-                        o[2 * jj][0] *= a0; o[2 * jj][1] *= a0; o[2 * jj + 1][0] *= a0; o[2 * jj + 1][1] *= a0;
-                        if (GH == 16) {
-                            o[2 * jj][2] *= a1; o[2 * jj][3] *= a1; o[2 * jj + 1][2] *= a1; o[2 * jj + 1][3] *= a1;
+                        if (rescale) {
+                            o[2 * jj][0] *= a0; o[2 * jj][1] *= a0; o[2 * jj + 1][0] *= a0; o[2 * jj + 1][1] *= a0;
+                            if (GH == 16) {
+                                o[2 * jj][2] *= a1; o[2 * jj][3] *= a1; o[2 * jj + 1][2] *= a1; o[2 * jj + 1][3] *= a1;
+                            }
                         }
                         mma_bf16_16816(o[2 * jj], pa[0], pa[1], pa[2], pa[3], b0, b1);
                         mma_bf16_16816(o[2 * jj + 1], pa[0], pa[1], pa[2], pa[3], b2, b3);
@@ -602,22 +614,22 @@ __global__ void __launch_bounds__(128) decode_combine_kernel(const float* __rest
 // ---------------------------------------------------------------------------------------------
 static int32_t round_up(int32_t x, int32_t m) { return (x + m - 1) / m * m; }
 
-static int32_t auto_chunk(int32_t S, int32_t Hkv, int32_t max_seq_len) {
+static int32_t auto_chunk(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t tok) {
     // ~8 work items per SM at the length upper bound, 128..512-token partitions, at most 128 partitions
     const int64_t upper = (int64_t)S * Hkv * (max_seq_len > 0 ? max_seq_len : 1);
     int64_t c = upper / ((int64_t)device_sm_count() * 8);
     if (c < 128) c = 128;
     if (c > 512) c = 512;
-    int32_t chunk = round_up((int32_t)c, kDecodeTok);
-    if ((max_seq_len + chunk - 1) / chunk > 128) chunk = round_up((max_seq_len + 127) / 128, kDecodeTok);
+    int32_t chunk = round_up((int32_t)c, tok);
+    if ((max_seq_len + chunk - 1) / chunk > 128) chunk = round_up((max_seq_len + 127) / 128, tok);
     return chunk;
 }
 
 // num_partitions = 0: balanced mode when a sequence can span at least two tiles.  Slots per row = pieces a stream
 // can be cut into: a CTA range is at least per_min = ceil(max_tiles / (slots - 1)) tiles long, so a stream of
 // max_tiles tiles meets at most slots CTA ranges.
-static bool balanced_plan(int32_t max_seq_len, int32_t* nparts, int32_t* per_min) {
-    const int32_t max_tiles = (max_seq_len + kDecodeTok - 1) / kDecodeTok;
+static bool balanced_plan(int32_t max_seq_len, int32_t tok, int32_t* nparts, int32_t* per_min) {
+    const int32_t max_tiles = (max_seq_len + tok - 1) / tok;
     if (max_tiles < 2) return false;
     int32_t slots = (max_tiles + 1) / 2 + 1;
     if (slots > 33) slots = 33;
@@ -626,18 +638,18 @@ static bool balanced_plan(int32_t max_seq_len, int32_t* nparts, int32_t* per_min
     return true;
 }
 
-static void partition_plan(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t num_partitions, int32_t* chunk,
-                           int32_t* nparts) {
+static void partition_plan(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t num_partitions, int32_t tok,
+                           int32_t* chunk, int32_t* nparts) {
     const int32_t msl = max_seq_len > 0 ? max_seq_len : 1;
     if (num_partitions <= 0) {
         int32_t per_min;
-        if (balanced_plan(msl, nparts, &per_min)) {
-            *chunk = kDecodeTok;
+        if (balanced_plan(msl, tok, nparts, &per_min)) {
+            *chunk = tok;
             return;
         }
-        *chunk = auto_chunk(S, Hkv, msl);
+        *chunk = auto_chunk(S, Hkv, msl, tok);
     } else {
-        *chunk = round_up((msl + num_partitions - 1) / num_partitions, kDecodeTok);
+        *chunk = round_up((msl + num_partitions - 1) / num_partitions, tok);
     }
     *nparts = (msl + *chunk - 1) / *chunk;
     if (num_partitions > 0 && *nparts > num_partitions) *nparts = num_partitions;
@@ -661,7 +673,7 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
     int grid = device_sm_count();
     if (grid > max_items) grid = max_items;
     if (grid < 1) grid = 1;
-    kern<<<grid, kDecodeThreads, smem, stream>>>(maps.k, maps.v, p);
+    kern<<<grid, decode_threads(FP8), smem, stream>>>(maps.k, maps.v, p);
     MSTAR_CUDA_OK(cudaGetLastError());
     launch_count_add(1);
     return MSTAR_OK;
@@ -672,7 +684,7 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
 extern "C" int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv_heads,
                                                            int32_t max_seq_len) {
     int32_t chunk, nparts;
-    mstar::partition_plan(num_seqs, num_kv_heads, max_seq_len, 0, &chunk, &nparts);
+    mstar::partition_plan(num_seqs, num_kv_heads, max_seq_len, 0, mstar::decode_tok(false), &chunk, &nparts);
     return nparts;
 }
 
@@ -709,8 +721,10 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
     const int D = pool->head_dim, PAGE = pool->page_size;
 
     DecodeParams p{};
-    partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, &p.chunk, &p.nparts);
-    if (num_partitions == 0) p.balanced = balanced_plan(max_seq_len > 0 ? max_seq_len : 1, &p.nparts, &p.per_min) ? 1 : 0;
+    const int32_t tok = decode_tok(fp8);
+    partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, tok, &p.chunk, &p.nparts);
+    if (num_partitions == 0)
+        p.balanced = balanced_plan(max_seq_len > 0 ? max_seq_len : 1, tok, &p.nparts, &p.per_min) ? 1 : 0;
     p.direct = (p.nparts == 1);
     if (!p.direct) {
         const size_t need = mstar_paged_attn_decode_workspace_bytes(num_seqs, num_q_heads, D, p.nparts);
