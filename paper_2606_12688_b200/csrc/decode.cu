@@ -85,6 +85,13 @@ __device__ __forceinline__ void store_out_vec(void* out, int out_f32, size_t idx
     }
 }
 
+// MSTAR_FP8_BIAS_IN_SCALES = 1: the packed multiply is dropped; the MMAs run on code values times 2^-120 (subnormal
+// codes are bf16 subnormals, which the tensor core takes exactly) and the factor is returned in two halves that keep
+// every accumulator in the normal fp32 range: Q and P carry 2^60, the logits and O get the other 2^60 in fp32.
+#ifndef MSTAR_FP8_BIAS_IN_SCALES
+#define MSTAR_FP8_BIAS_IN_SCALES 1
+#endif
+constexpr float kTwo60 = 1152921504606846976.f;  // 2^60
 // Two E4M3 codes -> two bf16, exactly.  PRMT picks the two bytes of w into the low byte of each 16-bit lane and
 // replicates their sign bit over the high byte (selector nibbles 8..11); times 16 moves the 7 exponent / mantissa
 // bits to bits [10:4]; the mask keeps them and one copy of the sign (bit 15).  That is the bf16 of the code's value
@@ -95,7 +102,9 @@ __device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t w) {
     uint32_t y;  // prmt in its default mode: selector nibbles 8..15 replicate the sign of byte (nibble & 7)
     asm("prmt.b32 %0, %1, %2, %3;" : "=r"(y) : "r"(w), "r"(0u), "n"(SEL));
     uint32_t x = (y * 16u) & 0x87f087f0u;
+#if !MSTAR_FP8_BIAS_IN_SCALES
     asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(x) : "r"(x), "r"(0x7B807B80u));
+#endif
     return x;
 }
 constexpr uint32_t kSelK01 = 0x9180, kSelK23 = 0xB3A2;  // bytes (0, 1) | (2, 3) of a word: 4 consecutive d of a token
@@ -340,6 +349,13 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     }
                 }
             }
+            if (FP8 && MSTAR_FP8_BIAS_IN_SCALES) {  // Q * 2^60 (exact; |q| < 2^67)
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks)
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(qa[ks][i]) : "r"(qa[ks][i]), "r"(0x5D805D80u));
+            }
             __syncwarp();
             if (lane == 0) mbar_arrive(qempty_bar(qs));
             qs ^= 1;
@@ -376,7 +392,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                             mma_bf16_16816(sc[1], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
                                            e4m3x2_to_bf16x2<kSelK01>(r3), e4m3x2_to_bf16x2<kSelK23>(r3));
                         }
-                        const float ksc = sc_ring[(st * 2 + 0) * 8 + (w * 16) / PAGE];  // this warp's page
+                        float ksc = sc_ring[(st * 2 + 0) * 8 + (w * 16) / PAGE];  // this warp's page
+                        if (MSTAR_FP8_BIAS_IN_SCALES) ksc *= kTwo60;
 #pragma unroll
                         for (int b = 0; b < 2; ++b) {
                             sc[b][0] *= ksc; sc[b][1] *= ksc; sc[b][2] *= ksc; sc[b][3] *= ksc;
@@ -417,7 +434,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     const float p11 = fast_exp2(sc[1][1] * p.scale_log2 - ms0);
                     l0 = l0 * a0 + (p00 + p01) + (p10 + p11);
                     // FP8: the page's V scale goes into P (the row sum l keeps the unscaled probabilities)
-                    const float vsc = FP8 ? sc_ring[(st * 2 + 1) * 8 + (w * 16) / PAGE] : 1.f;
+                    const float vsc = FP8 ? sc_ring[(st * 2 + 1) * 8 + (w * 16) / PAGE] *
+                                                (MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f) : 1.f;
                     uint32_t pa[4];
                     pa[0] = pack_bf16x2(p00 * vsc, p01 * vsc);
                     pa[2] = pack_bf16x2(p10 * vsc, p11 * vsc);
@@ -491,11 +509,12 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 for (int j = 0; j < D / 8; ++j) {
                     if constexpr (FP8) {  // n-blocks 2c | 2c+1 hold the even | odd d of block c: d = 16c + 4t4 + 0..3
                         if (j & 1) continue;
+                        const float f = MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f;
                         *reinterpret_cast<float4*>(mo + g * D + j * 8 + 4 * t4) =
-                            make_float4(o[j][0], o[j + 1][0], o[j][1], o[j + 1][1]);
+                            make_float4(o[j][0] * f, o[j + 1][0] * f, o[j][1] * f, o[j + 1][1] * f);
                         if (GH == 16)
                             *reinterpret_cast<float4*>(mo + (g + 8) * D + j * 8 + 4 * t4) =
-                                make_float4(o[j][2], o[j + 1][2], o[j][3], o[j + 1][3]);
+                                make_float4(o[j][2] * f, o[j + 1][2] * f, o[j][3] * f, o[j + 1][3] * f);
                     } else {
                         *reinterpret_cast<float2*>(mo + g * D + j * 8 + 2 * t4) = make_float2(o[j][0], o[j][1]);
                         if (GH == 16)

@@ -113,6 +113,25 @@ def test_decode_fp8_len1_is_the_dequantised_v_row():
             assert np.array_equal(got[s, h], (t[v8[pg, g, 0]] * vs_b).astype(np.float32).astype(np.float64))
 
 
+def test_decode_fp8_subnormal_codes_are_exact():
+    """Scales so large that almost every code is an E4M3 subnormal (|x / scale| < 2^-6): the kernel's byte -> bf16
+    conversion maps them to bf16 subnormals, which must survive the tensor core (a flush would zero K and V)."""
+    b = small_batch(340, [1, 40, 130, 700], Hq=8, Hkv=2, p=16)
+    k_scale = np.full((b.num_pages, b.num_kv_heads), 96.0, dtype=np.float32)
+    v_scale = np.full((b.num_pages, b.num_kv_heads), 160.0, dtype=np.float32)
+    db = DeviceBatchFp8(b, k_scale, v_scale)
+    db.quantise_store()
+    db.append()
+    k8, v8, ks, vs = oracle_pool(b, k_scale, v_scale)
+    used = k8[b.compact_block_table[3, :40]]
+    assert ((used & 0x78) == 0).mean() > 0.7 and (used & 0x7F).max() > 0  # mostly subnormal codes, not all zero
+    want, _ = ofp8.paged_decode_fp8(decode_q(b), k8, v8, ks, vs, b.compact_block_table, b.seq_lens, b.scale)
+    assert np.abs(want).max() > 0.5
+    for parts in (0, 1, 4):
+        out, _ = db.decode(num_partitions=parts)
+        check_parity(f64_of(out), want, "subnormal codes parts=%d" % parts)
+
+
 def test_decode_fp8_config2_bagel_cfg_pairs():
     b = W.config2_bagel_cfg_decode()
     stats = run_case(b, parts_list=(0,))
