@@ -132,6 +132,56 @@ def test_decode_fp8_subnormal_codes_are_exact():
         check_parity(f64_of(out), want, "subnormal codes parts=%d" % parts)
 
 
+def test_fp8_deterministic_graph_capturable_and_page_permutation_invariant():
+    b = small_batch(350, [500, 123, 64, 1], Hq=14, Hkv=2, p=16, pool=80)
+    k_scale, v_scale = W.fp8_page_scales(5, b.num_pages, b.num_kv_heads)
+    db = DeviceBatchFp8(b, k_scale, v_scale)
+    db.quantise_store()
+    S, Hq, D = 4, 14, 128
+    out = torch.zeros((S, Hq, D), dtype=torch.bfloat16, device="cuda")
+    ws = torch.empty(mstar.decode_workspace_bytes(S, Hq, D, 4), dtype=torch.uint8, device="cuda")
+
+    def step(bt=None):
+        db.append()
+        mstar.paged_attn_decode_fp8(out, db.q_decode, db.pool, db.block_table if bt is None else bt, db.seq_lens,
+                                    500, float(b.scale), num_partitions=4, workspace=ws)
+
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    first = out.clone()
+    codes_first = db.store_codes()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        step()
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(first.view(torch.int16), out.view(torch.int16))
+    assert all(np.array_equal(a, c) for a, c in zip(codes_first, db.store_codes()))
+    # relabel the physical pages of sequence 0 (codes and scales move with them): bit-identical output
+    used = np.zeros(b.num_pages, dtype=bool)
+    used[b.used_pages] = True
+    free = np.flatnonzero(~used)
+    bt2 = db.block_table.clone()
+    npg = (500 + 15) // 16
+    for i in range(npg):
+        src, dst = int(bt2[0, i]), int(free[i])
+        db.k_pool[dst] = db.k_pool[src]
+        db.v_pool[dst] = db.v_pool[src]
+        db.k_scale[dst] = db.k_scale[src]
+        db.v_scale[dst] = db.v_scale[src]
+        bt2[0, i] = dst
+    out.zero_()
+    mstar.paged_attn_decode_fp8(out, db.q_decode, db.pool, bt2, db.seq_lens, 500, float(b.scale), num_partitions=4,
+                                workspace=ws)
+    torch.cuda.synchronize()
+    assert torch.equal(first.view(torch.int16), out.view(torch.int16))
+
+
 def test_decode_fp8_config2_bagel_cfg_pairs():
     b = W.config2_bagel_cfg_decode()
     stats = run_case(b, parts_list=(0,))
