@@ -110,6 +110,13 @@ __device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t w) {
 constexpr uint32_t kSelK01 = 0x9180, kSelK23 = 0xB3A2;  // bytes (0, 1) | (2, 3) of a word: 4 consecutive d of a token
 constexpr uint32_t kSelV02 = 0xA280, kSelV13 = 0xB391;  // bytes (0, 2) | (1, 3): one d of two consecutive tokens
 
+// transpose of an 8x8 b16 matrix held one row per lane group (lane (g, t4): row g, columns 2t4, 2t4+1)
+__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
+    uint32_t d;
+    asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
+    return d;
+}
+
 template <int D, int PAGE, int GH, bool FP8>
 __global__ void __launch_bounds__(decode_threads(FP8), 1)
 decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_constant__ CUtensorMap vmap,
@@ -328,206 +335,322 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
             mbar_wait(qfull_bar(qs), qph);
             const ItemInfo it = info[qs];
             if (it.ntok < 0) break;
-            // Q fragments (A operand), rows = grouped query heads
-            uint32_t qa[D / 16][4];
-            {
-                const uint16_t* qb = qbuf_g + qs * (SM::kQBytes / 2);
+            if constexpr (FP8 && GH == 8) {
+                // ---- fp8 pool, G <= 8: operands swapped, S^T = K Q^T and O^T = V^T P^T, so the 16 MMA rows are tokens
+                // (or d) and the 8 columns are the grouped heads: half the MMAs and accumulator registers of the
+                // heads-as-rows form, no zero padding of the A operand.  Lane (g, t4): S^T rows = tokens g, g+8,
+                // columns = heads 2t4, 2t4+1.
+                uint32_t qb2[D / 16][2];  // B operand: Q^T[k slots of the 16-wide d block ks][head g]
+                {
+                    const uint16_t* qb = qbuf_g + qs * (SM::kQBytes / 2);
 #pragma unroll
-                for (int ks = 0; ks < D / 16; ++ks) {
-                    // FP8: this lane's K bytes of a 16-wide d block are d = 4*t4 .. 4*t4+3 (one ldmatrix word), so
-                    // the contraction index is permuted: MMA k-slots (2t4, 2t4+1 | 2t4+8, 2t4+9) <-> d (4t4, 4t4+1 |
-                    // 4t4+2, 4t4+3); Q takes the same permutation
-                    const int c0 = FP8 ? 4 * t4 : 2 * t4, c1 = FP8 ? 4 * t4 + 2 : 8 + 2 * t4;
-                    qa[ks][0] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + c0);
-                    qa[ks][2] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + c1);
-                    if (GH == 16) {
-                        qa[ks][1] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + c0);
-                        qa[ks][3] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + c1);
-                    } else {
-                        qa[ks][1] = 0u;
-                        qa[ks][3] = 0u;
-                    }
-                }
-            }
-            if (FP8 && MSTAR_FP8_BIAS_IN_SCALES) {  // Q * 2^60 (exact; |q| < 2^67)
-#pragma unroll
-                for (int ks = 0; ks < D / 16; ++ks)
-#pragma unroll
-                    for (int i = 0; i < 4; ++i)
-                        asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(qa[ks][i]) : "r"(qa[ks][i]), "r"(0x5D805D80u));
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(qempty_bar(qs));
-            qs ^= 1;
-            if (qs == 0) qph ^= 1;
-
-            float o[D / 8][4];
-#pragma unroll
-            for (int j = 0; j < D / 8; ++j) o[j][0] = o[j][1] = o[j][2] = o[j][3] = 0.f;
-            float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;  // rows g and g+8 (raw q.k units)
-
-            const int ntiles = (it.ntok + TOK - 1) / TOK;
-            for (int t = 0; t < ntiles; ++t) {
-                mbar_wait(full_bar(st), ph);
-                const int nv = min(16, it.ntok - t * TOK - w * 16);  // valid tokens in this warp's slice
-                if (nv > 0) {
-                    const uint32_t kb = ring + st * SM::kStageBytes;
-                    const uint32_t vb = kb + KBYTES;
-                    // ---- S = Q K^T for 16 tokens (two n-blocks of 8)
-                    float sc[2][4];
-#pragma unroll
-                    for (int b = 0; b < 2; ++b) sc[b][0] = sc[b][1] = sc[b][2] = sc[b][3] = 0.f;
-                    if constexpr (FP8) {
-#pragma unroll
-                        for (int c2 = 0; c2 < D / 32; ++c2) {
-                            uint32_t r0, r1, r2, r3;
-                            ldsm_x4(kb + swz128(f_row, 2 * c2 + f_csel), r0, r1, r2, r3);
-                            const int ka = 2 * c2, kc = 2 * c2 + 1;
-                            mma_bf16_16816(sc[0], qa[ka][0], qa[ka][1], qa[ka][2], qa[ka][3],
-                                           e4m3x2_to_bf16x2<kSelK01>(r0), e4m3x2_to_bf16x2<kSelK23>(r0));
-                            mma_bf16_16816(sc[1], qa[ka][0], qa[ka][1], qa[ka][2], qa[ka][3],
-                                           e4m3x2_to_bf16x2<kSelK01>(r1), e4m3x2_to_bf16x2<kSelK23>(r1));
-                            mma_bf16_16816(sc[0], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
-                                           e4m3x2_to_bf16x2<kSelK01>(r2), e4m3x2_to_bf16x2<kSelK23>(r2));
-                            mma_bf16_16816(sc[1], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
-                                           e4m3x2_to_bf16x2<kSelK01>(r3), e4m3x2_to_bf16x2<kSelK23>(r3));
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        qb2[ks][0] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + 4 * t4);
+                        qb2[ks][1] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + 4 * t4 + 2);
+                        if (MSTAR_FP8_BIAS_IN_SCALES) {  // Q * 2^60 (exact; |q| < 2^67)
+                            asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(qb2[ks][0]) : "r"(qb2[ks][0]), "r"(0x5D805D80u));
+                            asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(qb2[ks][1]) : "r"(qb2[ks][1]), "r"(0x5D805D80u));
                         }
-                        float ksc = sc_ring[(st * 2 + 0) * 8 + (w * 16) / PAGE];  // this warp's page
-                        if (MSTAR_FP8_BIAS_IN_SCALES) ksc *= kTwo60;
-#pragma unroll
-                        for (int b = 0; b < 2; ++b) {
-                            sc[b][0] *= ksc; sc[b][1] *= ksc; sc[b][2] *= ksc; sc[b][3] *= ksc;
-                        }
-                    } else {
-#pragma unroll
-                        for (int ks = 0; ks < D / 16; ++ks) {
-                            const uint32_t chunk = 2 * ks + k_csel;
-                            uint32_t b0, b1, b2, b3;
-                            ldsm_x4(kb + (chunk >> 3) * HT + swz128(k_row, chunk & 7), b0, b1, b2, b3);
-                            mma_bf16_16816(sc[0], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b0, b1);
-                            mma_bf16_16816(sc[1], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b2, b3);
-                        }
-                    }
-                    // ---- mask the ragged tail (slots >= seq_len may hold anything, incl. NaN)
-                    uint32_t vmask_lo = 0xffffffffu, vmask_hi = 0xffffffffu;
-                    if (nv < 16) {
-#pragma unroll
-                        for (int b = 0; b < 2; ++b) {
-                            const int c = b * 8 + 2 * t4;
-                            if (c >= nv) sc[b][0] = sc[b][2] = -INFINITY;
-                            if (c + 1 >= nv) sc[b][1] = sc[b][3] = -INFINITY;
-                        }
-                        vmask_lo = (2 * t4 < nv ? 0x0000ffffu : 0u) | (2 * t4 + 1 < nv ? 0xffff0000u : 0u);
-                        vmask_hi = (8 + 2 * t4 < nv ? 0x0000ffffu : 0u) | (8 + 2 * t4 + 1 < nv ? 0xffff0000u : 0u);
-                    }
-                    // ---- online softmax (fp32), row max over the quad by shuffles
-                    float mx0 = fmaxf(fmaxf(sc[0][0], sc[0][1]), fmaxf(sc[1][0], sc[1][1]));
-                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
-                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
-                    const float mn0 = fmaxf(m0, mx0);
-                    const float a0 = fast_exp2((m0 - mn0) * p.scale_log2);
-                    const float ms0 = mn0 * p.scale_log2;
-                    m0 = mn0;
-                    const float p00 = fast_exp2(sc[0][0] * p.scale_log2 - ms0);
-                    const float p01 = fast_exp2(sc[0][1] * p.scale_log2 - ms0);
-                    const float p10 = fast_exp2(sc[1][0] * p.scale_log2 - ms0);
-                    const float p11 = fast_exp2(sc[1][1] * p.scale_log2 - ms0);
-                    l0 = l0 * a0 + (p00 + p01) + (p10 + p11);
-                    // FP8: the page's V scale goes into P (the row sum l keeps the unscaled probabilities)
-                    const float vsc = FP8 ? sc_ring[(st * 2 + 1) * 8 + (w * 16) / PAGE] *
-                                                (MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f) : 1.f;
-                    uint32_t pa[4];
-                    pa[0] = pack_bf16x2(p00 * vsc, p01 * vsc);
-                    pa[2] = pack_bf16x2(p10 * vsc, p11 * vsc);
-                    pa[1] = 0u;
-                    pa[3] = 0u;
-                    float a1 = 1.f;
-                    if (GH == 16) {
-                        float mx1 = fmaxf(fmaxf(sc[0][2], sc[0][3]), fmaxf(sc[1][2], sc[1][3]));
-                        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
-                        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
-                        const float mn1 = fmaxf(m1, mx1);
-                        a1 = fast_exp2((m1 - mn1) * p.scale_log2);
-                        const float ms1 = mn1 * p.scale_log2;
-                        m1 = mn1;
-                        const float q00 = fast_exp2(sc[0][2] * p.scale_log2 - ms1);
-                        const float q01 = fast_exp2(sc[0][3] * p.scale_log2 - ms1);
-                        const float q10 = fast_exp2(sc[1][2] * p.scale_log2 - ms1);
-                        const float q11 = fast_exp2(sc[1][3] * p.scale_log2 - ms1);
-                        l1 = l1 * a1 + (q00 + q01) + (q10 + q11);
-                        pa[1] = pack_bf16x2(q00 * vsc, q01 * vsc);
-                        pa[3] = pack_bf16x2(q10 * vsc, q11 * vsc);
-                    }
-                    // ---- O = O * alpha + P V
-                    // FP8 (issue-bound): skip the multiplies of a stage in which no row's running max moved
-                    const bool rescale = !FP8 || __any_sync(0xffffffffu, a0 != 1.f || a1 != 1.f);
-                    uint32_t fr[4] = {0u, 0u, 0u, 0u};
-#pragma unroll
-                    for (int jj = 0; jj < D / 16; ++jj) {
-                        uint32_t b0, b1, b2, b3;
-                        if constexpr (FP8) {
-                            // transposed 8x8 b16 matrices = byte pairs: this lane gets V[2t4 | 2t4+1][2g | 2g+1] of
-                            // a 16-wide d block; n-block 2jj takes the even d (n = g <-> d = 2g), 2jj+1 the odd d
-                            if ((jj & 1) == 0) ldsm_x4_trans(vb + swz128(f_row, jj + f_csel), fr[0], fr[1], fr[2], fr[3]);
-                            const uint32_t lo = fr[(jj & 1) * 2], hi = fr[(jj & 1) * 2 + 1];
-                            b0 = e4m3x2_to_bf16x2<kSelV02>(lo);
-                            b1 = e4m3x2_to_bf16x2<kSelV02>(hi);
-                            b2 = e4m3x2_to_bf16x2<kSelV13>(lo);
-                            b3 = e4m3x2_to_bf16x2<kSelV13>(hi);
-                        } else {
-                            const uint32_t chunk = 2 * jj + v_csel;
-                            ldsm_x4_trans(vb + (chunk >> 3) * HT + swz128(v_row, chunk & 7), b0, b1, b2, b3);
-                        }
-                        if (nv < 16) {  // 0 * NaN guard: zero V rows that hold no token
-                            b0 &= vmask_lo; b1 &= vmask_hi; b2 &= vmask_lo; b3 &= vmask_hi;
-                        }
-                        if (rescale) {
-                            o[2 * jj][0] *= a0; o[2 * jj][1] *= a0; o[2 * jj + 1][0] *= a0; o[2 * jj + 1][1] *= a0;
-                            if (GH == 16) {
-                                o[2 * jj][2] *= a1; o[2 * jj][3] *= a1; o[2 * jj + 1][2] *= a1; o[2 * jj + 1][3] *= a1;
-                            }
-                        }
-                        mma_bf16_16816(o[2 * jj], pa[0], pa[1], pa[2], pa[3], b0, b1);
-                        mma_bf16_16816(o[2 * jj + 1], pa[0], pa[1], pa[2], pa[3], b2, b3);
                     }
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(empty_bar(st));
-                if (++st == nstages) { st = 0; ph ^= 1; }
-            }
+                if (lane == 0) mbar_arrive(qempty_bar(qs));
+                qs ^= 1;
+                if (qs == 0) qph ^= 1;
 
-            // ---- merge the four warps' (m, l, O) through shared memory
-            l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
-            l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
-            if (GH == 16) {
-                l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
-                l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
-            }
-            {
-                float* mo = merge_O + (size_t)w * GH * D;
+                float ot[D / 16][4];  // O^T: rows d = 16c + 2g (regs 0, 1) and 16c + 2g + 1 (regs 2, 3), columns = heads
 #pragma unroll
-                for (int j = 0; j < D / 8; ++j) {
-                    if constexpr (FP8) {  // n-blocks 2c | 2c+1 hold the even | odd d of block c: d = 16c + 4t4 + 0..3
-                        if (j & 1) continue;
-                        const float f = MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f;
-                        *reinterpret_cast<float4*>(mo + g * D + j * 8 + 4 * t4) =
-                            make_float4(o[j][0] * f, o[j + 1][0] * f, o[j][1] * f, o[j + 1][1] * f);
-                        if (GH == 16)
-                            *reinterpret_cast<float4*>(mo + (g + 8) * D + j * 8 + 4 * t4) =
-                                make_float4(o[j][2] * f, o[j + 1][2] * f, o[j][3] * f, o[j + 1][3] * f);
-                    } else {
-                        *reinterpret_cast<float2*>(mo + g * D + j * 8 + 2 * t4) = make_float2(o[j][0], o[j][1]);
-                        if (GH == 16)
-                            *reinterpret_cast<float2*>(mo + (g + 8) * D + j * 8 + 2 * t4) =
-                                make_float2(o[j][2], o[j][3]);
+                for (int c = 0; c < D / 16; ++c) ot[c][0] = ot[c][1] = ot[c][2] = ot[c][3] = 0.f;
+                float mh0 = -INFINITY, mh1 = -INFINITY, lh0 = 0.f, lh1 = 0.f;  // heads 2t4, 2t4+1
+                const int ntiles = (it.ntok + TOK - 1) / TOK;
+                for (int t = 0; t < ntiles; ++t) {
+                    mbar_wait(full_bar(st), ph);
+                    const int nv = min(16, it.ntok - t * TOK - w * 16);  // valid tokens in this warp's slice
+                    if (nv > 0) {
+                        const uint32_t kb = ring + st * SM::kStageBytes;
+                        const uint32_t vb = kb + KBYTES;
+                        float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};  // two MMA chains
+#pragma unroll
+                        for (int c2 = 0; c2 < D / 32; ++c2) {
+                            uint32_t r0, r1, r2, r3;  // (tokens 0-7 | 8-15) x (chunk 2c2 | 2c2+1)
+                            ldsm_x4(kb + swz128(f_row, 2 * c2 + f_csel), r0, r1, r2, r3);
+                            mma_bf16_16816(sa, e4m3x2_to_bf16x2<kSelK01>(r0), e4m3x2_to_bf16x2<kSelK01>(r1),
+                                           e4m3x2_to_bf16x2<kSelK23>(r0), e4m3x2_to_bf16x2<kSelK23>(r1),
+                                           qb2[2 * c2][0], qb2[2 * c2][1]);
+                            mma_bf16_16816(sb, e4m3x2_to_bf16x2<kSelK01>(r2), e4m3x2_to_bf16x2<kSelK01>(r3),
+                                           e4m3x2_to_bf16x2<kSelK23>(r2), e4m3x2_to_bf16x2<kSelK23>(r3),
+                                           qb2[2 * c2 + 1][0], qb2[2 * c2 + 1][1]);
+                        }
+                        float ksc = sc_ring[(st * 2 + 0) * 8 + (w * 16) / PAGE];  // this warp's page
+                        if (MSTAR_FP8_BIAS_IN_SCALES) ksc *= kTwo60;
+                        float s00 = (sa[0] + sb[0]) * ksc, s01 = (sa[1] + sb[1]) * ksc;  // token g,   heads 2t4, 2t4+1
+                        float s10 = (sa[2] + sb[2]) * ksc, s11 = (sa[3] + sb[3]) * ksc;  // token g+8
+                        if (g >= nv) s00 = s01 = -INFINITY;  // ragged tail: slots >= seq_len may hold any byte
+                        if (g + 8 >= nv) s10 = s11 = -INFINITY;
+                        // ---- online softmax per head: max over the 16 tokens = over the lanes of equal t4
+                        float mx0 = fmaxf(s00, s10), mx1 = fmaxf(s01, s11);
+#pragma unroll
+                        for (int o2 = 4; o2 < 32; o2 <<= 1) {
+                            mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, o2));
+                            mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, o2));
+                        }
+                        const float mn0 = fmaxf(mh0, mx0), mn1 = fmaxf(mh1, mx1);
+                        const float a0 = fast_exp2((mh0 - mn0) * p.scale_log2);
+                        const float a1 = fast_exp2((mh1 - mn1) * p.scale_log2);
+                        const float ms0 = mn0 * p.scale_log2, ms1 = mn1 * p.scale_log2;
+                        mh0 = mn0;
+                        mh1 = mn1;
+                        const float p00 = fast_exp2(s00 * p.scale_log2 - ms0), p01 = fast_exp2(s01 * p.scale_log2 - ms1);
+                        const float p10 = fast_exp2(s10 * p.scale_log2 - ms0), p11 = fast_exp2(s11 * p.scale_log2 - ms1);
+                        lh0 = lh0 * a0 + (p00 + p10);
+                        lh1 = lh1 * a1 + (p01 + p11);
+                        // the page's V scale goes into P (the row sums keep the unscaled probabilities); P^T as the
+                        // B operand = the 8x8 transposes of the two token halves
+                        const float vsc = sc_ring[(st * 2 + 1) * 8 + (w * 16) / PAGE] *
+                                          (MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f);
+                        const uint32_t pb0 = movmatrix_trans(pack_bf16x2(p00 * vsc, p01 * vsc));
+                        const uint32_t pb1 = movmatrix_trans(pack_bf16x2(p10 * vsc, p11 * vsc));
+                        const bool rescale = __any_sync(0xffffffffu, a0 != 1.f || a1 != 1.f);
+                        uint32_t fr[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+                        for (int c = 0; c < D / 16; ++c) {
+                            // transposed 8x8 b16 matrices = byte pairs: this lane gets V[2t4 | 2t4+1][2g | 2g+1] of the
+                            // 16-wide d block c; MMA row g takes the even d, row g+8 the odd d
+                            if ((c & 1) == 0) ldsm_x4_trans(vb + swz128(f_row, c + f_csel), fr[0], fr[1], fr[2], fr[3]);
+                            const uint32_t lo = fr[(c & 1) * 2], hi = fr[(c & 1) * 2 + 1];
+                            if (rescale) {
+                                ot[c][0] *= a0; ot[c][1] *= a1; ot[c][2] *= a0; ot[c][3] *= a1;
+                            }
+                            mma_bf16_16816(ot[c], e4m3x2_to_bf16x2<kSelV02>(lo), e4m3x2_to_bf16x2<kSelV13>(lo),
+                                           e4m3x2_to_bf16x2<kSelV02>(hi), e4m3x2_to_bf16x2<kSelV13>(hi), pb0, pb1);
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(empty_bar(st));
+                    if (++st == nstages) { st = 0; ph ^= 1; }
+                }
+                // ---- hand (m, l, O) of this warp to the merge: row sums over the lanes of equal t4
+#pragma unroll
+                for (int o2 = 4; o2 < 32; o2 <<= 1) {
+                    lh0 += __shfl_xor_sync(0xffffffffu, lh0, o2);
+                    lh1 += __shfl_xor_sync(0xffffffffu, lh1, o2);
+                }
+                float* mo = merge_O + (size_t)w * GH * D;
+                const float f = MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f;
+#pragma unroll
+                for (int c = 0; c < D / 16; ++c) {
+                    *reinterpret_cast<float2*>(mo + (2 * t4) * D + c * 16 + 2 * g) = make_float2(ot[c][0] * f, ot[c][2] * f);
+                    *reinterpret_cast<float2*>(mo + (2 * t4 + 1) * D + c * 16 + 2 * g) =
+                        make_float2(ot[c][1] * f, ot[c][3] * f);
+                }
+                if (g == 0) {
+                    merge_m[w * GH + 2 * t4] = mh0 * p.scale_log2;
+                    merge_m[w * GH + 2 * t4 + 1] = mh1 * p.scale_log2;
+                    merge_l[w * GH + 2 * t4] = lh0;
+                    merge_l[w * GH + 2 * t4 + 1] = lh1;
+                }
+            } else {
+                // Q fragments (A operand), rows = grouped query heads
+                uint32_t qa[D / 16][4];
+                {
+                    const uint16_t* qb = qbuf_g + qs * (SM::kQBytes / 2);
+    #pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        // FP8: this lane's K bytes of a 16-wide d block are d = 4*t4 .. 4*t4+3 (one ldmatrix word), so
+                        // the contraction index is permuted: MMA k-slots (2t4, 2t4+1 | 2t4+8, 2t4+9) <-> d (4t4, 4t4+1 |
+                        // 4t4+2, 4t4+3); Q takes the same permutation
+                        const int c0 = FP8 ? 4 * t4 : 2 * t4, c1 = FP8 ? 4 * t4 + 2 : 8 + 2 * t4;
+                        qa[ks][0] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + c0);
+                        qa[ks][2] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + c1);
+                        if (GH == 16) {
+                            qa[ks][1] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + c0);
+                            qa[ks][3] = *reinterpret_cast<const uint32_t*>(qb + (g + 8) * D + ks * 16 + c1);
+                        } else {
+                            qa[ks][1] = 0u;
+                            qa[ks][3] = 0u;
+                        }
                     }
                 }
-                if (t4 == 0) {
-                    merge_m[w * GH + g] = m0 * p.scale_log2;
-                    merge_l[w * GH + g] = l0;
-                    if (GH == 16) {
-                        merge_m[w * GH + g + 8] = m1 * p.scale_log2;
-                        merge_l[w * GH + g + 8] = l1;
+                if (FP8 && MSTAR_FP8_BIAS_IN_SCALES) {  // Q * 2^60 (exact; |q| < 2^67)
+    #pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks)
+    #pragma unroll
+                        for (int i = 0; i < 4; ++i)
+                            asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(qa[ks][i]) : "r"(qa[ks][i]), "r"(0x5D805D80u));
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(qempty_bar(qs));
+                qs ^= 1;
+                if (qs == 0) qph ^= 1;
+
+                float o[D / 8][4];
+    #pragma unroll
+                for (int j = 0; j < D / 8; ++j) o[j][0] = o[j][1] = o[j][2] = o[j][3] = 0.f;
+                float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;  // rows g and g+8 (raw q.k units)
+
+                const int ntiles = (it.ntok + TOK - 1) / TOK;
+                for (int t = 0; t < ntiles; ++t) {
+                    mbar_wait(full_bar(st), ph);
+                    const int nv = min(16, it.ntok - t * TOK - w * 16);  // valid tokens in this warp's slice
+                    if (nv > 0) {
+                        const uint32_t kb = ring + st * SM::kStageBytes;
+                        const uint32_t vb = kb + KBYTES;
+                        // ---- S = Q K^T for 16 tokens (two n-blocks of 8)
+                        float sc[2][4];
+    #pragma unroll
+                        for (int b = 0; b < 2; ++b) sc[b][0] = sc[b][1] = sc[b][2] = sc[b][3] = 0.f;
+                        if constexpr (FP8) {
+    #pragma unroll
+                            for (int c2 = 0; c2 < D / 32; ++c2) {
+                                uint32_t r0, r1, r2, r3;
+                                ldsm_x4(kb + swz128(f_row, 2 * c2 + f_csel), r0, r1, r2, r3);
+                                const int ka = 2 * c2, kc = 2 * c2 + 1;
+                                mma_bf16_16816(sc[0], qa[ka][0], qa[ka][1], qa[ka][2], qa[ka][3],
+                                               e4m3x2_to_bf16x2<kSelK01>(r0), e4m3x2_to_bf16x2<kSelK23>(r0));
+                                mma_bf16_16816(sc[1], qa[ka][0], qa[ka][1], qa[ka][2], qa[ka][3],
+                                               e4m3x2_to_bf16x2<kSelK01>(r1), e4m3x2_to_bf16x2<kSelK23>(r1));
+                                mma_bf16_16816(sc[0], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
+                                               e4m3x2_to_bf16x2<kSelK01>(r2), e4m3x2_to_bf16x2<kSelK23>(r2));
+                                mma_bf16_16816(sc[1], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
+                                               e4m3x2_to_bf16x2<kSelK01>(r3), e4m3x2_to_bf16x2<kSelK23>(r3));
+                            }
+                            float ksc = sc_ring[(st * 2 + 0) * 8 + (w * 16) / PAGE];  // this warp's page
+                            if (MSTAR_FP8_BIAS_IN_SCALES) ksc *= kTwo60;
+    #pragma unroll
+                            for (int b = 0; b < 2; ++b) {
+                                sc[b][0] *= ksc; sc[b][1] *= ksc; sc[b][2] *= ksc; sc[b][3] *= ksc;
+                            }
+                        } else {
+    #pragma unroll
+                            for (int ks = 0; ks < D / 16; ++ks) {
+                                const uint32_t chunk = 2 * ks + k_csel;
+                                uint32_t b0, b1, b2, b3;
+                                ldsm_x4(kb + (chunk >> 3) * HT + swz128(k_row, chunk & 7), b0, b1, b2, b3);
+                                mma_bf16_16816(sc[0], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b0, b1);
+                                mma_bf16_16816(sc[1], qa[ks][0], qa[ks][1], qa[ks][2], qa[ks][3], b2, b3);
+                            }
+                        }
+                        // ---- mask the ragged tail (slots >= seq_len may hold anything, incl. NaN)
+                        uint32_t vmask_lo = 0xffffffffu, vmask_hi = 0xffffffffu;
+                        if (nv < 16) {
+    #pragma unroll
+                            for (int b = 0; b < 2; ++b) {
+                                const int c = b * 8 + 2 * t4;
+                                if (c >= nv) sc[b][0] = sc[b][2] = -INFINITY;
+                                if (c + 1 >= nv) sc[b][1] = sc[b][3] = -INFINITY;
+                            }
+                            vmask_lo = (2 * t4 < nv ? 0x0000ffffu : 0u) | (2 * t4 + 1 < nv ? 0xffff0000u : 0u);
+                            vmask_hi = (8 + 2 * t4 < nv ? 0x0000ffffu : 0u) | (8 + 2 * t4 + 1 < nv ? 0xffff0000u : 0u);
+                        }
+                        // ---- online softmax (fp32), row max over the quad by shuffles
+                        float mx0 = fmaxf(fmaxf(sc[0][0], sc[0][1]), fmaxf(sc[1][0], sc[1][1]));
+                        mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+                        mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+                        const float mn0 = fmaxf(m0, mx0);
+                        const float a0 = fast_exp2((m0 - mn0) * p.scale_log2);
+                        const float ms0 = mn0 * p.scale_log2;
+                        m0 = mn0;
+                        const float p00 = fast_exp2(sc[0][0] * p.scale_log2 - ms0);
+                        const float p01 = fast_exp2(sc[0][1] * p.scale_log2 - ms0);
+                        const float p10 = fast_exp2(sc[1][0] * p.scale_log2 - ms0);
+                        const float p11 = fast_exp2(sc[1][1] * p.scale_log2 - ms0);
+                        l0 = l0 * a0 + (p00 + p01) + (p10 + p11);
+                        // FP8: the page's V scale goes into P (the row sum l keeps the unscaled probabilities)
+                        const float vsc = FP8 ? sc_ring[(st * 2 + 1) * 8 + (w * 16) / PAGE] *
+                                                    (MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f) : 1.f;
+                        uint32_t pa[4];
+                        pa[0] = pack_bf16x2(p00 * vsc, p01 * vsc);
+                        pa[2] = pack_bf16x2(p10 * vsc, p11 * vsc);
+                        pa[1] = 0u;
+                        pa[3] = 0u;
+                        float a1 = 1.f;
+                        if (GH == 16) {
+                            float mx1 = fmaxf(fmaxf(sc[0][2], sc[0][3]), fmaxf(sc[1][2], sc[1][3]));
+                            mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+                            mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+                            const float mn1 = fmaxf(m1, mx1);
+                            a1 = fast_exp2((m1 - mn1) * p.scale_log2);
+                            const float ms1 = mn1 * p.scale_log2;
+                            m1 = mn1;
+                            const float q00 = fast_exp2(sc[0][2] * p.scale_log2 - ms1);
+                            const float q01 = fast_exp2(sc[0][3] * p.scale_log2 - ms1);
+                            const float q10 = fast_exp2(sc[1][2] * p.scale_log2 - ms1);
+                            const float q11 = fast_exp2(sc[1][3] * p.scale_log2 - ms1);
+                            l1 = l1 * a1 + (q00 + q01) + (q10 + q11);
+                            pa[1] = pack_bf16x2(q00 * vsc, q01 * vsc);
+                            pa[3] = pack_bf16x2(q10 * vsc, q11 * vsc);
+                        }
+                        // ---- O = O * alpha + P V
+                        // FP8 (issue-bound): skip the multiplies of a stage in which no row's running max moved
+                        const bool rescale = !FP8 || __any_sync(0xffffffffu, a0 != 1.f || a1 != 1.f);
+                        uint32_t fr[4] = {0u, 0u, 0u, 0u};
+    #pragma unroll
+                        for (int jj = 0; jj < D / 16; ++jj) {
+                            uint32_t b0, b1, b2, b3;
+                            if constexpr (FP8) {
+                                // transposed 8x8 b16 matrices = byte pairs: this lane gets V[2t4 | 2t4+1][2g | 2g+1] of
+                                // a 16-wide d block; n-block 2jj takes the even d (n = g <-> d = 2g), 2jj+1 the odd d
+                                if ((jj & 1) == 0) ldsm_x4_trans(vb + swz128(f_row, jj + f_csel), fr[0], fr[1], fr[2], fr[3]);
+                                const uint32_t lo = fr[(jj & 1) * 2], hi = fr[(jj & 1) * 2 + 1];
+                                b0 = e4m3x2_to_bf16x2<kSelV02>(lo);
+                                b1 = e4m3x2_to_bf16x2<kSelV02>(hi);
+                                b2 = e4m3x2_to_bf16x2<kSelV13>(lo);
+                                b3 = e4m3x2_to_bf16x2<kSelV13>(hi);
+                            } else {
+                                const uint32_t chunk = 2 * jj + v_csel;
+                                ldsm_x4_trans(vb + (chunk >> 3) * HT + swz128(v_row, chunk & 7), b0, b1, b2, b3);
+                            }
+                            if (nv < 16) {  // 0 * NaN guard: zero V rows that hold no token
+                                b0 &= vmask_lo; b1 &= vmask_hi; b2 &= vmask_lo; b3 &= vmask_hi;
+                            }
+                            if (rescale) {
+                                o[2 * jj][0] *= a0; o[2 * jj][1] *= a0; o[2 * jj + 1][0] *= a0; o[2 * jj + 1][1] *= a0;
+                                if (GH == 16) {
+                                    o[2 * jj][2] *= a1; o[2 * jj][3] *= a1; o[2 * jj + 1][2] *= a1; o[2 * jj + 1][3] *= a1;
+                                }
+                            }
+                            mma_bf16_16816(o[2 * jj], pa[0], pa[1], pa[2], pa[3], b0, b1);
+                            mma_bf16_16816(o[2 * jj + 1], pa[0], pa[1], pa[2], pa[3], b2, b3);
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(empty_bar(st));
+                    if (++st == nstages) { st = 0; ph ^= 1; }
+                }
+
+                // ---- merge the four warps' (m, l, O) through shared memory
+                l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
+                l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+                if (GH == 16) {
+                    l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
+                    l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+                }
+                {
+                    float* mo = merge_O + (size_t)w * GH * D;
+    #pragma unroll
+                    for (int j = 0; j < D / 8; ++j) {
+                        if constexpr (FP8) {  // n-blocks 2c | 2c+1 hold the even | odd d of block c: d = 16c + 4t4 + 0..3
+                            if (j & 1) continue;
+                            const float f = MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f;
+                            *reinterpret_cast<float4*>(mo + g * D + j * 8 + 4 * t4) =
+                                make_float4(o[j][0] * f, o[j + 1][0] * f, o[j][1] * f, o[j + 1][1] * f);
+                            if (GH == 16)
+                                *reinterpret_cast<float4*>(mo + (g + 8) * D + j * 8 + 4 * t4) =
+                                    make_float4(o[j][2] * f, o[j + 1][2] * f, o[j][3] * f, o[j + 1][3] * f);
+                        } else {
+                            *reinterpret_cast<float2*>(mo + g * D + j * 8 + 2 * t4) = make_float2(o[j][0], o[j][1]);
+                            if (GH == 16)
+                                *reinterpret_cast<float2*>(mo + (g + 8) * D + j * 8 + 2 * t4) =
+                                    make_float2(o[j][2], o[j][3]);
+                        }
+                    }
+                    if (t4 == 0) {
+                        merge_m[w * GH + g] = m0 * p.scale_log2;
+                        merge_l[w * GH + g] = l0;
+                        if (GH == 16) {
+                            merge_m[w * GH + g + 8] = m1 * p.scale_log2;
+                            merge_l[w * GH + g + 8] = l1;
+                        }
                     }
                 }
             }
