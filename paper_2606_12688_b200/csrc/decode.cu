@@ -21,9 +21,10 @@ namespace mstar {
 
 // Consumer warps (16 tokens of every ring stage each): 4 for a bf16 pool; 8 for an fp8 pool, where the byte -> bf16
 // conversion is ALU work that two warps per scheduler overlap and a 128-token stage has the bytes of a bf16 one.
-constexpr int decode_consumer_warps(bool fp8) { return fp8 ? 8 : 4; }
-constexpr int decode_tok(bool fp8) { return 16 * decode_consumer_warps(fp8); }          // tokens per ring stage
-constexpr int decode_threads(bool fp8) { return 32 * (decode_consumer_warps(fp8) + 2); }  // + K and V producer
+// With G <= 8 the fp8 consumer (swapped operands, 110 registers) runs 12 warps, three per scheduler.
+constexpr int decode_consumer_warps(bool fp8, bool g16) { return fp8 ? (g16 ? 8 : 12) : 4; }
+constexpr int decode_tok(bool fp8, bool g16) { return 16 * decode_consumer_warps(fp8, g16); }  // tokens per ring stage
+constexpr int decode_threads(bool fp8, bool g16) { return 32 * (decode_consumer_warps(fp8, g16) + 2); }  // + K, V producer
 constexpr int kMaxStages = 16;
 
 struct DecodeParams {
@@ -61,9 +62,9 @@ struct ItemInfo {
 
 template <int D, int GH, int EB>  // EB = bytes per pool element (2 = bf16, 1 = e4m3)
 struct DecodeSmem {
-    static constexpr int kWarps = decode_consumer_warps(EB == 1);
+    static constexpr int kWarps = decode_consumer_warps(EB == 1, GH == 16);
     static constexpr int kStageBytes = 2 * 16 * kWarps * D * EB;
-    static constexpr int kScaleBytes = EB == 1 ? kMaxStages * 2 * 8 * 4 : 0;  // [stage][K|V][page of the stage] fp32
+    static constexpr int kScaleBytes = EB == 1 ? kMaxStages * 2 * 16 * 4 : 0;  // [stage][K|V][page of the stage] fp32
     static constexpr int kQBytes = GH * D * 2;
     static constexpr int kMergeBytes = kWarps * GH * (D + 2) * 4;
     // fixed part after the ring: Q slots, merge buffer, barriers, item info
@@ -118,11 +119,11 @@ __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
 }
 
 template <int D, int PAGE, int GH, bool FP8>
-__global__ void __launch_bounds__(decode_threads(FP8), 1)
+__global__ void __launch_bounds__(decode_threads(FP8, GH == 16), 1)
 decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_constant__ CUtensorMap vmap,
                      const DecodeParams p) {
-    constexpr int NW = decode_consumer_warps(FP8);
-    constexpr int TOK = decode_tok(FP8);
+    constexpr int NW = decode_consumer_warps(FP8, GH == 16);
+    constexpr int TOK = decode_tok(FP8, GH == 16);
     constexpr int PPS = TOK / PAGE;  // pages per stage
     constexpr int EB = FP8 ? 1 : 2;    // bytes per pool element
     constexpr int NH = D * EB / 128;   // 128-byte column slices per row (bf16: 64-column halves)
@@ -240,7 +241,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 if (FP8 && pg >= 0) pg_scale = __ldg((op_isv ? p.v_scale : p.k_scale) + (size_t)pg * p.Hkv + kvh);
                 mbar_wait(empty_bar(st), ph ^ 1);
                 if (FP8) {
-                    if (pg >= 0) sc_ring[(st * 2 + op_isv) * 8 + op_page] = pg_scale;
+                    if (pg >= 0) sc_ring[(st * 2 + op_isv) * 16 + op_page] = pg_scale;
                     __syncwarp();  // the scales are ordered before lane 0's (releasing) arrive
                 }
                 if (lane == 0) mbar_arrive_expect_tx(full_bar(st), (uint32_t)(npg * PAGE * D * EB));
@@ -381,7 +382,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                                            e4m3x2_to_bf16x2<kSelK23>(r2), e4m3x2_to_bf16x2<kSelK23>(r3),
                                            qb2[2 * c2 + 1][0], qb2[2 * c2 + 1][1]);
                         }
-                        float ksc = sc_ring[(st * 2 + 0) * 8 + (w * 16) / PAGE];  // this warp's page
+                        float ksc = sc_ring[(st * 2 + 0) * 16 + (w * 16) / PAGE];  // this warp's page
                         if (MSTAR_FP8_BIAS_IN_SCALES) ksc *= kTwo60;
                         float s00 = (sa[0] + sb[0]) * ksc, s01 = (sa[1] + sb[1]) * ksc;  // token g,   heads 2t4, 2t4+1
                         float s10 = (sa[2] + sb[2]) * ksc, s11 = (sa[3] + sb[3]) * ksc;  // token g+8
@@ -406,7 +407,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                         lh1 = lh1 * a1 + (p01 + p11);
                         // the page's V scale goes into P (the row sums keep the unscaled probabilities); P^T as the
                         // B operand = the 8x8 transposes of the two token halves
-                        const float vsc = sc_ring[(st * 2 + 1) * 8 + (w * 16) / PAGE] *
+                        const float vsc = sc_ring[(st * 2 + 1) * 16 + (w * 16) / PAGE] *
                                           (MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f);
                         const uint32_t pb0 = movmatrix_trans(pack_bf16x2(p00 * vsc, p01 * vsc));
                         const uint32_t pb1 = movmatrix_trans(pack_bf16x2(p10 * vsc, p11 * vsc));
@@ -514,7 +515,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                                 mma_bf16_16816(sc[1], qa[kc][0], qa[kc][1], qa[kc][2], qa[kc][3],
                                                e4m3x2_to_bf16x2<kSelK01>(r3), e4m3x2_to_bf16x2<kSelK23>(r3));
                             }
-                            float ksc = sc_ring[(st * 2 + 0) * 8 + (w * 16) / PAGE];  // this warp's page
+                            float ksc = sc_ring[(st * 2 + 0) * 16 + (w * 16) / PAGE];  // this warp's page
                             if (MSTAR_FP8_BIAS_IN_SCALES) ksc *= kTwo60;
     #pragma unroll
                             for (int b = 0; b < 2; ++b) {
@@ -556,7 +557,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                         const float p11 = fast_exp2(sc[1][1] * p.scale_log2 - ms0);
                         l0 = l0 * a0 + (p00 + p01) + (p10 + p11);
                         // FP8: the page's V scale goes into P (the row sum l keeps the unscaled probabilities)
-                        const float vsc = FP8 ? sc_ring[(st * 2 + 1) * 8 + (w * 16) / PAGE] *
+                        const float vsc = FP8 ? sc_ring[(st * 2 + 1) * 16 + (w * 16) / PAGE] *
                                                     (MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f) : 1.f;
                         uint32_t pa[4];
                         pa[0] = pack_bf16x2(p00 * vsc, p01 * vsc);
@@ -815,7 +816,7 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
     int grid = device_sm_count();
     if (grid > max_items) grid = max_items;
     if (grid < 1) grid = 1;
-    kern<<<grid, decode_threads(FP8), smem, stream>>>(maps.k, maps.v, p);
+    kern<<<grid, decode_threads(FP8, GH == 16), smem, stream>>>(maps.k, maps.v, p);
     MSTAR_CUDA_OK(cudaGetLastError());
     launch_count_add(1);
     return MSTAR_OK;
@@ -826,7 +827,7 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
 extern "C" int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv_heads,
                                                            int32_t max_seq_len) {
     int32_t chunk, nparts;
-    mstar::partition_plan(num_seqs, num_kv_heads, max_seq_len, 0, mstar::decode_tok(false), &chunk, &nparts);
+    mstar::partition_plan(num_seqs, num_kv_heads, max_seq_len, 0, mstar::decode_tok(false, false), &chunk, &nparts);
     return nparts;
 }
 
@@ -863,7 +864,7 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
     const int D = pool->head_dim, PAGE = pool->page_size;
 
     DecodeParams p{};
-    const int32_t tok = decode_tok(fp8);
+    const int32_t tok = decode_tok(fp8, G > 8);
     partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, tok, &p.chunk, &p.nparts);
     if (num_partitions == 0)
         p.balanced = balanced_plan(max_seq_len > 0 ? max_seq_len : 1, tok, &p.nparts, &p.per_min) ? 1 : 0;
