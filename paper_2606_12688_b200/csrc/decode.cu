@@ -21,10 +21,13 @@ namespace mstar {
 
 // Consumer warps (16 tokens of every ring stage each): 4 for a bf16 pool; 8 for an fp8 pool, where the byte -> bf16
 // conversion is ALU work that two warps per scheduler overlap and a 128-token stage has the bytes of a bf16 one.
-// With G <= 8 the fp8 consumer (swapped operands, 110 registers) runs 12 warps, three per scheduler.
-constexpr int decode_consumer_warps(bool fp8, bool g16) { return fp8 ? (g16 ? 8 : 12) : 4; }
-constexpr int decode_tok(bool fp8, bool g16) { return 16 * decode_consumer_warps(fp8, g16); }  // tokens per ring stage
-constexpr int decode_threads(bool fp8, bool g16) { return 32 * (decode_consumer_warps(fp8, g16) + 2); }  // + K, V producer
+// With G <= 8 the fp8 consumer (swapped operands, 111 registers) can run 12 warps, three per scheduler: the host
+// picks them for long sequences (192-token stages cost short, ragged streams more in tail tiles than they gain).
+constexpr int decode_tok(int nw) { return 16 * nw; }            // tokens per ring stage
+constexpr int decode_threads(int nw) { return 32 * (nw + 2); }  // + K and V producer warps
+static int decode_pick_warps(bool fp8, int G, int max_seq_len) {
+    return fp8 ? ((G <= 8 && max_seq_len > 8192) ? 12 : 8) : 4;
+}
 constexpr int kMaxStages = 16;
 
 struct DecodeParams {
@@ -60,9 +63,9 @@ struct ItemInfo {
     int32_t s, kvh, part, tok0, ntok;
 };
 
-template <int D, int GH, int EB>  // EB = bytes per pool element (2 = bf16, 1 = e4m3)
+template <int D, int GH, int EB, int NWARPS>  // EB = bytes per pool element (2 = bf16, 1 = e4m3)
 struct DecodeSmem {
-    static constexpr int kWarps = decode_consumer_warps(EB == 1, GH == 16);
+    static constexpr int kWarps = NWARPS;
     static constexpr int kStageBytes = 2 * 16 * kWarps * D * EB;
     static constexpr int kScaleBytes = EB == 1 ? kMaxStages * 2 * 16 * 4 : 0;  // [stage][K|V][page of the stage] fp32
     static constexpr int kQBytes = GH * D * 2;
@@ -118,18 +121,18 @@ __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
     return d;
 }
 
-template <int D, int PAGE, int GH, bool FP8>
-__global__ void __launch_bounds__(decode_threads(FP8, GH == 16), 1)
+template <int D, int PAGE, int GH, bool FP8, int NWARPS>
+__global__ void __launch_bounds__(decode_threads(NWARPS), 1)
 decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_constant__ CUtensorMap vmap,
                      const DecodeParams p) {
-    constexpr int NW = decode_consumer_warps(FP8, GH == 16);
-    constexpr int TOK = decode_tok(FP8, GH == 16);
+    constexpr int NW = NWARPS;
+    constexpr int TOK = decode_tok(NWARPS);
     constexpr int PPS = TOK / PAGE;  // pages per stage
     constexpr int EB = FP8 ? 1 : 2;    // bytes per pool element
     constexpr int NH = D * EB / 128;   // 128-byte column slices per row (bf16: 64-column halves)
     constexpr int HT = TOK * 128;      // bytes of one slice tile (TOK rows x 128 B)
     constexpr int KBYTES = NH * HT;    // K part of a stage
-    using SM = DecodeSmem<D, GH, EB>;
+    using SM = DecodeSmem<D, GH, EB, NWARPS>;
     static_assert(!FP8 || D == 128, "fp8 pool: one 128-byte line per token row");
     constexpr int VEC = D / 32;
 
@@ -798,16 +801,16 @@ static void partition_plan(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t 
     if (num_partitions > 0 && *nparts > num_partitions) *nparts = num_partitions;
 }
 
-template <int D, int PAGE, int GH, bool FP8>
+template <int D, int PAGE, int GH, bool FP8, int NWARPS>
 static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, cudaStream_t stream) {
-    using SM = DecodeSmem<D, GH, FP8 ? 1 : 2>;
+    using SM = DecodeSmem<D, GH, FP8 ? 1 : 2, NWARPS>;
     const int max_smem = device_max_smem_optin();
     int nstages = (int)(((int64_t)max_smem - 1024 - SM::kFixed - (int64_t)(p.S + 1) * 4 - 16) / SM::kStageBytes);
     if (nstages > kMaxStages) nstages = kMaxStages;
     if (nstages < 2) return MSTAR_ERR_UNSUPPORTED;
     p.nstages = nstages;
     const size_t smem = SM::bytes(nstages, p.S);
-    auto kern = decode_splitk_kernel<D, PAGE, GH, FP8>;
+    auto kern = decode_splitk_kernel<D, PAGE, GH, FP8, NWARPS>;
     static bool attr_set = false;  // per instantiation
     if (!attr_set) {
         MSTAR_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
@@ -816,7 +819,7 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
     int grid = device_sm_count();
     if (grid > max_items) grid = max_items;
     if (grid < 1) grid = 1;
-    kern<<<grid, decode_threads(FP8, GH == 16), smem, stream>>>(maps.k, maps.v, p);
+    kern<<<grid, decode_threads(NWARPS), smem, stream>>>(maps.k, maps.v, p);
     MSTAR_CUDA_OK(cudaGetLastError());
     launch_count_add(1);
     return MSTAR_OK;
@@ -827,7 +830,7 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
 extern "C" int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv_heads,
                                                            int32_t max_seq_len) {
     int32_t chunk, nparts;
-    mstar::partition_plan(num_seqs, num_kv_heads, max_seq_len, 0, mstar::decode_tok(false, false), &chunk, &nparts);
+    mstar::partition_plan(num_seqs, num_kv_heads, max_seq_len, 0, mstar::decode_tok(4), &chunk, &nparts);
     return nparts;
 }
 
@@ -864,7 +867,8 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
     const int D = pool->head_dim, PAGE = pool->page_size;
 
     DecodeParams p{};
-    const int32_t tok = decode_tok(fp8, G > 8);
+    const int nw = decode_pick_warps(fp8, G, max_seq_len);
+    const int32_t tok = decode_tok(nw);
     partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, tok, &p.chunk, &p.nparts);
     if (num_partitions == 0)
         p.balanced = balanced_plan(max_seq_len > 0 ? max_seq_len : 1, tok, &p.nparts, &p.per_min) ? 1 : 0;
@@ -902,17 +906,21 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
     const int max_items = max_items64 > (1 << 30) ? (1 << 30) : (int)max_items64;
     cudaStream_t st = (cudaStream_t)stream;
     const bool g16 = G > 8;
-#define MSTAR_DECODE_CASE(DD, PP, F8)                                                    \
-    if (D == DD && PAGE == PP && fp8 == F8)                                              \
-        rc = g16 ? launch_decode<DD, PP, 16, F8>(maps, p, max_items, st)                 \
-                 : launch_decode<DD, PP, 8, F8>(maps, p, max_items, st);
+#define MSTAR_DECODE_CASE(DD, PP, F8, NWW)                                               \
+    if (D == DD && PAGE == PP && fp8 == F8 && nw == NWW)                                 \
+        rc = g16 ? launch_decode<DD, PP, 16, F8, NWW>(maps, p, max_items, st)            \
+                 : launch_decode<DD, PP, 8, F8, NWW>(maps, p, max_items, st);
     rc = MSTAR_ERR_UNSUPPORTED;
-    MSTAR_DECODE_CASE(128, 16, false)
-    MSTAR_DECODE_CASE(128, 32, false)
-    MSTAR_DECODE_CASE(64, 16, false)
-    MSTAR_DECODE_CASE(64, 32, false)
-    MSTAR_DECODE_CASE(128, 16, true)
-    MSTAR_DECODE_CASE(128, 32, true)
+    MSTAR_DECODE_CASE(128, 16, false, 4)
+    MSTAR_DECODE_CASE(128, 32, false, 4)
+    MSTAR_DECODE_CASE(64, 16, false, 4)
+    MSTAR_DECODE_CASE(64, 32, false, 4)
+    MSTAR_DECODE_CASE(128, 16, true, 8)
+    MSTAR_DECODE_CASE(128, 32, true, 8)
+    if (!g16) {  // 12 warps need the 111-register consumer of the G <= 8 form
+        if (D == 128 && PAGE == 16 && fp8 && nw == 12) rc = launch_decode<128, 16, 8, true, 12>(maps, p, max_items, st);
+        if (D == 128 && PAGE == 32 && fp8 && nw == 12) rc = launch_decode<128, 32, 8, true, 12>(maps, p, max_items, st);
+    }
 #undef MSTAR_DECODE_CASE
     if (rc != MSTAR_OK) return rc;
 

@@ -94,6 +94,15 @@ def test_decode_fp8_many_sequences_nhd_and_long_stream():
     run_case(b, parts_list=(0, 4), layout="NHD")
 
 
+@pytest.mark.parametrize("p,G", [(16, 7), (32, 4), (16, 1)])
+def test_decode_fp8_long_sequences_take_the_12_warp_kernel(p, G):
+    """max_seq_len > 8192 and G <= 8 select 12 consumer warps on 192-token stages: lengths around the stage and
+    partition boundaries of that geometry, next to one long stream."""
+    lens = [9000, 0, 1, 191, 192, 193, 383, 385, 16 * 192 + 5, 2111, 2113]
+    b = small_batch(360 + G, lens, Hq=G * 2, Hkv=2, p=p, table_width=9000 // p + 8)
+    run_case(b, parts_list=(0, 1, 5, 16))
+
+
 def test_decode_fp8_len1_is_the_dequantised_v_row():
     b = small_batch(320, [1, 1, 1], Hq=8, Hkv=2, p=16)
     k_scale, v_scale = W.fp8_page_scales(3, b.num_pages, b.num_kv_heads)
