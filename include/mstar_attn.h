@@ -157,7 +157,8 @@ int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv
  * Arguments as mstar_kv_append; bit-exact by definition (R24-R25).
  *
  * mstar_paged_attn_decode_fp8: mstar_paged_attn_decode on the dequantised K and V; all other arguments, the
- * partition rules and the workspace size are those of mstar_paged_attn_decode.  Codes are converted to bf16
+ * partition rules and the workspace size are those of mstar_paged_attn_decode, with partition lengths rounded up to
+ * the kernel's stage size (128 tokens, or 192 when Hq/Hkv <= 8 and max_seq_len > 8192) instead of 64.  Codes are converted to bf16
  * exactly in the kernel; k_scale multiplies the logits of a page, v_scale its probabilities (fp32).  Slots at or
  * past seq_len may hold any byte.  NaN codes inside a sequence give undefined output.
  */
