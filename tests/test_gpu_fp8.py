@@ -86,6 +86,12 @@ def test_decode_fp8_edge_lengths(p, G):
     run_case(b, parts_list=(0, 1, 3, 9))
 
 
+@pytest.mark.parametrize("Hkv,G", [(1, 8), (8, 4), (1, 12)])
+def test_decode_fp8_kv_head_counts(Hkv, G):
+    b = small_batch(380 + Hkv + G, [700, 1, 65, 300, 129], Hq=Hkv * G, Hkv=Hkv, p=32)
+    run_case(b, parts_list=(0, 3))
+
+
 def test_decode_fp8_many_sequences_nhd_and_long_stream():
     rng = np.random.default_rng(17)
     lens = rng.integers(1, 500, 149).tolist()

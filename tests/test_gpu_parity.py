@@ -141,6 +141,13 @@ def test_decode_edge_lengths(D, p, G):
     run_decode_case(b, parts_list=(0, 1, 3, 9), check_f32=(G in (1, 7)))
 
 
+@pytest.mark.parametrize("Hkv,G", [(1, 8), (1, 1), (8, 4), (8, 2)])
+def test_decode_kv_head_counts(Hkv, G):
+    """SURVEY 8(c) edge matrix: Hkv in {1, 8} (2 and 4 are what the other cases use)."""
+    b = small_batch(260 + Hkv * 10 + G, [700, 1, 65, 300, 129], Hq=Hkv * G, Hkv=Hkv, D=128, p=32)
+    run_decode_case(b, parts_list=(0, 3), check_f32=False)
+
+
 def test_decode_many_sequences_and_nhd_layout():
     rng = np.random.default_rng(7)
     lens = rng.integers(1, 700, 300).tolist()
@@ -331,6 +338,12 @@ def test_prefill_ragged_small(D, p, G):
     b = small_batch(300 + G, lens, q_lens=qls, Hq=G * 2, Hkv=2, D=D, p=p)
     run_prefill_case(b)
     run_prefill_case(b, causal=False)
+
+
+@pytest.mark.parametrize("Hkv,G", [(1, 8), (8, 4)])
+def test_prefill_kv_head_counts(Hkv, G):
+    b = small_batch(270 + Hkv, [300, 140, 64], q_lens=[130, 140, 1], Hq=Hkv * G, Hkv=Hkv, D=128, p=16)
+    run_prefill_case(b)
 
 
 def test_prefill_new_tokens_times_prefix_matrix():
