@@ -161,6 +161,10 @@ int32_t mstar_paged_attn_decode_auto_partitions(int32_t num_seqs, int32_t num_kv
  * the kernel's stage size (128 tokens, or 192 when Hq/Hkv <= 8 and max_seq_len > 8192) instead of 64.  Codes are converted to bf16
  * exactly in the kernel; k_scale multiplies the logits of a page, v_scale its probabilities (fp32).  Slots at or
  * past seq_len may hold any byte.  NaN codes inside a sequence give undefined output.
+ *
+ * Page moves of a quantised pool are the bit copies above on the same bytes described as a bf16 pool of head_dim 64
+ * (two codes per element, all strides halved): mstar_kv_copy_pages / mstar_kv_gather need no fp8 variant.  The scale
+ * rows of the moved pages are the caller's to copy.
  */
 int mstar_kv_append_fp8(const mstar_kv_pool* pool8, const float* k_scale, const float* v_scale, const void* k_new,
                         const void* v_new, const int64_t* slot_mapping, int64_t num_tokens, void* stream);

@@ -192,6 +192,13 @@ class KVPoolFp8:
             self.head_dim, int(k_pool.stride(0)), int(k_pool.stride(1)), int(k_pool.stride(2)))
 
 
+    def as_bit_pool(self) -> "KVPool":
+        """The same bytes described as a bf16 pool of head_dim 64 (two codes per 16-bit element): what the bit-copy
+        entry points (mstar_kv_copy_pages, mstar_kv_gather) take to move pages of a quantised pool.  The scales
+        [num_pages, Hkv] travel separately (they are the caller's)."""
+        return KVPool(self.k_pool.view(torch.bfloat16), self.v_pool.view(torch.bfloat16))
+
+
 def kv_append_fp8(pool: KVPoolFp8, k_new: torch.Tensor, v_new: torch.Tensor, slot_mapping: torch.Tensor) -> None:
     """mstar_kv_append_fp8: quantise k_new/v_new [T,Hkv,D] bf16 to E4M3 codes at slot_mapping [T] int64."""
     _want(k_new, torch.bfloat16, "k_new"); _want(v_new, torch.bfloat16, "v_new")

@@ -203,6 +203,46 @@ def test_decode_fp8_config2_bagel_cfg_pairs():
     print("config 2 fp8", stats)
 
 
+def test_fp8_page_moves_through_the_bit_pool_view():
+    """mstar_kv_copy_pages / mstar_kv_gather on the quantised pool described as a bf16 pool of head_dim 64: moved pages
+    (codes by the kernel, scale rows by the caller) decode bit-identically; gathered rows equal the oracle's codes."""
+    b = small_batch(390, [300, 77, 1], Hq=8, Hkv=2, p=16, pool=96)
+    k_scale, v_scale = W.fp8_page_scales(6, b.num_pages, b.num_kv_heads)
+    db = DeviceBatchFp8(b, k_scale, v_scale)
+    db.quantise_store()
+    db.append()
+    out0, _ = db.decode(num_partitions=2)
+    bits = db.pool.as_bit_pool()
+    used = np.zeros(b.num_pages, dtype=bool)
+    used[b.used_pages] = True
+    free = np.flatnonzero(~used)[:len(b.used_pages)].astype(np.int64)
+    src = torch.from_numpy(b.used_pages.astype(np.int64)).cuda()
+    dst = torch.from_numpy(free).cuda()
+    mstar.kv_copy_pages(bits, bits, dst, src)
+    db.k_scale[dst] = db.k_scale[src]
+    db.v_scale[dst] = db.v_scale[src]
+    remap = np.full(b.num_pages, -1, dtype=np.int32)
+    remap[b.used_pages] = free
+    bt2 = np.where(b.block_table >= 0, remap[np.maximum(b.block_table, 0)], -1).astype(np.int32)
+    db.block_table = torch.from_numpy(bt2).cuda()
+    db.k_pool[src] = 0x7F  # the old pages are poison now
+    db.v_pool[src] = 0x7F
+    out1, _ = db.decode(num_partitions=2)
+    assert torch.equal(out0.view(torch.int16), out1.view(torch.int16))
+    # gather the codes of every sequence to contiguous rows
+    cu = np.zeros(b.num_seqs + 1, dtype=np.int32)
+    cu[1:] = np.cumsum(b.seq_lens)
+    kg = torch.zeros((int(cu[-1]), b.num_kv_heads, 64), dtype=torch.bfloat16, device="cuda")
+    vg = torch.zeros_like(kg)
+    mstar.kv_gather(kg, vg, bits, db.block_table, db.seq_lens, torch.from_numpy(cu).cuda())
+    k8, v8, _, _ = oracle_pool(b, k_scale, v_scale)
+    gk = kg.view(torch.uint8).cpu().numpy()
+    for s in range(b.num_seqs):
+        for j in range(int(b.seq_lens[s])):
+            pg = int(b.compact_block_table[s, j // 16])
+            assert np.array_equal(gk[cu[s] + j], k8[pg, :, j % 16, :])
+
+
 def test_fp8_error_codes():
     b = small_batch(330, [5], Hq=8, Hkv=2, p=16)
     dev = "cuda"
