@@ -13,7 +13,7 @@ import sys
 PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libmstar_attn.so")
-SOURCES = ["host_common.cu", "kv_append.cu", "kv_append_fp8.cu", "kv_transfer.cu", "decode.cu", "merge_states.cu", "prefill.cu", "prefill_umma.cu"]
+SOURCES = ["host_common.cu", "kv_append.cu", "kv_append_fp8.cu", "kv_transfer.cu", "decode.cu", "merge_states.cu", "prefill.cu", "prefill_umma.cu", "hbm_probe.cu"]
 HEADERS = ["host_common.h", "ptx.cuh", "umma.cuh", os.path.join("..", "..", "include", "mstar_attn.h")]
 
 NVCC_FLAGS = [
