@@ -204,6 +204,10 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         __syncwarp();
         const int n_items = carry * p.Hkv;
         const uint64_t pol = policy_evict_first();
+        // Programmatic dependent launch behind mstar_kv_append (the only kernels of the library that release their
+        // dependents early): launch latency, the set-up above and the work-list prefix sums overlap the append; the
+        // pool is read only after the append grid has completed.  Behind any other kernel this returns at once.
+        asm volatile("griddepcontrol.wait;" ::: "memory");
 
         // this lane's TMA op within a stage: (page i, K or V, 64-column half)
         constexpr int OPS = PPS * NH;
@@ -819,7 +823,17 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
     int grid = device_sm_count();
     if (grid > max_items) grid = max_items;
     if (grid < 1) grid = 1;
-    kern<<<grid, decode_threads(NWARPS), smem, stream>>>(maps.k, maps.v, p);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(decode_threads(NWARPS));
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, kern, maps.k, maps.v, p));
     MSTAR_CUDA_OK(cudaGetLastError());
     launch_count_add(1);
     return MSTAR_OK;

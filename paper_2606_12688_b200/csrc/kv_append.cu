@@ -24,6 +24,8 @@ __global__ void __launch_bounds__(256) kv_append_kernel(uint16_t* __restrict__ k
                                                         int32_t chunks_per_row /* D/8 */, int32_t Hkv,
                                                         int32_t page_size, int64_t stride_page, int64_t stride_head,
                                                         int64_t stride_token) {
+    // a decode launched behind this append may start its set-up now; it reads the pool only after this grid is done
+    asm volatile("griddepcontrol.launch_dependents;");
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     for (; i0 < n_chunks; i0 += stride * UNROLL) {

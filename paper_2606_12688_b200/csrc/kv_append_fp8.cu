@@ -41,6 +41,8 @@ __global__ void __launch_bounds__(256) kv_append_fp8_kernel(uint8_t* __restrict_
                                                             int32_t chunks_per_row /* D/8 */, int32_t Hkv,
                                                             int32_t page_size, int64_t stride_page, int64_t stride_head,
                                                             int64_t stride_token) {
+    // a decode launched behind this append may start its set-up now; it reads the pool only after this grid is done
+    asm volatile("griddepcontrol.launch_dependents;");
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_chunks; i += stride) {
         const int64_t row = i / chunks_per_row;  // (token, head)
