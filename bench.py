@@ -40,10 +40,10 @@ METRIC = "paged_decode_attn_GBps"
 UNIT = "GB/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r1d_full_summary.csv: split-K read + write, combine read; prefill read + write); valid for the
+# (profiles/r1f_full_summary.csv: split-K read + write, combine read; prefill read + write); valid for the
 # full-size workloads only.
-NCU_TRAFFIC = {"decode": 2147743000 + 5796096 + 4272000, "prefill": 88004000 + 12191232,
-               "source": "profiles/r1d_full_summary.csv"}
+NCU_TRAFFIC = {"decode": 2147743000 + 5533952 + 4272000, "prefill": 87985000 + 12952064,
+               "source": "profiles/r1f_full_summary.csv"}
 
 
 def load_peaks():
