@@ -71,6 +71,9 @@ def kv_append_fp8(k_pool8, v_pool8, k_scale, v_scale, k_new, v_new, slot_mapping
     ks, vs = np.asarray(k_scale, dtype=np.float32), np.asarray(v_scale, dtype=np.float32)
     slot = np.asarray(slot_mapping, dtype=np.int64)
     ok = slot >= 0
+    # R19: two rows naming one slot in a call is a caller error; the bf16 oracle's sequential loop gives "last writer
+    # wins", numpy fancy assignment gives no stated order, so this vectorised form refuses duplicates outright
+    assert np.unique(slot[ok]).size == int(ok.sum()), "duplicate slots in one append (undefined, R19)"
     page, off = slot[ok] // p, slot[ok] % p
     # fp32 / fp32 -> fp32, IEEE round to nearest even, element by element (the scale of the row's page and head)
     yk = kf[ok] / ks[page][:, :, None]
