@@ -513,18 +513,19 @@ def run_ours(args):
     # of random pages, the same memory the decode kernel streams), CUDA events, median of 7 after 2 warm-ups
     read_ceiling = None
     if rank == 0:
+        from paper_2606_12688_b200 import bench_aux
         nbytes = min(4 << 30, D5.k_pool.numel() * 2)
         ts = []
         for _ in range(9):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            mstar.hbm_read_probe(D5.k_pool, nbytes)
+            bench_aux.hbm_read_probe(D5.k_pool, nbytes)
             e1.record()
             torch.cuda.synchronize()
             ts.append(e0.elapsed_time(e1))
         ms_probe = sorted(ts[2:])[len(ts[2:]) // 2]
         read_ceiling = {"GBps": nbytes / (ms_probe * 1e-3) / 1e9, "bytes": nbytes, "ms": ms_probe,
-                        "kernel": "mstar_hbm_read_probe (16-byte read-only loads, 8 in flight per thread)"}
+                        "kernel": "bench_aux hbm_read_probe (16-byte read-only loads, 8 in flight per thread)"}
 
     other = None
     if rank == 0 and not args.no_other:

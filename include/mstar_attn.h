@@ -225,14 +225,6 @@ int mstar_build_slot_mapping(const int32_t* block_table, int64_t block_table_str
                              const int32_t* cu_seqlens_q, const int32_t* seq_lens, int32_t num_seqs,
                              int32_t total_q, int32_t page_size, int64_t* slot_mapping_out, void* stream);
 
-/*
- * mstar_hbm_read_probe: measurement aid, not a step of the path.  Streams `bytes` bytes
- * (a multiple of 16, 16-B aligned, device) through 16-byte read-only loads and adds the wrapping sum of their 32-bit
- * words to *sum_out (device, may be NULL; not zeroed by the call).  bench.py times it over 4 GiB of the K pool as the
- * practical HBM-read ceiling beside the decode kernel's rate.
- */
-int mstar_hbm_read_probe(const void* buf, size_t bytes, unsigned long long* sum_out, void* stream);
-
 /* Number of kernels the last call on this thread enqueued (bench.py's gpu_launches claim). */
 int32_t mstar_last_launch_count(void);
 

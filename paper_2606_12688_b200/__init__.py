@@ -25,7 +25,6 @@ from .binding import (  # noqa: F401
     build_slot_mapping,
     decode_auto_partitions,
     decode_workspace_bytes,
-    hbm_read_probe,
     kv_append,
     kv_append_fp8,
     kv_copy_pages,

@@ -33,7 +33,6 @@ EXPORTS = (
     "mstar_paged_attn_prefill_workspace_bytes",
     "mstar_paged_attn_prefill",
     "mstar_build_slot_mapping",
-    "mstar_hbm_read_probe",
     "mstar_last_launch_count",
     "mstar_status_string",
     "mstar_version",
@@ -110,8 +109,6 @@ def load_library() -> ctypes.CDLL:
     lib.mstar_build_slot_mapping.restype = c.c_int
     lib.mstar_build_slot_mapping.argtypes = [c.c_void_p, c.c_int64, c.c_void_p, c.c_void_p, c.c_int32, c.c_int32,
                                              c.c_int32, c.c_void_p, c.c_void_p]
-    lib.mstar_hbm_read_probe.restype = c.c_int
-    lib.mstar_hbm_read_probe.argtypes = [c.c_void_p, c.c_size_t, c.c_void_p, c.c_void_p]
     lib.mstar_last_launch_count.restype = c.c_int32
     lib.mstar_last_launch_count.argtypes = []
     lib.mstar_status_string.restype = c.c_char_p
@@ -296,16 +293,6 @@ def merge_attn_states(out: torch.Tensor, out_a: torch.Tensor, lse_a: torch.Tenso
     lib = load_library()
     _check(lib.mstar_merge_attn_states(_ptr(out), _ptr(lse_out), _ptr(out_a), _ptr(lse_a), _ptr(row_map_a),
                                        _ptr(out_b), _ptr(lse_b), N, D, flags, _stream()), "mstar_merge_attn_states")
-
-
-def hbm_read_probe(buf: torch.Tensor, nbytes: int, sum_out: Optional[torch.Tensor] = None) -> None:
-    """mstar_hbm_read_probe: stream the first ``nbytes`` bytes of ``buf`` through 16-byte read-only loads."""
-    if not buf.is_cuda:
-        raise MstarError("buf must be a CUDA tensor")
-    if sum_out is not None:
-        _want(sum_out, torch.int64, "sum_out")
-    _check(load_library().mstar_hbm_read_probe(_ptr(buf), int(nbytes), _ptr(sum_out), _stream()),
-           "mstar_hbm_read_probe")
 
 
 def decode_auto_partitions(num_seqs: int, num_kv_heads: int, max_seq_len: int) -> int:

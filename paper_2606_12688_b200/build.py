@@ -1,4 +1,4 @@
-"""Build ``libmstar_attn.so`` in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+"""Build ``libmstar_attn.so`` (and the bench-only ``bench_aux/libmstar_benchaux.so``) in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_2606_12688_b200.build [--force] [--verbose]
 
@@ -13,7 +13,12 @@ import sys
 PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libmstar_attn.so")
-SOURCES = ["host_common.cu", "kv_append.cu", "kv_append_fp8.cu", "kv_transfer.cu", "decode.cu", "merge_states.cu", "prefill.cu", "prefill_umma.cu", "hbm_probe.cu"]
+SOURCES = ["host_common.cu", "kv_append.cu", "kv_append_fp8.cu", "kv_transfer.cu", "decode.cu", "merge_states.cu",
+           "prefill.cu", "prefill_umma.cu"]
+# measurement aid for bench.py, a library of its own (not part of the product ABI)
+AUX_DIR = os.path.join(PKG_DIR, "bench_aux")
+AUX_LIB_PATH = os.path.join(AUX_DIR, "libmstar_benchaux.so")
+AUX_SOURCES = ["hbm_probe.cu"]
 HEADERS = ["host_common.h", "ptx.cuh", "umma.cuh", os.path.join("..", "..", "include", "mstar_attn.h")]
 
 NVCC_FLAGS = [
@@ -30,10 +35,11 @@ def _nvcc() -> str:
 
 
 def _stale() -> bool:
-    if not os.path.exists(LIB_PATH):
+    if not os.path.exists(LIB_PATH) or not os.path.exists(AUX_LIB_PATH):
         return True
-    t = os.path.getmtime(LIB_PATH)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    t = min(os.path.getmtime(LIB_PATH), os.path.getmtime(AUX_LIB_PATH))
+    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.join(AUX_DIR, f) for f in AUX_SOURCES]
+    deps.append(os.path.abspath(__file__))
     return any(os.path.getmtime(d) > t for d in deps if os.path.exists(d))
 
 
@@ -44,15 +50,16 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     procs = []
     build_dir = os.path.join(PKG_DIR, "build")
     os.makedirs(build_dir, exist_ok=True)
-    for src in SOURCES:
+    aux_objs = []
+    for src_dir, src in [(CSRC, f) for f in SOURCES] + [(AUX_DIR, f) for f in AUX_SOURCES]:
         obj = os.path.join(build_dir, src.replace(".cu", ".o"))
-        cmd = [_nvcc(), *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [_nvcc(), *NVCC_FLAGS, "-c", os.path.join(src_dir, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas")
             cmd.insert(2, "-v")
             print(" ".join(cmd), flush=True)
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
-        objs.append(obj)
+        (objs if src_dir == CSRC else aux_objs).append(obj)
     failed = False
     for src, pr in procs:
         out, _ = pr.communicate()
@@ -63,10 +70,12 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(out)
     if failed:
         raise RuntimeError("nvcc failed; see messages above")
-    tmp = LIB_PATH + ".tmp.%d" % os.getpid()
-    link = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs, "-cudart", "static"]
-    subprocess.check_call(link)
-    os.replace(tmp, LIB_PATH)
+    for path, parts in ((LIB_PATH, objs), (AUX_LIB_PATH, aux_objs)):
+        tmp = path + ".tmp.%d" % os.getpid()
+        link = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *parts, "-cudart",
+                "static"]
+        subprocess.check_call(link)
+        os.replace(tmp, path)
     return LIB_PATH
 
 

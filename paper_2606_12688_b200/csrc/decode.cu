@@ -177,6 +177,11 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
     // let the combine grid (launched with programmatic stream serialization) become resident now; it blocks in
     // griddepcontrol.wait until this grid has completed
     asm volatile("griddepcontrol.launch_dependents;");
+    // This grid is itself launched with programmatic stream serialization: everything above (barrier init, Q-slot
+    // zeroing) may overlap the tail of the previous kernel in the stream.  Every global read or write below -- seq_lens
+    // and the block table may have been written by that kernel (a device-side step advance in a captured decode
+    // loop), `out` may still be read by it -- happens after it has completed and its writes are visible.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 
     if (warp >= NW) {
         // Two producer warps walk the same item list: warp NW loads the K half of every stage (and Q and the item
@@ -204,11 +209,6 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         __syncwarp();
         const int n_items = carry * p.Hkv;
         const uint64_t pol = policy_evict_first();
-        // Programmatic dependent launch behind mstar_kv_append (the only kernels of the library that release their
-        // dependents early): launch latency, the set-up above and the work-list prefix sums overlap the append; the
-        // pool is read only after the append grid has completed.  Behind any other kernel this returns at once.
-        asm volatile("griddepcontrol.wait;" ::: "memory");
-
         // this lane's TMA op within a stage: (page i, K or V, 64-column half)
         constexpr int OPS = PPS * NH;
         const int op_page = lane / NH;
@@ -815,11 +815,8 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
     p.nstages = nstages;
     const size_t smem = SM::bytes(nstages, p.S);
     auto kern = decode_splitk_kernel<D, PAGE, GH, FP8, NWARPS>;
-    static bool attr_set = false;  // per instantiation
-    if (!attr_set) {
-        MSTAR_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-        attr_set = true;
-    }
+    static PerDeviceOnce attr_once;  // per instantiation
+    MSTAR_CUDA_OK(set_max_dynamic_smem(attr_once, kern, max_smem));
     int grid = device_sm_count();
     if (grid > max_items) grid = max_items;
     if (grid < 1) grid = 1;

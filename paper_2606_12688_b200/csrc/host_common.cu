@@ -136,32 +136,50 @@ int make_rows_map(const void* base, int64_t rows, int32_t num_heads, int32_t hea
     return r == CUDA_SUCCESS ? MSTAR_OK : MSTAR_ERR_INVALID_ARG;
 }
 
-int device_sm_count() {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
-            (void)cudaGetLastError();
-            n = 0;
-            return 148;
-        }
+int current_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 0;
     }
-    return n;
+    return dev;
+}
+
+static std::mutex g_dev_mu;
+constexpr int kMaxCachedDevices = 64;
+
+static int device_attr_cached(cudaDeviceAttr attr, int (&cache)[kMaxCachedDevices], int fallback) {
+    const int dev = current_device();
+    std::lock_guard<std::mutex> lock(g_dev_mu);
+    if (dev >= 0 && dev < kMaxCachedDevices && cache[dev] > 0) return cache[dev];
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, attr, dev) != cudaSuccess || v <= 0) {
+        (void)cudaGetLastError();
+        return fallback;
+    }
+    if (dev >= 0 && dev < kMaxCachedDevices) cache[dev] = v;
+    return v;
+}
+
+int device_sm_count() {
+    static int cache[kMaxCachedDevices] = {};
+    return device_attr_cached(cudaDevAttrMultiProcessorCount, cache, 148);
 }
 
 int device_max_smem_optin() {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&n, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) {
-            (void)cudaGetLastError();
-            n = 0;
-            return 227 * 1024;
-        }
-    }
-    return n;
+    static int cache[kMaxCachedDevices] = {};
+    return device_attr_cached(cudaDevAttrMaxSharedMemoryPerBlockOptin, cache, 227 * 1024);
+}
+
+bool per_device_test(PerDeviceOnce& once, int dev) {
+    if (dev < 0 || dev >= 64) return false;
+    std::lock_guard<std::mutex> lock(g_dev_mu);
+    return (once.done >> dev) & 1ull;
+}
+void per_device_mark(PerDeviceOnce& once, int dev) {
+    if (dev < 0 || dev >= 64) return;
+    std::lock_guard<std::mutex> lock(g_dev_mu);
+    once.done |= 1ull << dev;
 }
 
 }  // namespace mstar

@@ -23,7 +23,8 @@ int check_pool_fp8(const mstar_kv_pool* pool);
 // One tensor map per pool tensor: 4-D view (D, page_size, Hkv, num_pages) of bf16 with a
 // (64, page_size, 1, 1) box and 128-B swizzle, so that a (page, kv head, 64-column half) slab lands in
 // shared memory as page_size rows of 128 B, conflict-free for ldmatrix.  Cached per
-// (pointer, geometry); thread-safe.
+// (pointer, geometry); thread-safe.  A tensor map encodes a (unified) virtual address and a geometry, nothing of
+// the device that owns the memory, so the cache needs no device key.
 struct PoolMaps {
     CUtensorMap k;
     CUtensorMap v;
@@ -46,8 +47,26 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
                         size_t workspace_bytes, cudaStream_t stream);
 size_t prefill_umma_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads);
 
+// Properties of the CURRENT device (cudaGetDevice), cached per device ordinal; thread-safe.
 int device_sm_count();
 int device_max_smem_optin();
+int current_device();
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: one flag bit per device ordinal and kernel
+// instantiation (devices >= 64 set the attribute on every call).
+struct PerDeviceOnce {
+    unsigned long long done = 0;
+};
+bool per_device_test(PerDeviceOnce& once, int dev);
+void per_device_mark(PerDeviceOnce& once, int dev);
+template <typename Kernel>
+inline cudaError_t set_max_dynamic_smem(PerDeviceOnce& once, Kernel kernel, int bytes) {
+    const int dev = current_device();
+    if (per_device_test(once, dev)) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) per_device_mark(once, dev);
+    return e;
+}
 
 #define MSTAR_CUDA_OK(expr)                         \
     do {                                            \

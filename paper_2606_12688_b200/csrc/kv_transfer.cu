@@ -10,9 +10,11 @@
 
 namespace mstar {
 
+// Coherent streaming load (not the read-only .nc path): mstar_kv_copy_pages may read and write the same pool in one
+// launch, and .nc is only defined for data no thread of the grid writes.
 __device__ __forceinline__ int4 ldg_stream16(const void* p) {
     int4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0, %1, %2, %3}, [%4];"
+    asm volatile("ld.global.L1::no_allocate.v4.s32 {%0, %1, %2, %3}, [%4];"
                  : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
                  : "l"(p));
     return r;

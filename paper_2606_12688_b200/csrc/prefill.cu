@@ -278,11 +278,8 @@ static int launch_prefill(const PoolMaps& maps, PrefillParams& p, cudaStream_t s
     if (nstages < 2) return MSTAR_ERR_UNSUPPORTED;
     p.nstages = nstages;
     auto kern = prefill_mma_kernel<D, PAGE>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        MSTAR_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-        attr_set = true;
-    }
+    static PerDeviceOnce attr_once;  // per instantiation
+    MSTAR_CUDA_OK(set_max_dynamic_smem(attr_once, kern, max_smem));
     const int64_t grid = (int64_t)p.n_qblocks * p.S * p.Hkv * p.head_groups;
     if (grid > 0x7fffffffLL) return MSTAR_ERR_UNSUPPORTED;
     kern<<<(unsigned)grid, 32 * (p.nwc + 1), SM::bytes(nstages), stream>>>(maps.k, maps.v, p);

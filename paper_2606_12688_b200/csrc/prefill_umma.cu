@@ -42,10 +42,6 @@ constexpr int kPuMmaWarp = 9;
 constexpr int kPuHT = 128 * 128;  // bytes of a half tile: 128 rows x 64 bf16, 128-B swizzled
 constexpr int kPuSplit = 96;      // keys of a stage in the first P hand-off (the second carries the rest)
 constexpr float kPuTau = 8.0f;    // lazy-rescale threshold, log2 units
-#ifndef MSTAR_PU_EMU
-#define MSTAR_PU_EMU 0
-#endif
-constexpr int kPuEmu = MSTAR_PU_EMU;  // of every 4 score pairs, this many take 2^x on the FMA pipe, the rest on the SFU
 constexpr int kPlanBuckets = 1024;
 constexpr int kPlanHeaderInts = 8;  // [0] work counter  [1] CTAs done  [2] number of units
 
@@ -74,37 +70,6 @@ struct PrefillUmmaParams {
     int32_t causal;
 };
 
-#ifdef MSTAR_PU_TRACE
-// Debug build only (-DMSTAR_PU_TRACE): CTA 0 records (clock, event) words per role.
-constexpr int kTraceCap = 2048;
-__device__ unsigned int g_pu_trace[4][kTraceCap];
-__device__ int g_pu_trace_n[4];
-// per CTA: globaltimer at entry, at the first unit, at exit; units and KV stages processed
-__device__ unsigned long long g_pu_cta[160][5];
-__device__ __forceinline__ unsigned long long pu_gtime() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-    return t;
-}
-#define PU_CTA(i, v) do { if ((threadIdx.x & 31) == 0 && blockIdx.x < 160) g_pu_cta[blockIdx.x][i] = (v); } while (0)
-#define PU_TRACE(role, evt)                                                                                 \
-    do {                                                                                                    \
-        if (pu_trace_on && pu_trace_n < kTraceCap)                                                          \
-            g_pu_trace[role][pu_trace_n++] = ((unsigned)clock() << 6) | (unsigned)(evt);                    \
-    } while (0)
-#define PU_TRACE_DECL   \
-    int pu_trace_n = 0; \
-    const bool pu_trace_on = blockIdx.x == 0 && (threadIdx.x & 31) == 0;
-#define PU_TRACE_FLUSH(role)                            \
-    do {                                                \
-        if (pu_trace_on) g_pu_trace_n[role] = pu_trace_n; \
-    } while (0)
-#else
-#define PU_CTA(i, v)
-#define PU_TRACE(role, evt)
-#define PU_TRACE_DECL
-#define PU_TRACE_FLUSH(role)
-#endif
 
 // ------------------------------------------------------------------------------------------------ plan
 __global__ void __launch_bounds__(kPlanBuckets)
@@ -199,43 +164,6 @@ __device__ __forceinline__ void fadd2(float& d0, float& d1, float a0, float a1, 
         : "=f"(d0), "=f"(d1)
         : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
 }
-// 2^x for a pair of arguments on the FMA / ALU pipes instead of the SFU (the SFU pipe, 16 ex2 per clock per SM,
-// costs as many cycles per score as the two MMAs around it): x = j + f with j = round(x), f in [-0.5, 0.5];
-// 2^f by a degree-3 minimax polynomial (relative error 7.5e-5, far below the bf16 rounding of P), 2^j by adding
-// j to the exponent field.  j is read from the low mantissa bits of x + 1.5 * 2^23.  x <= ~9 by construction
-// (running max, lazy rescale); clamped below at -126 (exponent field cannot wrap).
-__device__ __forceinline__ void exp2_poly2(float& p0, float& p1, float x0, float x1) {
-    x0 = fmaxf(x0, -126.f);
-    x1 = fmaxf(x1, -126.f);
-    uint32_t u0, u1;
-    asm("{\n\t.reg .b64 x, t, j, f, q, mg, nmg, mone, c3, c2, c1, c0;\n\t"
-        ".reg .b32 t0, t1, q0, q1;\n\t"
-        "mov.b64 x, {%2, %3};\n\t"
-        "mov.b64 mg, {%4, %4};\n\t"
-        "mov.b64 nmg, {%5, %5};\n\t"
-        "mov.b64 mone, {%6, %6};\n\t"
-        "mov.b64 c3, {%7, %7};\n\t"
-        "mov.b64 c2, {%8, %8};\n\t"
-        "mov.b64 c1, {%9, %9};\n\t"
-        "mov.b64 c0, {%10, %10};\n\t"
-        "add.rn.f32x2 t, x, mg;\n\t"
-        "add.rn.f32x2 j, t, nmg;\n\t"
-        "fma.rn.f32x2 f, j, mone, x;\n\t"
-        "fma.rn.f32x2 q, c3, f, c2;\n\t"
-        "fma.rn.f32x2 q, q, f, c1;\n\t"
-        "fma.rn.f32x2 q, q, f, c0;\n\t"
-        "mov.b64 {t0, t1}, t;\n\t"
-        "mov.b64 {q0, q1}, q;\n\t"
-        "shl.b32 t0, t0, 23;\n\t"
-        "shl.b32 t1, t1, 23;\n\t"
-        "add.u32 %0, q0, t0;\n\t"
-        "add.u32 %1, q1, t1;\n\t}"
-        : "=r"(u0), "=r"(u1)
-        : "f"(x0), "f"(x1), "f"(12582912.f), "f"(-12582912.f), "f"(-1.f), "f"(0.0551716648042202f),
-          "f"(0.2426111251115799f), "f"(0.6932609677314758f), "f"(0.9999280571937561f));
-    p0 = __uint_as_float(u0);
-    p1 = __uint_as_float(u1);
-}
 __device__ __forceinline__ float fmax3(float a, float b, float c) {
     float d;
     asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
@@ -266,7 +194,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
     auto bar = [&](int i) { return bars + 8u * i; };
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    PU_TRACE_DECL
     if (threadIdx.x == 0) {
         for (int i = 0; i < 2; ++i) {
             mbar_init(bar(B_QFULL0 + i), 1);
@@ -419,10 +346,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             const uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
             const uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
             uint32_t qph[2] = {0, 0}, kph = 0, vph = 0, pph[2] = {0, 0}, oeph = 0, uph = 0;
-#ifdef MSTAR_PU_TRACE
-            unsigned long long cta_units = 0, cta_stages = 0;
-            PU_CTA(0, pu_gtime());
-#endif
             int ks = 0, vs = 0, uslot = 0;
             // Descriptors differ only in the 14-bit start-address field (bytes >> 4) of their low word: the bases are
             // built once, the per-instruction offsets are compile-time constants.
@@ -466,12 +389,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 if (uslot == 0) uph ^= 1;
                 if (x.T == 0) break;
                 const int T = x.T;
-                PU_TRACE(1, 1);
-#ifdef MSTAR_PU_TRACE
-                if (cta_units == 0) PU_CTA(1, pu_gtime());
-                ++cta_units;
-                cta_stages += T;
-#endif
                 mbar_wait(bar(B_KFULL0 + ks), kph);
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
@@ -485,9 +402,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 ks ^= 1;
                 if (ks == 0) kph ^= 1;
                 for (int j = 0; j < T; ++j) {
-                    PU_TRACE(1, 46);
                     mbar_wait(bar(B_VFULL0 + vs), vph);
-                    PU_TRACE(1, 17);
                     if (j == T - 1) {
                         // rows of the last V stage that hold no visible token (not loaded, or NaN poison) -> 0,
                         // so that p = 0 there cannot produce 0 * NaN inside the MMA
@@ -505,30 +420,21 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
 #pragma unroll
                     for (int t = 0; t < 2; ++t) {
                         if (j == 0) mbar_wait(bar(B_OEMPTY0 + t), oeph ^ 1);
-                        PU_TRACE(1, 10 + t);
                         mbar_wait(bar(B_PFULL00 + 2 * t), pph[t]);
-                        PU_TRACE(1, 12 + t);
                         tc_fence_after();
                         issue_pv(t, vs, j > 0, false);
-                        PU_TRACE(1, 40 + t);
                         mbar_wait(bar(B_PFULL00 + 2 * t + 1), pph[t]);
-                        PU_TRACE(1, 14 + t);
                         pph[t] ^= 1;
                         tc_fence_after();
                         issue_pv(t, vs, true, true);
-                        PU_TRACE(1, 42 + t);
                         commit_if(t == 1, B_VEMPTY0 + vs);
                         commit_if(j == T - 1, B_OFULL0 + t);
-                        PU_TRACE(1, 44 + t);
                         if (j + 1 < T) {
                             if (t == 0) {
-                                PU_TRACE(1, 47);
                                 mbar_wait(bar(B_KFULL0 + ks), kph);
                                 tc_fence_after();
-                                PU_TRACE(1, 16);
                             }
                             issue_qk(t, ks);
-                            PU_TRACE(1, 18 + t);
                             commit_if(j + 1 == T - 1, B_QEMPTY0 + t);
                             commit_if(t == 1, B_KEMPTY0 + ks);
                         }
@@ -542,11 +448,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 }
                 oeph ^= 1;
             }
-#ifdef MSTAR_PU_TRACE
-            PU_CTA(2, pu_gtime());
-            PU_CTA(3, cta_units);
-            PU_CTA(4, cta_stages);
-#endif
         }
     } else {
         // =============================== SOFTMAX / EPILOGUE WARPGROUPS ===============================
@@ -575,9 +476,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             float m_ref = -INFINITY, l = 0.f;
             for (int j = 0; j < x.T; ++j) {
                 const int j0 = j * kPuTok;
-                if ((warp & 3) == 0) PU_TRACE(2 + t, 20);
                 mbar_wait(bar(B_SFULL0 + t), sph);
-                if ((warp & 3) == 0) PU_TRACE(2 + t, 21);
                 sph ^= 1;
                 tc_fence_after();
                 uint32_t r[128];
@@ -592,7 +491,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     tmem_ld_32x32b_x32(s_addr + 96, r3);
                     tmem_wait_ld();
                 }
-                if ((warp & 3) == 0) PU_TRACE(2 + t, 22);
                 // ---- mask (diagonal / last stages only; warp-uniform branch)
                 if (__any_sync(0xffffffffu, j0 + kPuTok - 1 > lim)) {
                     const int rel = lim - j0;  // columns i > rel are invisible to this row
@@ -640,7 +538,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                         tmem_wait_st();
                     }
                 }
-                if ((warp & 3) == 0) PU_TRACE(2 + t, 23);
                 // ---- p = 2^(s*c - m_ref*c), P -> bf16 -> TMEM (over the columns of S), handed over in two parts:
                 // the first kPuSplit keys, then the rest, so that little P V work is left after the last hand-off
                 const float nmc = -m_ref * c;
@@ -650,13 +547,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     for (int i = 0; i < kPuSplit; i += 2) {
                         float x0, x1;
                         ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), c, nmc);
-                        float p0, p1;
-                        if (((i >> 1) & 3) < kPuEmu) {
-                            exp2_poly2(p0, p1, x0, x1);
-                        } else {
-                            p0 = fast_exp2(x0);
-                            p1 = fast_exp2(x1);
-                        }
+                        const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
                         r[i] = __float_as_uint(p0);
                         r[i + 1] = __float_as_uint(p1);
                         pk[i >> 1] = pack_bf16x2(p0, p1);
@@ -667,7 +558,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_PFULL00 + 2 * t));
-                    if ((warp & 3) == 0) PU_TRACE(2 + t, 24);
                 }
                 {
                     uint32_t pk[(128 - kPuSplit) / 2];
@@ -675,13 +565,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     for (int i = kPuSplit; i < 128; i += 2) {
                         float x0, x1;
                         ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), c, nmc);
-                        float p0, p1;
-                        if (((i >> 1) & 3) < kPuEmu) {
-                            exp2_poly2(p0, p1, x0, x1);
-                        } else {
-                            p0 = fast_exp2(x0);
-                            p1 = fast_exp2(x1);
-                        }
+                        const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
                         r[i] = __float_as_uint(p0);
                         r[i + 1] = __float_as_uint(p1);
                         pk[(i - kPuSplit) >> 1] = pack_bf16x2(p0, p1);
@@ -691,7 +575,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_PFULL00 + 2 * t + 1));
-                    if ((warp & 3) == 0) PU_TRACE(2 + t, 25);
                 }
                 // ---- row sum, after the hand-off (packed adds, four chains)
                 float s0 = __uint_as_float(r[0]), s1 = __uint_as_float(r[1]);
@@ -704,7 +587,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 l += (s0 + s1) + (s2 + s3);
             }
             // ---- epilogue: O / l -> out
-            if ((warp & 3) == 0) PU_TRACE(2 + t, 30);
             mbar_wait(bar(B_OFULL0 + t), oph);
             oph ^= 1;
             tc_fence_after();
@@ -726,7 +608,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_OEMPTY0 + t));
-            if ((warp & 3) == 0) PU_TRACE(2 + t, 31);
             // Full tiles of bf16 output leave through shared memory and one TMA store per 64-column half (the
             // box of the Q load, so rows land at (token, head)); per-thread row stores would be 32 scattered
             // 16-byte writes per instruction.  Ragged tail tiles and the fp32 diagnostic output go direct.
@@ -784,9 +665,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
         }
     }
     if (warp < 8 && (warp & 3) == 0 && lane == 0) bulk_wait_group0();  // output stores issued by this thread
-    if (warp == kPuMmaWarp) PU_TRACE_FLUSH(1);
-    if (warp == 0) PU_TRACE_FLUSH(2);
-    if (warp == 4) PU_TRACE_FLUSH(3);
     tc_fence_before();
     __syncthreads();
     if (warp == kPuMmaWarp) tmem_dealloc(tmem, 512);
@@ -869,12 +747,9 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
     if (grid < 1) grid = 1;
     auto k16 = prefill_umma_kernel<16>;
     auto k32 = prefill_umma_kernel<32>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        MSTAR_CUDA_OK(cudaFuncSetAttribute(k16, cudaFuncAttributeMaxDynamicSharedMemorySize, kPuSmemBytes));
-        MSTAR_CUDA_OK(cudaFuncSetAttribute(k32, cudaFuncAttributeMaxDynamicSharedMemorySize, kPuSmemBytes));
-        attr_set = true;
-    }
+    static PerDeviceOnce once16, once32;
+    MSTAR_CUDA_OK(set_max_dynamic_smem(once16, k16, kPuSmemBytes));
+    MSTAR_CUDA_OK(set_max_dynamic_smem(once32, k32, kPuSmemBytes));
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3(kPuThreads);
@@ -893,18 +768,3 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
 
 }  // namespace mstar
 
-#ifdef MSTAR_PU_TRACE
-extern "C" int mstar_debug_pu_trace(unsigned int* host_out, int* host_n) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(host_out, mstar::g_pu_trace, sizeof(unsigned int) * 4 * mstar::kTraceCap);
-    cudaMemcpyFromSymbol(host_n, mstar::g_pu_trace_n, sizeof(int) * 4);
-    int z[4] = {0, 0, 0, 0};
-    cudaMemcpyToSymbol(mstar::g_pu_trace_n, z, sizeof(z));
-    return mstar::kTraceCap;
-}
-extern "C" int mstar_debug_pu_cta(unsigned long long* host_out) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(host_out, mstar::g_pu_cta, sizeof(unsigned long long) * 160 * 5);
-    return 160;
-}
-#endif
