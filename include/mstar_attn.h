@@ -51,7 +51,9 @@ typedef enum {
 #define MSTAR_FLAG_OUT_F32 1u /* `out` is fp32 instead of bf16 (diagnostic: separates kernel error from
                                  output rounding).  Unknown bits => MSTAR_ERR_INVALID_ARG. */
 #define MSTAR_FLAG_PREFILL_MMA_SYNC 2u /* prefill only, diagnostic: use the warp-level mma.sync kernel instead
-                                          of the tcgen05/TMEM kernel (head_dim 64 always uses it). */
+                                          of the tcgen05/TMEM kernel.  head_dim 64 always takes this kernel: it is
+                                          a correctness path (about a fifth of the tcgen05 kernel's rate), no
+                                          BASELINE config prefills at head_dim 64. */
 
 #define MSTAR_FLAG_PREFILL_REUSE_PLAN 4u /* prefill only: `workspace` still holds the plan a previous call built
                                           for the SAME cu_seqlens_q, seq_lens, head geometry and causal flag (the
@@ -123,11 +125,14 @@ int mstar_kv_gather(void* k_out, void* v_out, const mstar_kv_pool* pool, const i
  *                  [i*c, (i+1)*c) with c = ceil(max_seq_len/P) rounded up to a multiple of 64; partitions
  *                  past a sequence's end are empty; 1 = no combine pass.  0 = balanced: the 64-token
  *                  tiles of all (sequence, kv head) streams are laid end to end and every CTA takes an
- *                  equal contiguous range, so ragged batches finish together; a stream cut by range
- *                  boundaries is merged by the combine pass (the cut points depend on seq_lens and
- *                  the SM count only, never on page ids).
+ *                  equal contiguous range, so ragged batches finish together; a stream that lies inside
+ *                  one range is finished by its CTA, a stream cut by range boundaries (at most one per
+ *                  CTA) is merged by the combine pass (the cut points depend on seq_lens and the SM
+ *                  count only, never on page ids).
  *   workspace      device, >= mstar_paged_attn_decode_workspace_bytes(...) bytes, 16-B aligned
- * Requires Hq % Hkv == 0 and Hq/Hkv <= 16.
+ *   scale          must be positive and finite (MSTAR_ERR_INVALID_ARG otherwise)
+ * Requires Hq % Hkv == 0 and Hq/Hkv <= 16 (MSTAR_ERR_UNSUPPORTED otherwise), and num_seqs <= 16384
+ * (MSTAR_ERR_UNSUPPORTED: the per-sequence work-list prefix sums live in shared memory).
  */
 size_t mstar_paged_attn_decode_workspace_bytes(int32_t num_seqs, int32_t num_q_heads, int32_t head_dim,
                                                int32_t max_partitions);
@@ -203,6 +208,7 @@ int mstar_merge_attn_states(void* out, float* lse_out, const float* out_a, const
  *   cu_seqlens_q   device, [S+1] int32, cu_seqlens_q[0] = 0, cu_seqlens_q[S] = total_q
  *   seq_lens       device, [S] int32, total KV length INCLUDING the new tokens (>= n_s)
  *   max_q_len, max_seq_len   host upper bounds on n_s and seq_lens
+ *   scale          must be positive and finite (MSTAR_ERR_INVALID_ARG otherwise)
  *   workspace      device, >= mstar_paged_attn_prefill_workspace_bytes(...) bytes, 16-B aligned.  Holds the
  *                  device-built attention plan (PAPER.md:136 builds its plan on the CPU): work units sorted
  *                  heaviest first plus the work counter.  Contents need no initialisation.

@@ -21,6 +21,8 @@ from .binding import (  # noqa: F401
     KVPoolFp8,
     LIB_PATH,
     MSTAR_FLAG_OUT_F32,
+    MSTAR_FLAG_PREFILL_MMA_SYNC,
+    MSTAR_FLAG_PREFILL_REUSE_PLAN,
     MstarError,
     build_slot_mapping,
     decode_auto_partitions,

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_PKG_DIR, "libmstar_attn.so")
 MSTAR_OK = 0
 MSTAR_FLAG_OUT_F32 = 1
 MSTAR_FLAG_PREFILL_MMA_SYNC = 2
+MSTAR_FLAG_PREFILL_REUSE_PLAN = 4
 
 EXPORTS = (
     "mstar_kv_append",
@@ -335,14 +336,19 @@ def prefill_workspace_bytes(num_seqs: int, total_q: int, num_q_heads: int, head_
 def paged_attn_prefill(out: torch.Tensor, q: torch.Tensor, cu_seqlens_q: torch.Tensor, pool: KVPool,
                        block_table: torch.Tensor, seq_lens: torch.Tensor, max_q_len: int, max_seq_len: int,
                        scale: float, causal: bool = True, workspace: Optional[torch.Tensor] = None,
-                       lse_out: Optional[torch.Tensor] = None, mma_sync: bool = False) -> None:
+                       lse_out: Optional[torch.Tensor] = None, mma_sync: bool = False,
+                       reuse_plan: bool = False) -> None:
     """mstar_paged_attn_prefill.  q/out [T,Hq,D]; K/V of the new tokens must already be in the pool.
-    ``mma_sync=True`` sets MSTAR_FLAG_PREFILL_MMA_SYNC (diagnostic: the warp-level MMA kernel)."""
+    ``mma_sync=True`` sets MSTAR_FLAG_PREFILL_MMA_SYNC (diagnostic: the warp-level MMA kernel);
+    ``reuse_plan=True`` sets MSTAR_FLAG_PREFILL_REUSE_PLAN (``workspace`` holds the plan of a previous call on the
+    same batch geometry, e.g. the previous layer)."""
     _want(q, torch.bfloat16, "q"); _want(cu_seqlens_q, torch.int32, "cu_seqlens_q")
     _want(block_table, torch.int32, "block_table"); _want(seq_lens, torch.int32, "seq_lens")
     T, Hq, D = (int(x) for x in q.shape)
     S = int(cu_seqlens_q.shape[0]) - 1
     flags = MSTAR_FLAG_PREFILL_MMA_SYNC if mma_sync else 0
+    if reuse_plan:
+        flags |= MSTAR_FLAG_PREFILL_REUSE_PLAN
     if out.dtype == torch.float32:
         flags |= MSTAR_FLAG_OUT_F32
     elif out.dtype != torch.bfloat16:

@@ -29,6 +29,7 @@ static int decode_pick_warps(bool fp8, int G, int max_seq_len) {
     return fp8 ? ((G <= 8 && max_seq_len > 8192) ? 12 : 8) : 4;
 }
 constexpr int kMaxStages = 16;
+constexpr int kMaxDecodeGrid = 1024;  // split-K CTAs (one per SM); sizes the cut-record area of the workspace
 
 struct DecodeParams {
     const uint16_t* q;
@@ -48,12 +49,14 @@ struct DecodeParams {
     int32_t direct;  // nparts == 1: write the final output, no combine pass
     int32_t nstages;
     // balanced mode (num_partitions = 0): the (sequence, kv head) streams are laid end to end in 64-token tiles and
-    // every CTA takes an equal, contiguous range of them; a stream cut by CTA boundaries yields one partial per
-    // piece.  chunk == decode_tok then, per_min bounds the pieces of one stream by nparts, and piece_count
-    // [S*Hkv] tells the combine pass how many partials each stream has.
+    // every CTA takes an equal, contiguous range of them.  A stream that lies inside one range is finished by its CTA
+    // (final output, no partial); a stream cut by range boundaries yields one partial per piece, and the CTA that
+    // holds its first piece records it in cut[] for the combine pass -- at most one record per CTA, since only the
+    // last stream of a range can continue into the next.  chunk == decode_tok then; per_min bounds the pieces of
+    // one stream by nparts.
     int32_t balanced;
     int32_t per_min;
-    int32_t* piece_count;
+    int4* cut;  // [gridDim.x] per CTA: {s, kvh, pieces, 0} of the cut stream that BEGINS in its range, s = -1 if none
     // quantised pool (FP8 instantiations): value = e4m3(code) * scale[page][kv head]
     const float* k_scale;
     const float* v_scale;
@@ -61,6 +64,7 @@ struct DecodeParams {
 
 struct ItemInfo {
     int32_t s, kvh, part, tok0, ntok;
+    int32_t whole;  // the item is the sequence's whole stream: the consumers write the final output
 };
 
 template <int D, int GH, int EB, int NWARPS>  // EB = bytes per pool element (2 = bf16, 1 = e4m3)
@@ -73,7 +77,7 @@ struct DecodeSmem {
     // fixed part after the ring: Q slots, merge buffer, barriers, item info
     static constexpr int kFixed = 2 * kQBytes + kMergeBytes + (2 * kMaxStages + 4) * 8 + 2 * 32 + kScaleBytes;
     static size_t bytes(int nstages, int S) {
-        return 1024 + (size_t)nstages * kStageBytes + kFixed + (size_t)(S + 1) * 4 + 16;
+        return 1024 + (size_t)nstages * kStageBytes + kFixed + (size_t)(2 * S + 1) * 4 + 16;
     }
 };
 
@@ -151,7 +155,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
     const uint32_t bars = smem_u32(bars_g);
     ItemInfo* info = reinterpret_cast<ItemInfo*>(bars_g + 2 * kMaxStages + 4);
     float* sc_ring = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(info) + 2 * 32);  // FP8 only
-    int32_t* cum = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(info) + 2 * 32 + SM::kScaleBytes);
+    int32_t* cum = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(info) + 2 * 32 + SM::kScaleBytes);  // [S + 1]
+    int32_t* lens = cum + p.S + 1;                                                                              // [S]
     auto full_bar = [&](int st) { return bars + 8u * st; };
     auto empty_bar = [&](int st) { return bars + 8u * (kMaxStages + st); };
     auto qfull_bar = [&](int qs) { return bars + 8u * (2 * kMaxStages + qs); };
@@ -195,7 +200,9 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         int carry = 0;
         for (int s0 = 0; s0 < p.S; s0 += 32) {
             const int s = s0 + lane;
-            const int n = (s < p.S) ? (p.seq_lens[s] + p.chunk - 1) / p.chunk : 0;
+            const int len = (s < p.S) ? max(__ldg(p.seq_lens + s), 0) : 0;
+            if (s < p.S) lens[s] = len;
+            const int n = (len + p.chunk - 1) / p.chunk;
             int incl = n;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -217,11 +224,11 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
 
         int st = 0, ph = 0, qs = 0, qph = 0;
         // hand one work item to the consumers and stream its K/V tiles into the ring
-        auto emit_item = [&](int s, int kvh, int part, int tok0, int ntok) {
+        auto emit_item = [&](int s, int kvh, int part, int tok0, int ntok, int whole) {
             const int ntiles = (ntok + TOK - 1) / TOK;
             if (!op_isv) mbar_wait(qempty_bar(qs), qph ^ 1);
             if (lane == 0 && !op_isv) {
-                info[qs] = ItemInfo{s, kvh, part, tok0, ntok};
+                info[qs] = ItemInfo{s, kvh, part, tok0, ntok, whole};
                 mbar_arrive_expect_tx(qfull_bar(qs), (uint32_t)(p.G * D * 2));
                 bulk_load_1d(qbuf + qs * SM::kQBytes, p.q + ((size_t)s * p.Hq + (size_t)kvh * p.G) * D,
                              (uint32_t)(p.G * D * 2), qfull_bar(qs));
@@ -266,6 +273,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
             if (per < p.per_min) per = p.per_min;
             const int64_t fa = (int64_t)blockIdx.x * per;
             const int64_t fb = (fa + per < N) ? fa + per : N;
+            bool cut_here = false;  // a stream begins in this range and continues past its end
             if (fa < N) {
                 int lo = 0, hi = p.S;  // cum[lo]*Hkv <= fa < cum[hi]*Hkv
                 while (hi - lo > 1) {
@@ -282,11 +290,15 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     const int64_t fs = F0 + (int64_t)kvh * nt;  // flat start of this stream
                     const int ntl = (int)(((int64_t)(nt - tile) < fb - f) ? (nt - tile) : (fb - f));
                     const int piece = (int)((int64_t)blockIdx.x - fs / per);
-                    if (tile == 0 && lane == 0 && !op_isv)
-                        p.piece_count[(size_t)s * p.Hkv + kvh] = (int)((fs + nt - 1) / per - fs / per) + 1;
-                    const int L = p.seq_lens[s];
+                    const int whole = (tile == 0 && ntl == nt) ? 1 : 0;
+                    if (tile == 0 && !whole) {
+                        cut_here = true;
+                        if (lane == 0 && !op_isv)
+                            p.cut[blockIdx.x] = make_int4(s, kvh, (int)((fs + nt - 1) / per - fs / per) + 1, 0);
+                    }
+                    const int L = lens[s];
                     const int tok0 = tile * TOK;
-                    emit_item(s, kvh, piece, tok0, min(L - tok0, ntl * TOK));
+                    emit_item(s, kvh, piece, tok0, min(L - tok0, ntl * TOK), whole);
                     f += ntl;
                     if (tile + ntl == nt && kvh == p.Hkv - 1) {
                         ++s;
@@ -294,6 +306,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     }
                 }
             }
+            if (!cut_here && lane == 0 && !op_isv) p.cut[blockIdx.x] = make_int4(-1, 0, 0, 0);
         } else {
             for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
                 const int pi = item / p.Hkv, kvh = item - pi * p.Hkv;
@@ -303,9 +316,9 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     if (cum[mid] <= pi) lo = mid; else hi = mid;
                 }
                 const int s = lo, part = pi - cum[lo];
-                const int L = p.seq_lens[s];
+                const int L = lens[s];
                 const int tok0 = part * p.chunk;
-                emit_item(s, kvh, part, tok0, min(L - tok0, p.chunk));
+                emit_item(s, kvh, part, tok0, min(L - tok0, p.chunk), (p.direct || L <= p.chunk) ? 1 : 0);
             }
         }
         // sentinel: tell the consumers to stop
@@ -318,9 +331,9 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         // =============================== CONSUMERS ===============================
         const int w = warp;
         const int g = lane >> 2, t4 = lane & 3;
-        if (p.direct) {  // empty sequences get out = 0, lse = -inf (no work item ever touches them)
+        {  // empty sequences get out = 0, lse = -inf (no work item ever touches them, nor does the combine pass)
             for (int s = blockIdx.x * NW + w; s < p.S; s += gridDim.x * NW) {
-                if (p.seq_lens[s] != 0) continue;
+                if (__ldg(p.seq_lens + s) > 0) continue;
                 for (int i = lane; i < p.Hq * D; i += 32) {
                     const size_t idx = (size_t)s * p.Hq * D + i;
                     if (p.out_f32) reinterpret_cast<float*>(p.out)[idx] = 0.f;
@@ -681,7 +694,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     for (int i = 0; i < VEC; ++i) acc[i] += a * src[i];
                 }
                 const size_t row = (size_t)it.s * p.Hq + (size_t)it.kvh * p.G + r;
-                if (p.direct) {
+                if (it.whole) {
                     const float inv = 1.f / lsum;
 #pragma unroll
                     for (int i = 0; i < VEC; ++i) acc[i] *= inv;
@@ -703,62 +716,98 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
 }
 
 // ---------------------------------------------------------------------------------------------
-// step a3: merge the partitions of every (sequence, head) row by log-sum-exp, normalise, round once.
-// One warp per row; lanes own D/32 consecutive output elements.  Partition count per sequence is
-// ceil(seq_len / chunk): the same arithmetic the split-K kernel used.
+// step a3: merge the partials of every (sequence, head) row that has more than one by log-sum-exp, normalise, round
+// once.  One CTA of four warps per row; warp w takes pieces w, w + 4, ... with all of its loads in flight at once
+// (a single round trip to memory for up to 16 pieces), the four warps meet in shared memory.  Rows:
+//   fixed partitions  block = row; pieces = ceil(seq_len / chunk), the arithmetic the split-K kernel used; rows with
+//                     one piece (or none) were finished by the split-K kernel.
+//   balanced          block = (split-K CTA c, head r of the group): the cut record of c names the stream that begins
+//                     in c's range and continues in the next ones, and its piece count; no record, nothing to do.
+// The merge order is the piece order: deterministic.
 template <int D>
 __global__ void __launch_bounds__(128) decode_combine_kernel(const float* __restrict__ part_O,
                                                              const float* __restrict__ part_m,
                                                              const float* __restrict__ part_l,
                                                              const int32_t* __restrict__ seq_lens, int32_t chunk,
-                                                             const int32_t* __restrict__ piece_count, int32_t G,
-                                                             int32_t nparts, int32_t Hq, int32_t n_rows,
-                                                             void* __restrict__ out, float* __restrict__ lse,
-                                                             int32_t out_f32) {
+                                                             const int4* __restrict__ cut, int32_t G,
+                                                             int32_t nparts, int32_t Hq, void* __restrict__ out,
+                                                             float* __restrict__ lse, int32_t out_f32) {
     constexpr int VEC = D / 32;
-    const int lane = threadIdx.x & 31;
-    const int row = blockIdx.x * 4 + (threadIdx.x >> 5);
+    constexpr int PB = 4;  // pieces per warp per batch
+    __shared__ float s_acc[4][D];
+    __shared__ float s_l[4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // programmatic dependent launch: this grid may be resident before the split-K grid has finished; nothing it
-    // reads (partials, piece counts) is valid before this returns
+    // reads (partials, cut records) is valid before this returns
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    if (row >= n_rows) return;
-    const int s = row / Hq;
-    const int L = seq_lens[s];
-    // balanced mode: the split-K kernel recorded the number of pieces of every (sequence, kv head) stream
-    const int np = (L <= 0) ? 0 : piece_count ? piece_count[(size_t)s * (Hq / G) + (row - s * Hq) / G]
-                                              : (L + chunk - 1) / chunk;
+    int64_t row;
+    int np;
+    if (cut) {
+        const int4 rec = cut[blockIdx.x / G];
+        if (rec.x < 0) return;
+        row = (int64_t)rec.x * Hq + (int64_t)rec.y * G + (blockIdx.x % G);
+        np = rec.z;
+    } else {
+        row = blockIdx.x;
+        const int L = seq_lens[row / Hq];
+        np = (L + chunk - 1) / chunk;
+        if (np <= 1) return;
+    }
+    const float* pm = part_m + row * nparts;
+    const float* pl = part_l + row * nparts;
+    const float* po = part_O + row * nparts * D + lane * VEC;
+    float M = -INFINITY;
+    for (int i = lane; i < np; i += 32) M = fmaxf(M, pm[i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
     float acc[VEC];
 #pragma unroll
     for (int i = 0; i < VEC; ++i) acc[i] = 0.f;
-    float lse_v = -INFINITY;
-    if (np > 0) {
-        const float* pm = part_m + (size_t)row * nparts;
-        const float* pl = part_l + (size_t)row * nparts;
-        float M = -INFINITY;
-        for (int i = lane; i < np; i += 32) M = fmaxf(M, pm[i]);
+    float lsum = 0.f;
+    for (int i0 = warp; i0 < np; i0 += 4 * PB) {
+        float v[PB][VEC], mi[PB], li[PB];
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
-        float lsum = 0.f;
-        const float* po = part_O + (size_t)row * nparts * D + lane * VEC;
-#pragma unroll 4
-        for (int i = 0; i < np; ++i) {
-            const float a = fast_exp2(pm[i] - M);
-            lsum += a * pl[i];
-            if constexpr (VEC == 4) {
-                const float4 v = *reinterpret_cast<const float4*>(po + (size_t)i * D);
-                acc[0] += a * v.x; acc[1] += a * v.y; acc[2] += a * v.z; acc[3] += a * v.w;
-            } else {
-                const float2 v = *reinterpret_cast<const float2*>(po + (size_t)i * D);
-                acc[0] += a * v.x; acc[1] += a * v.y;
+        for (int u = 0; u < PB; ++u) {
+            const int i = i0 + 4 * u;
+            mi[u] = -INFINITY;
+            li[u] = 0.f;
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) v[u][e] = 0.f;
+            if (i < np) {
+                mi[u] = pm[i];
+                li[u] = pl[i];
+                if constexpr (VEC == 4) {
+                    const float4 t = *reinterpret_cast<const float4*>(po + (size_t)i * D);
+                    v[u][0] = t.x; v[u][1] = t.y; v[u][2] = t.z; v[u][3] = t.w;
+                } else {
+                    const float2 t = *reinterpret_cast<const float2*>(po + (size_t)i * D);
+                    v[u][0] = t.x; v[u][1] = t.y;
+                }
             }
         }
-        const float inv = 1.f / lsum;
 #pragma unroll
-        for (int i = 0; i < VEC; ++i) acc[i] *= inv;
-        lse_v = (M + log2f(lsum)) * 0.6931471805599453f;
+        for (int u = 0; u < PB; ++u) {
+            const float a = (mi[u] == -INFINITY) ? 0.f : fast_exp2(mi[u] - M);
+            lsum += a * li[u];
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) acc[e] += a * v[u][e];
+        }
     }
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) s_acc[warp][lane * VEC + e] = acc[e];
+    if (lane == 0) s_l[warp] = lsum;
+    __syncthreads();
+    if (warp != 0) return;
+    lsum = (s_l[0] + s_l[1]) + (s_l[2] + s_l[3]);
+#pragma unroll
+    for (int e = 0; e < VEC; ++e)
+        acc[e] = (s_acc[0][lane * VEC + e] + s_acc[1][lane * VEC + e]) +
+                 (s_acc[2][lane * VEC + e] + s_acc[3][lane * VEC + e]);
+    const float inv = 1.f / lsum;
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) acc[e] *= inv;
     store_out_vec(out, out_f32, (size_t)row * D + lane * VEC, acc, VEC);
-    if (lse && lane == 0) lse[row] = lse_v;
+    if (lse && lane == 0) lse[row] = (M + log2f(lsum)) * 0.6931471805599453f;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -806,10 +855,10 @@ static void partition_plan(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t 
 }
 
 template <int D, int PAGE, int GH, bool FP8, int NWARPS>
-static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, cudaStream_t stream) {
+static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, cudaStream_t stream, int* grid_out) {
     using SM = DecodeSmem<D, GH, FP8 ? 1 : 2, NWARPS>;
     const int max_smem = device_max_smem_optin();
-    int nstages = (int)(((int64_t)max_smem - 1024 - SM::kFixed - (int64_t)(p.S + 1) * 4 - 16) / SM::kStageBytes);
+    int nstages = (int)(((int64_t)max_smem - 1024 - SM::kFixed - (int64_t)(2 * p.S + 1) * 4 - 16) / SM::kStageBytes);
     if (nstages > kMaxStages) nstages = kMaxStages;
     if (nstages < 2) return MSTAR_ERR_UNSUPPORTED;
     p.nstages = nstages;
@@ -818,8 +867,10 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
     static PerDeviceOnce attr_once;  // per instantiation
     MSTAR_CUDA_OK(set_max_dynamic_smem(attr_once, kern, max_smem));
     int grid = device_sm_count();
+    if (grid > kMaxDecodeGrid) grid = kMaxDecodeGrid;
     if (grid > max_items) grid = max_items;
     if (grid < 1) grid = 1;
+    *grid_out = grid;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3(decode_threads(NWARPS));
@@ -849,8 +900,8 @@ extern "C" size_t mstar_paged_attn_decode_workspace_bytes(int32_t num_seqs, int3
                                                           int32_t max_partitions) {
     if (num_seqs <= 0 || num_q_heads <= 0 || head_dim <= 0 || max_partitions <= 1) return 256;
     const size_t rows = (size_t)num_seqs * num_q_heads * max_partitions;
-    // partials (O, m, l) + one piece count per (sequence, kv head) stream (bounded by the q heads)
-    return 256 + rows * head_dim * 4 + 2 * rows * 4 + 256 + (size_t)num_seqs * num_q_heads * 4;
+    // partials (O, m, l) + one 16-byte cut record per split-K CTA (balanced mode)
+    return 256 + rows * head_dim * 4 + 2 * rows * 4 + 256 + 16 + (size_t)mstar::kMaxDecodeGrid * 16;
 }
 
 // bf16 pool (k_scale == v_scale == NULL, fp8 false) or quantised pool
@@ -892,7 +943,9 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
         p.part_O = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + 256);
         p.part_m = p.part_O + rows * D;
         p.part_l = p.part_m + rows;
-        p.piece_count = p.balanced ? reinterpret_cast<int32_t*>(p.part_l + rows + 64) : nullptr;
+        p.cut = p.balanced ? reinterpret_cast<int4*>((reinterpret_cast<uintptr_t>(p.part_l + rows + 64) + 15) &
+                                                     ~uintptr_t(15))
+                           : nullptr;
     }
     p.q = reinterpret_cast<const uint16_t*>(q);
     p.block_table = block_table;
@@ -917,10 +970,11 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
     const int max_items = max_items64 > (1 << 30) ? (1 << 30) : (int)max_items64;
     cudaStream_t st = (cudaStream_t)stream;
     const bool g16 = G > 8;
+    int grid = 0;
 #define MSTAR_DECODE_CASE(DD, PP, F8, NWW)                                               \
     if (D == DD && PAGE == PP && fp8 == F8 && nw == NWW)                                 \
-        rc = g16 ? launch_decode<DD, PP, 16, F8, NWW>(maps, p, max_items, st)            \
-                 : launch_decode<DD, PP, 8, F8, NWW>(maps, p, max_items, st);
+        rc = g16 ? launch_decode<DD, PP, 16, F8, NWW>(maps, p, max_items, st, &grid)     \
+                 : launch_decode<DD, PP, 8, F8, NWW>(maps, p, max_items, st, &grid);
     rc = MSTAR_ERR_UNSUPPORTED;
     MSTAR_DECODE_CASE(128, 16, false, 4)
     MSTAR_DECODE_CASE(128, 32, false, 4)
@@ -929,15 +983,17 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
     MSTAR_DECODE_CASE(128, 16, true, 8)
     MSTAR_DECODE_CASE(128, 32, true, 8)
     if (!g16) {  // 12 warps need the 111-register consumer of the G <= 8 form
-        if (D == 128 && PAGE == 16 && fp8 && nw == 12) rc = launch_decode<128, 16, 8, true, 12>(maps, p, max_items, st);
-        if (D == 128 && PAGE == 32 && fp8 && nw == 12) rc = launch_decode<128, 32, 8, true, 12>(maps, p, max_items, st);
+        if (D == 128 && PAGE == 16 && fp8 && nw == 12)
+            rc = launch_decode<128, 16, 8, true, 12>(maps, p, max_items, st, &grid);
+        if (D == 128 && PAGE == 32 && fp8 && nw == 12)
+            rc = launch_decode<128, 32, 8, true, 12>(maps, p, max_items, st, &grid);
     }
 #undef MSTAR_DECODE_CASE
     if (rc != MSTAR_OK) return rc;
 
     if (!p.direct) {
-        const int n_rows = num_seqs * num_q_heads;
-        const int blocks = (n_rows + 3) / 4;
+        // fixed partitions: one block per (sequence, head) row; balanced: one per (split-K CTA, head of the group)
+        const int64_t blocks = p.balanced ? (int64_t)grid * G : (int64_t)num_seqs * num_q_heads;
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3((unsigned)blocks);
         cfg.blockDim = dim3(128);
@@ -951,15 +1007,13 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
         const float* cO = p.part_O;
         const float* cm = p.part_m;
         const float* cl = p.part_l;
-        const int32_t* cpc = p.piece_count;
+        const int4* ccut = p.cut;
         if (D == 128)
-            MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, decode_combine_kernel<128>, cO, cm, cl, seq_lens, p.chunk, cpc,
-                                             (int32_t)G, p.nparts, num_q_heads, (int32_t)n_rows, out, lse_out,
-                                             p.out_f32));
+            MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, decode_combine_kernel<128>, cO, cm, cl, seq_lens, p.chunk, ccut,
+                                             (int32_t)G, p.nparts, num_q_heads, out, lse_out, p.out_f32));
         else
-            MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, decode_combine_kernel<64>, cO, cm, cl, seq_lens, p.chunk, cpc,
-                                             (int32_t)G, p.nparts, num_q_heads, (int32_t)n_rows, out, lse_out,
-                                             p.out_f32));
+            MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, decode_combine_kernel<64>, cO, cm, cl, seq_lens, p.chunk, ccut,
+                                             (int32_t)G, p.nparts, num_q_heads, out, lse_out, p.out_f32));
         MSTAR_CUDA_OK(cudaGetLastError());
         launch_count_add(1);
     }

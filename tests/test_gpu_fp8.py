@@ -33,8 +33,8 @@ def oracle_pool(b, k_scale, v_scale):
     return k8, v8, ks, vs
 
 
-def run_case(b, parts_list=(0,), layout="HND", seed=1):
-    k_scale, v_scale = W.fp8_page_scales(seed, b.num_pages, b.num_kv_heads)
+def run_case(b, parts_list=(0,), layout="HND", seed=1, scale_range=(0.006, 0.02)):
+    k_scale, v_scale = W.fp8_page_scales(seed, b.num_pages, b.num_kv_heads, lo=scale_range[0], hi=scale_range[1])
     db = DeviceBatchFp8(b, k_scale, v_scale, layout=layout)
     db.quantise_store()
     db.append()

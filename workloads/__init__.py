@@ -27,3 +27,4 @@ from .generators import (  # noqa: F401
     fp8_page_scales,
     CONFIG_SEED_BASE,
 )
+from .adversarial import KINDS as ADVERSARIAL_KINDS, logical_kv, make_adversarial, overwrite_k, overwrite_v  # noqa: F401
