@@ -127,6 +127,43 @@ def test_cascade_identity_stacked_prefix_plus_suffix_merge():
             assert np.abs(out - full[s, h]).max() < 1e-12 and abs(lse - full_lse[s, h]) < 1e-12
 
 
+def test_cascade_identity_three_branches_ragged_shared_lens_split_pieces():
+    """The work split of mstar_paged_attn_decode_cascade in fp64: per request a prefix state over its shared_lens[r]
+    tokens (ragged over requests, 0 allowed; branches grouped two + one as the 16 MMA rows allow at G = 7), cut in
+    pieces, plus per-branch suffix states cut in pieces, all merged by COMBINE, equals the plain decode over the
+    whole sequence, for three CFG labels."""
+    B, p = 3, 16
+    shared_r = [48, 0, 112]
+    sfx = [[5, 40, 1], [33, 17, 64], [1, 90, 16]]   # a suffix of one token is only the step's new token
+    lens = [shared_r[r] + sfx[r][b] for r in range(3) for b in range(B)]
+    share = [-1 if b == 0 else r * B for r in range(3) for b in range(B)]
+    shared = [shared_r[r] for r in range(3) for b in range(B)]
+    rng = np.random.default_rng(78)
+    b = W.make_batch(rng, "cfg3", lens, [1] * 9, 14, 2, 64, p, 96, share_with=share, shared_tokens=shared)
+    k, v = compact_pool_after_append(b)
+    q = decode_q(b)
+    full, full_lse = oracle.paged_decode(q, k, v, b.compact_block_table, b.seq_lens, b.scale)
+    S, Hq = 9, 14
+    chunk = 32   # pieces of 32 tokens
+    for s in range(S):
+        r = s // B
+        for h in range(Hq):
+            ms, ls, os_ = [], [], []
+            # prefix pieces: computed once per request from any branch's block-table row, with this row's query
+            for a in range(0, shared_r[r], chunk):
+                m, l, o = oracle.decode_partition(q[s:s + 1], k, v, b.compact_block_table[r * B:r * B + 1],
+                                                  np.array([shared_r[r]], np.int32), b.scale, 0, h, a,
+                                                  min(a + chunk, shared_r[r]))
+                ms.append(m); ls.append(l); os_.append(o)
+            for a in range(shared_r[r], int(b.seq_lens[s]), chunk):
+                m, l, o = oracle.decode_partition(q[s:s + 1], k, v, b.compact_block_table[s:s + 1],
+                                                  b.seq_lens[s:s + 1], b.scale, 0, h, a,
+                                                  min(a + chunk, int(b.seq_lens[s])))
+                ms.append(m); ls.append(l); os_.append(o)
+            out, lse = oracle.lse_combine(np.array(ms), np.array(ls), np.stack(os_))
+            assert np.abs(out - full[s, h]).max() < 1e-12 and abs(lse - full_lse[s, h]) < 1e-12
+
+
 def test_append_negative_slot_skipped():
     b = small_batch(2, [20, 9], q_lens=[3, 2], Hq=2, Hkv=1, D=64)
     k0, v0 = b.full_pool()

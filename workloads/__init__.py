@@ -24,6 +24,7 @@ from .generators import (  # noqa: F401
     config4_talker,
     config5_long_context,
     flow_step_bagel,
+    cfg_cascade_decode,
     fp8_page_scales,
     CONFIG_SEED_BASE,
 )

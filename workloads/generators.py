@@ -129,14 +129,15 @@ def make_batch(
     page_size: int,
     num_pages: int,
     share_with: Optional[Sequence[int]] = None,
-    shared_tokens: int = 0,
+    shared_tokens=0,
     table_width: Optional[int] = None,
 ) -> PagedBatch:
     """Draw one batch.  Draw order: page permutation, Q, K store, V store.
 
     ``share_with[s] = r`` (r < s) makes sequence s reuse the physical pages of the
     first ``shared_tokens`` tokens of sequence r (``shared_tokens`` must be a
-    multiple of ``page_size`` and <= both lengths minus their new tokens).
+    multiple of ``page_size`` and <= both lengths minus their new tokens; an int for
+    the whole batch or one value per sequence).
     """
     S = len(seq_lens)
     p, D, Hq, Hkv = page_size, head_dim, num_q_heads, num_kv_heads
@@ -150,8 +151,8 @@ def make_batch(
 
     if share_with is None:
         share_with = [-1] * S
-    shared_pages = shared_tokens // p
-    assert shared_tokens % p == 0
+    shared_arr = np.broadcast_to(np.asarray(shared_tokens, dtype=np.int64), (S,)) if S else np.zeros(0, np.int64)
+    assert np.all(shared_arr % p == 0)
 
     perm = rng.permutation(num_pages).astype(np.int64)
     block_table = np.full((S, width), -1, dtype=np.int32)
@@ -162,10 +163,11 @@ def make_batch(
         r = share_with[s]
         first_private = 0
         if r is not None and r >= 0:
-            assert r < s and shared_tokens <= int(seq_lens[s]) - int(q_lens[s])
-            assert shared_tokens <= int(seq_lens[r]) - int(q_lens[r])
-            block_table[s, :shared_pages] = block_table[r, :shared_pages]
-            first_private = shared_pages
+            sh = int(shared_arr[s])
+            assert r < s and sh <= int(seq_lens[s]) - int(q_lens[s])
+            assert sh <= int(seq_lens[r]) - int(q_lens[r])
+            block_table[s, :sh // p] = block_table[r, :sh // p]
+            first_private = sh // p
         m = n - first_private
         assert cursor + m <= num_pages, "pool too small"
         ids = perm[cursor:cursor + m]
@@ -310,6 +312,30 @@ def flow_step_bagel(num_requests: int = 4, n_latent: int = 4096, n_labels: int =
         share = [-1] * len(lens)
     return make_batch(rng, "flow_step_bagel", lens, [n_latent] * len(lens), 28, 4, 128, 16,
                       2 * _pages(lens, 16), share_with=share, shared_tokens=64 if n_labels >= 3 else 0)
+
+
+def cfg_cascade_decode(num_requests: int = 16, n_branches: int = 3, num_q_heads: int = 28, num_kv_heads: int = 4,
+                       page_size: int = 16, ctx_lo: int = 2048, ctx_hi: int = 6144, sfx_lo: int = 16,
+                       sfx_hi: int = 512, seed: int = 71):
+    """SURVEY 8(f) rank 3, a decode step in which sharing dominates ("three labels over a single paged
+    KV pool ... reading page tables in place"; :104-106, the three CFG contexts): ``num_requests`` requests x
+    ``n_branches`` CFG labels, request-major; the labels of a request reference the same physical pages for a
+    context of U{ctx_lo..ctx_hi} tokens rounded down to whole pages (ragged across requests) and each label adds a
+    private suffix of U{sfx_lo..sfx_hi} tokens (the part of the context the label keeps to itself plus what it has
+    generated).  The paper gives no lengths; with the defaults about 90 % of the logical K/V bytes are shared.
+    BAGEL-like geometry of configs[1] (28 q / 4 kv heads, head_dim 128, page 16).  Returns (batch, shared_lens[R])."""
+    rng = np.random.default_rng(CONFIG_SEED_BASE + seed)
+    p = page_size
+    ctx = (rng.integers(ctx_lo, ctx_hi + 1, num_requests) // p) * p
+    lens, share, shared = [], [], []
+    for r in range(num_requests):
+        for b in range(n_branches):
+            lens.append(int(ctx[r]) + int(rng.integers(sfx_lo, sfx_hi + 1)))
+            share.append(-1 if b == 0 else r * n_branches)
+            shared.append(int(ctx[r]))
+    b = make_batch(rng, "cfg_cascade_decode", lens, [1] * len(lens), num_q_heads, num_kv_heads, 128, p,
+                   2 * _pages(lens, p), share_with=share, shared_tokens=shared)
+    return b, ctx.astype(np.int32)
 
 
 def fp8_page_scales(seed: int, num_pages: int, num_kv_heads: int, lo: float = 0.006, hi: float = 0.02):
