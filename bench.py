@@ -298,19 +298,41 @@ def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15
         "frac_of_measured_hbm": tot / (ms_both * 1e-3) / 1e9 / hbm_peak,
         "decode_tokens_per_s": (bt.num_seqs + bk.num_seqs) / (ms_both * 1e-3)}
     del dk, ct, ck
-    # shared-prefix cascade on configs[1] (prefix pass with stacked heads + suffix pass + merge)
-    from paper_2606_12688_b200.harness import CascadeDecode
-    d2c = DeviceBatch(b2, device=dev)
-    d2c.append()
-    casc = CascadeDecode(d2c, n_branches=2, shared_tokens=256)
-    ms_c2 = median_ms([casc.run])
-    res["configs[1] as shared-prefix cascade (SURVEY 8(f) rank 3)"] = {
-        "us": ms_c2 * 1e3, "kv_bytes_unique": b2.kv_bytes_unique(),
-        "GBps_unique": b2.kv_bytes_unique() / (ms_c2 * 1e-3) / 1e9,
-        "note": "3 calls: decode over the 256 shared tokens with both branches' queries stacked as grouped heads, "
-                "decode over the private suffixes, mstar_merge_attn_states; shared pages are 5 % of the bytes, so "
-                "the extra launches outweigh the saving at this shape"}
-    del d2c, casc
+    # shared-prefix cascade decode (mstar_paged_attn_decode_cascade, one call) against the plain
+    # call on the same batch: configs[1] (5 % of the bytes shared) and 16 requests x {2, 3} CFG labels over a shared
+    # context of 2048..6144 tokens (about 90 % of the logical bytes shared)
+    def cascade_entry(b, n_br, shared):
+        d = DeviceBatch(b, device=dev)
+        d.append()
+        S, Hq, Dh = b.num_seqs, b.num_q_heads, b.head_dim
+        parts = mstar.decode_auto_partitions(S, b.num_kv_heads, b.max_seq_len)
+        out = torch.empty((S, Hq, Dh), dtype=torch.bfloat16, device=dev)
+        ws = torch.empty(mstar.decode_workspace_bytes(S, Hq, Dh, parts), dtype=torch.uint8, device=dev)
+        wsc = torch.empty(mstar.decode_cascade_workspace_bytes(S, Hq, b.num_kv_heads, Dh, b.max_seq_len),
+                          dtype=torch.uint8, device=dev)
+        sh = torch.from_numpy(np.ascontiguousarray(shared, dtype=np.int32)).to(dev)
+        ms_p = median_ms([lambda: mstar.paged_attn_decode(out, d.q_decode, d.pool, d.block_table, d.seq_lens,
+                                                          b.max_seq_len, float(b.scale), num_partitions=0,
+                                                          workspace=ws)])
+        ms_c = median_ms([lambda: mstar.paged_attn_decode_cascade(out, d.q_decode, d.pool, d.block_table, d.seq_lens,
+                                                                  sh, n_br, b.max_seq_len, float(b.scale),
+                                                                  workspace=wsc)])
+        lg, uq = b.kv_bytes_logical(), b.kv_bytes_unique()
+        return {"seqs": S, "branches": n_br, "kv_bytes_logical": lg, "kv_bytes_unique": uq,
+                "plain_us": ms_p * 1e3, "cascade_us": ms_c * 1e3, "cascade_over_plain": ms_c / ms_p,
+                "plain_GBps_logical": lg / (ms_p * 1e-3) / 1e9, "cascade_GBps_unique": uq / (ms_c * 1e-3) / 1e9}
+
+    res["cascade decode (SURVEY 8(f) rank 3): configs[1], CFG pairs sharing 256 tokens"] = cascade_entry(
+        b2, 2, [256] * (b2.num_seqs // 2))
+    for n_br in (2, 3):
+        bc, shc = W.cfg_cascade_decode(n_branches=n_br)
+        res["cascade decode (SURVEY 8(f) rank 3): 16 requests x %d labels over a shared context" % n_br] = \
+            cascade_entry(bc, n_br, shc)
+        del bc
+    res["cascade decode note"] = ("one call: prefix streams (one consumer warp group per branch, the shared pages "
+                                  "pass through shared memory once) + suffix streams + LSE combine; the plain call "
+                                  "already fetches shared pages from HBM once when the branches' CTAs read them at "
+                                  "the same time (126 MB L2), so the gain is L2 -> SM traffic and SM work")
     # the BAGEL-like denoise (flow) step, 4 requests x 3 CFG labels x 4096 latent tokens,
     # bidirectional block over the cached label context (causal = 0), appended to scratch pages first
     bf = W.flow_step_bagel()

@@ -189,12 +189,39 @@ int mstar_paged_attn_decode_fp8(void* out, float* lse_out, const void* q, const 
  *   out_a      device, [*][D] fp32, lse_a [*] fp32; row r of the result reads row row_map_a[r] of state A
  *              (row_map_a: device int32 [num_rows], or NULL for the identity)
  *   out_b      device, [num_rows][D] fp32, lse_b [num_rows] fp32
- * The two states are the fp32 outputs (MSTAR_FLAG_OUT_F32) and LSEs of two mstar_paged_attn_decode calls: one over
- * the shared prefix with the branches' queries stacked as grouped heads, one over the private suffixes.
+ * The two states are the fp32 outputs (MSTAR_FLAG_OUT_F32) and LSEs of two attention calls over disjoint key sets
+ * (a caller that splits a context by hand; mstar_paged_attn_decode_cascade needs no such step).
  */
 int mstar_merge_attn_states(void* out, float* lse_out, const float* out_a, const float* lse_a,
                             const int32_t* row_map_a, const float* out_b, const float* lse_b, int64_t num_rows,
                             int32_t head_dim, uint32_t flags, void* stream);
+
+/*
+ * mstar_paged_attn_decode_cascade: mstar_paged_attn_decode for CFG branches whose labels
+ * reference the same prefix pages -- "three labels over a single paged KV pool ... reading page tables in place"
+ * (the Parallel region LLM / LLM_cfg_text / LLM_cfg_img of PAPER.md:104-106).  The result is that of
+ * mstar_paged_attn_decode on the same arguments (same definition, same tolerances); the shared pages of a request
+ * pass through shared memory once for up to three of its branches (G = Hq / Hkv <= 8: one consumer warp group per
+ * branch works on the same tile; four or more branches go in groups of three; G > 8: every branch reads the prefix
+ * itself).
+ *   Sequences are request-major: sequence r * n_branches + b is branch b of request r (num_seqs % n_branches == 0).
+ *   shared_lens    device, [num_seqs / n_branches] int32: the first shared_lens[r] tokens of every branch of request
+ *                  r are the same tokens -- the block-table rows of the branches hold the same page ids for them.
+ *                  Multiples of page_size, <= the seq_len of every branch (values past a branch's seq_len:
+ *                  undefined).  0 = nothing shared.
+ * One call = one split-K launch over prefix streams (the kernel's Q load fetches the rows of every branch, q stays
+ * in its natural [S][Hq][D] layout) and suffix streams, laid end to end in 64-token tiles and cut
+ * into equal CTA ranges as in the balanced mode of mstar_paged_attn_decode, plus one combine launch that merges the
+ * prefix and suffix pieces of every (sequence, head) row by log-sum-exp.  Deterministic, CUDA-graph capturable.
+ * bf16 pool only.  Other arguments, flags and errors as mstar_paged_attn_decode (num_partitions is always 0).
+ */
+size_t mstar_paged_attn_decode_cascade_workspace_bytes(int32_t num_seqs, int32_t num_q_heads, int32_t num_kv_heads,
+                                                       int32_t head_dim, int32_t max_seq_len);
+int mstar_paged_attn_decode_cascade(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool,
+                                    const int32_t* block_table, int64_t block_table_stride,
+                                    const int32_t* seq_lens, const int32_t* shared_lens, int32_t num_seqs,
+                                    int32_t n_branches, int32_t num_q_heads, int32_t max_seq_len, float scale,
+                                    uint32_t flags, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
  * mstar_paged_attn_prefill (step a4): many query tokens per sequence, causal over a cached prefix.

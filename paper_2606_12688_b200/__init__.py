@@ -11,7 +11,8 @@ Python binding.  Names mirror the C entry points:
     build_slot_mapping   <- mstar_build_slot_mapping
     kv_copy_pages        <- mstar_kv_copy_pages       (page moves pool -> pool)
     kv_gather            <- mstar_kv_gather           (pool -> contiguous rows)
-    merge_attn_states    <- mstar_merge_attn_states   (LSE merge for shared-prefix cascade decode)
+    merge_attn_states    <- mstar_merge_attn_states   (LSE merge of two attention states)
+    paged_attn_decode_cascade <- mstar_paged_attn_decode_cascade (CFG branches sharing prefix pages, one call)
 
 There is no CPU fallback: without the built library every call raises ``MstarError``.
 """
@@ -26,6 +27,7 @@ from .binding import (  # noqa: F401
     MstarError,
     build_slot_mapping,
     decode_auto_partitions,
+    decode_cascade_workspace_bytes,
     decode_workspace_bytes,
     kv_append,
     kv_append_fp8,
@@ -35,6 +37,7 @@ from .binding import (  # noqa: F401
     load_library,
     merge_attn_states,
     paged_attn_decode,
+    paged_attn_decode_cascade,
     paged_attn_decode_fp8,
     paged_attn_prefill,
     prefill_workspace_bytes,

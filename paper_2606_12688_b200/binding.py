@@ -31,6 +31,8 @@ EXPORTS = (
     "mstar_paged_attn_decode_workspace_bytes",
     "mstar_paged_attn_decode",
     "mstar_paged_attn_decode_auto_partitions",
+    "mstar_paged_attn_decode_cascade_workspace_bytes",
+    "mstar_paged_attn_decode_cascade",
     "mstar_paged_attn_prefill_workspace_bytes",
     "mstar_paged_attn_prefill",
     "mstar_build_slot_mapping",
@@ -100,6 +102,12 @@ def load_library() -> ctypes.CDLL:
     lib.mstar_paged_attn_decode.argtypes = [
         c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_int64, c.c_void_p,
         c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_uint32, c.c_void_p, c.c_size_t, c.c_void_p]
+    lib.mstar_paged_attn_decode_cascade_workspace_bytes.restype = c.c_size_t
+    lib.mstar_paged_attn_decode_cascade_workspace_bytes.argtypes = [c.c_int32] * 5
+    lib.mstar_paged_attn_decode_cascade.restype = c.c_int
+    lib.mstar_paged_attn_decode_cascade.argtypes = [
+        c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_int64, c.c_void_p, c.c_void_p,
+        c.c_int32, c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_uint32, c.c_void_p, c.c_size_t, c.c_void_p]
     lib.mstar_paged_attn_prefill_workspace_bytes.restype = c.c_size_t
     lib.mstar_paged_attn_prefill_workspace_bytes.argtypes = [c.c_int32] * 4
     lib.mstar_paged_attn_prefill.restype = c.c_int
@@ -327,6 +335,40 @@ def paged_attn_decode(out: torch.Tensor, q: torch.Tensor, pool: KVPool, block_ta
         _ptr(out), _ptr(lse_out), _ptr(q), ctypes.byref(pool.c), _ptr(block_table),
         int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens), S, Hq, int(max_seq_len),
         float(scale), int(num_partitions), flags, _ptr(workspace), ws_bytes, _stream()), "mstar_paged_attn_decode")
+
+
+def decode_cascade_workspace_bytes(num_seqs: int, num_q_heads: int, num_kv_heads: int, head_dim: int,
+                                   max_seq_len: int) -> int:
+    return int(load_library().mstar_paged_attn_decode_cascade_workspace_bytes(num_seqs, num_q_heads, num_kv_heads,
+                                                                               head_dim, max_seq_len))
+
+
+def paged_attn_decode_cascade(out: torch.Tensor, q: torch.Tensor, pool: KVPool, block_table: torch.Tensor,
+                              seq_lens: torch.Tensor, shared_lens: torch.Tensor, n_branches: int, max_seq_len: int,
+                              scale: float, workspace: torch.Tensor, lse_out: Optional[torch.Tensor] = None) -> None:
+    """mstar_paged_attn_decode_cascade: decode of request-major CFG branches that share prefix pages.
+    shared_lens [S / n_branches] int32 on the device."""
+    _want(q, torch.bfloat16, "q"); _want(block_table, torch.int32, "block_table")
+    _want(seq_lens, torch.int32, "seq_lens"); _want(shared_lens, torch.int32, "shared_lens")
+    S, Hq, D = (int(x) for x in q.shape)
+    if n_branches < 1 or S % n_branches or int(shared_lens.shape[0]) != S // n_branches:
+        raise MstarError("shared_lens must have one entry per request (num_seqs / n_branches)")
+    flags = 0
+    if out.dtype == torch.float32:
+        flags |= MSTAR_FLAG_OUT_F32
+    elif out.dtype != torch.bfloat16:
+        raise MstarError("out must be bf16 or fp32")
+    if not out.is_cuda or not out.is_contiguous() or tuple(out.shape) != (S, Hq, D):
+        raise MstarError("out must be a contiguous CUDA tensor [S, Hq, D]")
+    if lse_out is not None:
+        _want(lse_out, torch.float32, "lse_out")
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    lib = load_library()
+    _check(lib.mstar_paged_attn_decode_cascade(
+        _ptr(out), _ptr(lse_out), _ptr(q), ctypes.byref(pool.c), _ptr(block_table),
+        int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens), _ptr(shared_lens), S,
+        int(n_branches), Hq, int(max_seq_len), float(scale), flags, _ptr(workspace), ws_bytes, _stream()),
+        "mstar_paged_attn_decode_cascade")
 
 
 def prefill_workspace_bytes(num_seqs: int, total_q: int, num_q_heads: int, head_dim: int) -> int:

@@ -24,7 +24,7 @@ namespace mstar {
 // With G <= 8 the fp8 consumer (swapped operands, 111 registers) can run 12 warps, three per scheduler: the host
 // picks them for long sequences (192-token stages cost short, ragged streams more in tail tiles than they gain).
 constexpr int decode_tok(int nw) { return 16 * nw; }            // tokens per ring stage
-constexpr int decode_threads(int nw) { return 32 * (nw + 2); }  // + K and V producer warps
+constexpr int decode_threads(int nw, int nb = 1) { return 32 * (nw * nb + 2); }  // + K and V producer warps
 static int decode_pick_warps(bool fp8, int G, int max_seq_len) {
     return fp8 ? ((G <= 8 && max_seq_len > 8192) ? 12 : 8) : 4;
 }
@@ -38,7 +38,8 @@ struct DecodeParams {
     const int32_t* seq_lens;
     int32_t S, Hq, Hkv, G;
     int32_t chunk;   // tokens per partition, multiple of the stage size (decode_tok)
-    int32_t nparts;  // partition slots per (sequence, head) in the workspace
+    int32_t nparts;  // partition slots per (sequence, head) in the workspace (per set: a cascade row has two sets)
+    int32_t slots;   // partial slots of a row = its stride in part_O / part_m / part_l (nparts; cascade 2 nparts)
     float scale_log2;
     float* part_O;  // [S*Hq][nparts][D]
     float* part_m;  // [S*Hq][nparts]   (log2 domain: max of scale*log2e*q.k)
@@ -60,20 +61,33 @@ struct DecodeParams {
     // quantised pool (FP8 instantiations): value = e4m3(code) * scale[page][kv head]
     const float* k_scale;
     const float* v_scale;
+    // Shared-prefix cascade (mstar_paged_attn_decode_cascade; casc_B = 0 otherwise).  The work list runs over V
+    // VIRTUAL sequences instead of the S real ones: first casc_R * casc_ng prefix streams -- request r, branch group
+    // bg: tokens [0, shared_lens[r]) read once for the casc_bpg branches of the group, one consumer warp group per
+    // branch -- then the S suffix streams, tokens [shared_lens[s / B], seq_len) of
+    // sequence s.  Every stream leaves partials only (prefix pieces in slots [0, nparts), suffix pieces in
+    // [nparts, 2 nparts) of a row); the cascade combine merges the two sets of every (sequence, head) row.
+    int32_t V;
+    int32_t casc_B, casc_bpg, casc_ng, casc_R;
+    const int32_t* shared_lens;  // [casc_R]
+    int32_t* vpieces;            // [V][Hkv]: pieces of a stream, written by the CTA that holds its first tile (balanced)
 };
 
 struct ItemInfo {
     int32_t s, kvh, part, tok0, ntok;
     int32_t whole;  // the item is the sequence's whole stream: the consumers write the final output
+    int32_t nb;     // sequences s .. s + nb - 1 share the item's K/V, one consumer warp group each (cascade prefix
+                    // streams; 1 otherwise)
 };
 
-template <int D, int GH, int EB, int NWARPS>  // EB = bytes per pool element (2 = bf16, 1 = e4m3)
+// EB = bytes per pool element (2 = bf16, 1 = e4m3); NB = consumer warp groups (cascade: one per stacked branch)
+template <int D, int GH, int EB, int NWARPS, int NB = 1>
 struct DecodeSmem {
     static constexpr int kWarps = NWARPS;
     static constexpr int kStageBytes = 2 * 16 * kWarps * D * EB;
     static constexpr int kScaleBytes = EB == 1 ? kMaxStages * 2 * 16 * 4 : 0;  // [stage][K|V][page of the stage] fp32
-    static constexpr int kQBytes = GH * D * 2;
-    static constexpr int kMergeBytes = kWarps * GH * (D + 2) * 4;
+    static constexpr int kQBytes = NB * GH * D * 2;
+    static constexpr int kMergeBytes = NB * kWarps * GH * (D + 2) * 4;
     // fixed part after the ring: Q slots, merge buffer, barriers, item info
     static constexpr int kFixed = 2 * kQBytes + kMergeBytes + (2 * kMaxStages + 4) * 8 + 2 * 32 + kScaleBytes;
     static size_t bytes(int nstages, int S) {
@@ -125,18 +139,22 @@ __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
     return d;
 }
 
-template <int D, int PAGE, int GH, bool FP8, int NWARPS>
-__global__ void __launch_bounds__(decode_threads(NWARPS), 1)
+// NB > 1 (cascade calls): NB groups of NWARPS consumer warps work on the same ring stage, group b with the query
+// rows of branch b of the item (sequence it.s + b), so the K/V of a shared prefix pass through shared memory once for
+// NB branches at the per-warp cost of a single one; groups b >= it.nb only hand the stage back.
+template <int D, int PAGE, int GH, bool FP8, int NWARPS, int NB = 1>
+__global__ void __launch_bounds__(decode_threads(NWARPS, NB), 1)
 decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_constant__ CUtensorMap vmap,
                      const DecodeParams p) {
-    constexpr int NW = NWARPS;
+    constexpr int NW = NWARPS;       // consumer warps of a group (16 tokens of a stage each)
+    constexpr int NC = NWARPS * NB;  // consumer warps
     constexpr int TOK = decode_tok(NWARPS);
     constexpr int PPS = TOK / PAGE;  // pages per stage
     constexpr int EB = FP8 ? 1 : 2;    // bytes per pool element
     constexpr int NH = D * EB / 128;   // 128-byte column slices per row (bf16: 64-column halves)
     constexpr int HT = TOK * 128;      // bytes of one slice tile (TOK rows x 128 B)
     constexpr int KBYTES = NH * HT;    // K part of a stage
-    using SM = DecodeSmem<D, GH, EB, NWARPS>;
+    using SM = DecodeSmem<D, GH, EB, NWARPS, NB>;
     static_assert(!FP8 || D == 128, "fp8 pool: one 128-byte line per token row");
     constexpr int VEC = D / 32;
 
@@ -148,15 +166,15 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
     const uint32_t qbuf = ring + nstages * SM::kStageBytes;
     uint8_t* g_after = gbase + (size_t)nstages * SM::kStageBytes;
     uint16_t* qbuf_g = reinterpret_cast<uint16_t*>(g_after);
-    float* merge_O = reinterpret_cast<float*>(g_after + 2 * SM::kQBytes);        // [NW][GH][D]
-    float* merge_m = merge_O + NW * GH * D;                                      // [NW][GH]
-    float* merge_l = merge_m + NW * GH;                                          // [NW][GH]
+    float* merge_O = reinterpret_cast<float*>(g_after + 2 * SM::kQBytes);        // [NC][GH][D]
+    float* merge_m = merge_O + NC * GH * D;                                      // [NC][GH]
+    float* merge_l = merge_m + NC * GH;                                          // [NC][GH]
     uint64_t* bars_g = reinterpret_cast<uint64_t*>(g_after + 2 * SM::kQBytes + SM::kMergeBytes);
     const uint32_t bars = smem_u32(bars_g);
     ItemInfo* info = reinterpret_cast<ItemInfo*>(bars_g + 2 * kMaxStages + 4);
     float* sc_ring = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(info) + 2 * 32);  // FP8 only
-    int32_t* cum = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(info) + 2 * 32 + SM::kScaleBytes);  // [S + 1]
-    int32_t* lens = cum + p.S + 1;                                                                              // [S]
+    int32_t* cum = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(info) + 2 * 32 + SM::kScaleBytes);  // [V + 1]
+    int32_t* lens = cum + p.V + 1;                                                                              // [V]
     auto full_bar = [&](int st) { return bars + 8u * st; };
     auto empty_bar = [&](int st) { return bars + 8u * (kMaxStages + st); };
     auto qfull_bar = [&](int qs) { return bars + 8u * (2 * kMaxStages + qs); };
@@ -167,11 +185,11 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
     if (threadIdx.x == 0) {
         for (int i = 0; i < nstages; ++i) {
             mbar_init(full_bar(i), 2);  // K producer + V producer (each with its own transaction bytes)
-            mbar_init(empty_bar(i), NW);
+            mbar_init(empty_bar(i), NC);
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(qfull_bar(i), 1);
-            mbar_init(qempty_bar(i), NW);
+            mbar_init(qempty_bar(i), NC);
         }
         fence_mbar_init();
     }
@@ -188,20 +206,27 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
     // loop), `out` may still be read by it -- happens after it has completed and its writes are visible.
     asm volatile("griddepcontrol.wait;" ::: "memory");
 
-    if (warp >= NW) {
+    if (warp >= NC) {
         // Two producer warps walk the same item list: warp NW loads the K half of every stage (and Q and the item
         // record), warp NW + 1 the V half.  Each TMA issue with per-lane coordinates is serialised by the hardware
         // interface, so two warps halve the issue time per stage (16 operations per stage at page size 16).
-        const int op_isv = warp - NW;
+        const int op_isv = warp - NC;
         // =============================== PRODUCER ===============================
         prefetch_tensormap(&kmap);
         prefetch_tensormap(&vmap);
-        // exclusive prefix sum of per-sequence partition counts -> compact work list
+        // exclusive prefix sum of per-sequence partition counts -> compact work list (over the virtual sequences
+        // of a cascade call: prefix streams, then suffix streams)
+        const int n_prefix = p.casc_B ? p.casc_R * p.casc_ng : 0;
+        auto vlen = [&](int v) -> int {
+            if (!p.casc_B) return max(__ldg(p.seq_lens + v), 0);
+            if (v < n_prefix) return max(__ldg(p.shared_lens + v / p.casc_ng), 0);
+            const int sq = v - n_prefix;
+            return max(__ldg(p.seq_lens + sq) - max(__ldg(p.shared_lens + sq / p.casc_B), 0), 0);
+        };
         int carry = 0;
-        for (int s0 = 0; s0 < p.S; s0 += 32) {
+        auto scan_round = [&](int s0, int len) {
             const int s = s0 + lane;
-            const int len = (s < p.S) ? max(__ldg(p.seq_lens + s), 0) : 0;
-            if (s < p.S) lens[s] = len;
+            if (s < p.V) lens[s] = len;
             const int n = (len + p.chunk - 1) / p.chunk;
             int incl = n;
 #pragma unroll
@@ -209,10 +234,20 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 const int t = __shfl_up_sync(0xffffffffu, incl, o);
                 if (lane >= o) incl += t;
             }
-            if (s < p.S) cum[s] = carry + incl - n;
+            if (s < p.V) cum[s] = carry + incl - n;
             carry += __shfl_sync(0xffffffffu, incl, 31);
-        }
-        if (lane == 0) cum[p.S] = carry;
+        };
+        // the lengths of the first 256 sequences are requested together (one round trip to memory instead of one
+        // per 32 sequences: the serving batches are a few hundred sequences and this is the start of every CTA)
+        constexpr int PRE = 8;
+        int pre[PRE];
+#pragma unroll
+        for (int k = 0; k < PRE; ++k) pre[k] = (k * 32 + lane < p.V) ? vlen(k * 32 + lane) : 0;
+#pragma unroll
+        for (int k = 0; k < PRE; ++k)
+            if (k * 32 < p.V) scan_round(k * 32, pre[k]);
+        for (int s0 = PRE * 32; s0 < p.V; s0 += 32) scan_round(s0, (s0 + lane < p.V) ? vlen(s0 + lane) : 0);
+        if (lane == 0) cum[p.V] = carry;
         __syncwarp();
         const int n_items = carry * p.Hkv;
         const uint64_t pol = policy_evict_first();
@@ -226,12 +261,27 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         // hand one work item to the consumers and stream its K/V tiles into the ring
         auto emit_item = [&](int s, int kvh, int part, int tok0, int ntok, int whole) {
             const int ntiles = (ntok + TOK - 1) / TOK;
+            int nb = 1;
+            if (p.casc_B) {  // s is a virtual sequence: translate to (first real sequence, branches, token offset)
+                whole = 0;
+                if (s < n_prefix) {
+                    const int r = s / p.casc_ng, bg = s - r * p.casc_ng;
+                    nb = min(p.casc_bpg, p.casc_B - bg * p.casc_bpg);
+                    s = r * p.casc_B + bg * p.casc_bpg;
+                } else {
+                    s -= n_prefix;
+                    tok0 += max(__ldg(p.shared_lens + s / p.casc_B), 0);
+                    part += p.nparts;
+                }
+            }
             if (!op_isv) mbar_wait(qempty_bar(qs), qph ^ 1);
             if (lane == 0 && !op_isv) {
-                info[qs] = ItemInfo{s, kvh, part, tok0, ntok, whole};
-                mbar_arrive_expect_tx(qfull_bar(qs), (uint32_t)(p.G * D * 2));
-                bulk_load_1d(qbuf + qs * SM::kQBytes, p.q + ((size_t)s * p.Hq + (size_t)kvh * p.G) * D,
-                             (uint32_t)(p.G * D * 2), qfull_bar(qs));
+                info[qs] = ItemInfo{s, kvh, part, tok0, ntok, whole, nb};
+                mbar_arrive_expect_tx(qfull_bar(qs), (uint32_t)(nb * p.G * D * 2));
+                for (int b = 0; b < nb; ++b)
+                    bulk_load_1d(qbuf + qs * SM::kQBytes + b * GH * D * 2,
+                                 p.q + ((size_t)(s + b) * p.Hq + (size_t)kvh * p.G) * D, (uint32_t)(p.G * D * 2),
+                                 qfull_bar(qs));
             }
             qs ^= 1;
             if (qs == 0) qph ^= 1;
@@ -275,7 +325,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
             const int64_t fb = (fa + per < N) ? fa + per : N;
             bool cut_here = false;  // a stream begins in this range and continues past its end
             if (fa < N) {
-                int lo = 0, hi = p.S;  // cum[lo]*Hkv <= fa < cum[hi]*Hkv
+                int lo = 0, hi = p.V;  // cum[lo]*Hkv <= fa < cum[hi]*Hkv
                 while (hi - lo > 1) {
                     const int mid = (lo + hi) >> 1;
                     if ((int64_t)cum[mid] * p.Hkv <= fa) lo = mid; else hi = mid;
@@ -291,7 +341,10 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     const int ntl = (int)(((int64_t)(nt - tile) < fb - f) ? (nt - tile) : (fb - f));
                     const int piece = (int)((int64_t)blockIdx.x - fs / per);
                     const int whole = (tile == 0 && ntl == nt) ? 1 : 0;
-                    if (tile == 0 && !whole) {
+                    if (p.casc_B) {  // every stream leaves partials: the CTA with its first tile records the count
+                        if (tile == 0 && lane == 0 && !op_isv)
+                            p.vpieces[(size_t)s * p.Hkv + kvh] = (int)((fs + nt - 1) / per - fs / per) + 1;
+                    } else if (tile == 0 && !whole) {
                         cut_here = true;
                         if (lane == 0 && !op_isv)
                             p.cut[blockIdx.x] = make_int4(s, kvh, (int)((fs + nt - 1) / per - fs / per) + 1, 0);
@@ -302,15 +355,15 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     f += ntl;
                     if (tile + ntl == nt && kvh == p.Hkv - 1) {
                         ++s;
-                        while (s < p.S && cum[s + 1] == cum[s]) ++s;  // sequences without tokens
+                        while (s < p.V && cum[s + 1] == cum[s]) ++s;  // sequences without tokens
                     }
                 }
             }
-            if (!cut_here && lane == 0 && !op_isv) p.cut[blockIdx.x] = make_int4(-1, 0, 0, 0);
+            if (!p.casc_B && !cut_here && lane == 0 && !op_isv) p.cut[blockIdx.x] = make_int4(-1, 0, 0, 0);
         } else {
             for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
                 const int pi = item / p.Hkv, kvh = item - pi * p.Hkv;
-                int lo = 0, hi = p.S;  // cum[lo] <= pi < cum[hi]
+                int lo = 0, hi = p.V;  // cum[lo] <= pi < cum[hi]
                 while (hi - lo > 1) {
                     const int mid = (lo + hi) >> 1;
                     if (cum[mid] <= pi) lo = mid; else hi = mid;
@@ -329,10 +382,10 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         }
     } else {
         // =============================== CONSUMERS ===============================
-        const int w = warp;
+        const int grp = warp / NW, w = warp % NW;  // warp group (branch of a stacked item), token slice of a stage
         const int g = lane >> 2, t4 = lane & 3;
         {  // empty sequences get out = 0, lse = -inf (no work item ever touches them, nor does the combine pass)
-            for (int s = blockIdx.x * NW + w; s < p.S; s += gridDim.x * NW) {
+            for (int s = blockIdx.x * NC + warp; s < p.S; s += gridDim.x * NC) {
                 if (__ldg(p.seq_lens + s) > 0) continue;
                 for (int i = lane; i < p.Hq * D; i += 32) {
                     const size_t idx = (size_t)s * p.Hq * D + i;
@@ -356,6 +409,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
             mbar_wait(qfull_bar(qs), qph);
             const ItemInfo it = info[qs];
             if (it.ntok < 0) break;
+            const bool active = NB == 1 || grp < it.nb;  // a group without a branch in this item only frees the stages
             if constexpr (FP8 && GH == 8) {
                 // ---- fp8 pool, G <= 8: operands swapped, S^T = K Q^T and O^T = V^T P^T, so the 16 MMA rows are tokens
                 // (or d) and the 8 columns are the grouped heads: half the MMAs and accumulator registers of the
@@ -363,7 +417,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 // columns = heads 2t4, 2t4+1.
                 uint32_t qb2[D / 16][2];  // B operand: Q^T[k slots of the 16-wide d block ks][head g]
                 {
-                    const uint16_t* qb = qbuf_g + qs * (SM::kQBytes / 2);
+                    const uint16_t* qb = qbuf_g + qs * (SM::kQBytes / 2) + grp * GH * D;
 #pragma unroll
                     for (int ks = 0; ks < D / 16; ++ks) {
                         qb2[ks][0] = *reinterpret_cast<const uint32_t*>(qb + g * D + ks * 16 + 4 * t4);
@@ -387,7 +441,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 for (int t = 0; t < ntiles; ++t) {
                     mbar_wait(full_bar(st), ph);
                     const int nv = min(16, it.ntok - t * TOK - w * 16);  // valid tokens in this warp's slice
-                    if (nv > 0) {
+                    if (active && nv > 0) {
                         const uint32_t kb = ring + st * SM::kStageBytes;
                         const uint32_t vb = kb + KBYTES;
                         float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};  // two MMA chains
@@ -456,7 +510,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     lh0 += __shfl_xor_sync(0xffffffffu, lh0, o2);
                     lh1 += __shfl_xor_sync(0xffffffffu, lh1, o2);
                 }
-                float* mo = merge_O + (size_t)w * GH * D;
+                float* mo = merge_O + (size_t)(grp * NW + w) * GH * D;
                 const float f = MSTAR_FP8_BIAS_IN_SCALES ? kTwo60 : 1.f;
 #pragma unroll
                 for (int c = 0; c < D / 16; ++c) {
@@ -465,16 +519,16 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                         make_float2(ot[c][1] * f, ot[c][3] * f);
                 }
                 if (g == 0) {
-                    merge_m[w * GH + 2 * t4] = mh0 * p.scale_log2;
-                    merge_m[w * GH + 2 * t4 + 1] = mh1 * p.scale_log2;
-                    merge_l[w * GH + 2 * t4] = lh0;
-                    merge_l[w * GH + 2 * t4 + 1] = lh1;
+                    merge_m[(grp * NW + w) * GH + 2 * t4] = mh0 * p.scale_log2;
+                    merge_m[(grp * NW + w) * GH + 2 * t4 + 1] = mh1 * p.scale_log2;
+                    merge_l[(grp * NW + w) * GH + 2 * t4] = lh0;
+                    merge_l[(grp * NW + w) * GH + 2 * t4 + 1] = lh1;
                 }
             } else {
                 // Q fragments (A operand), rows = grouped query heads
                 uint32_t qa[D / 16][4];
                 {
-                    const uint16_t* qb = qbuf_g + qs * (SM::kQBytes / 2);
+                    const uint16_t* qb = qbuf_g + qs * (SM::kQBytes / 2) + grp * GH * D;
     #pragma unroll
                     for (int ks = 0; ks < D / 16; ++ks) {
                         // FP8: this lane's K bytes of a 16-wide d block are d = 4*t4 .. 4*t4+3 (one ldmatrix word), so
@@ -513,7 +567,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 for (int t = 0; t < ntiles; ++t) {
                     mbar_wait(full_bar(st), ph);
                     const int nv = min(16, it.ntok - t * TOK - w * 16);  // valid tokens in this warp's slice
-                    if (nv > 0) {
+                    if (active && nv > 0) {
                         const uint32_t kb = ring + st * SM::kStageBytes;
                         const uint32_t vb = kb + KBYTES;
                         // ---- S = Q K^T for 16 tokens (two n-blocks of 8)
@@ -647,7 +701,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
                 }
                 {
-                    float* mo = merge_O + (size_t)w * GH * D;
+                    float* mo = merge_O + (size_t)(grp * NW + w) * GH * D;
     #pragma unroll
                     for (int j = 0; j < D / 8; ++j) {
                         if constexpr (FP8) {  // n-blocks 2c | 2c+1 hold the even | odd d of block c: d = 16c + 4t4 + 0..3
@@ -666,34 +720,34 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                         }
                     }
                     if (t4 == 0) {
-                        merge_m[w * GH + g] = m0 * p.scale_log2;
-                        merge_l[w * GH + g] = l0;
+                        merge_m[(grp * NW + w) * GH + g] = m0 * p.scale_log2;
+                        merge_l[(grp * NW + w) * GH + g] = l0;
                         if (GH == 16) {
-                            merge_m[w * GH + g + 8] = m1 * p.scale_log2;
-                            merge_l[w * GH + g + 8] = l1;
+                            merge_m[(grp * NW + w) * GH + g + 8] = m1 * p.scale_log2;
+                            merge_l[(grp * NW + w) * GH + g + 8] = l1;
                         }
                     }
                 }
             }
-            named_bar_sync(1, NW * 32);
-            for (int r = w; r < p.G; r += NW) {
+            named_bar_sync(1 + grp, NW * 32);
+            for (int r = w; r < (active ? p.G : 0); r += NW) {
                 float M = -INFINITY;
 #pragma unroll
-                for (int x = 0; x < NW; ++x) M = fmaxf(M, merge_m[x * GH + r]);
+                for (int x = 0; x < NW; ++x) M = fmaxf(M, merge_m[(grp * NW + x) * GH + r]);
                 float acc[VEC];
 #pragma unroll
                 for (int i = 0; i < VEC; ++i) acc[i] = 0.f;
                 float lsum = 0.f;
 #pragma unroll
                 for (int x = 0; x < NW; ++x) {
-                    const float mx = merge_m[x * GH + r];
+                    const float mx = merge_m[(grp * NW + x) * GH + r];
                     const float a = (mx == -INFINITY) ? 0.f : fast_exp2(mx - M);
-                    lsum += a * merge_l[x * GH + r];
-                    const float* src = merge_O + ((size_t)x * GH + r) * D + lane * VEC;
+                    lsum += a * merge_l[(grp * NW + x) * GH + r];
+                    const float* src = merge_O + ((size_t)(grp * NW + x) * GH + r) * D + lane * VEC;
 #pragma unroll
                     for (int i = 0; i < VEC; ++i) acc[i] += a * src[i];
                 }
-                const size_t row = (size_t)it.s * p.Hq + (size_t)it.kvh * p.G + r;
+                const size_t row = (size_t)(it.s + grp) * p.Hq + (size_t)it.kvh * p.G + r;  // group = branch
                 if (it.whole) {
                     const float inv = 1.f / lsum;
 #pragma unroll
@@ -701,16 +755,16 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     store_out_vec(p.out, p.out_f32, row * D + lane * VEC, acc, VEC);
                     if (p.lse && lane == 0) p.lse[row] = (M + log2f(lsum)) * 0.6931471805599453f;
                 } else {
-                    float* dst = p.part_O + (row * p.nparts + it.part) * D + lane * VEC;
+                    float* dst = p.part_O + (row * p.slots + it.part) * D + lane * VEC;
 #pragma unroll
                     for (int i = 0; i < VEC; ++i) dst[i] = acc[i];
                     if (lane == 0) {
-                        p.part_m[row * p.nparts + it.part] = M;
-                        p.part_l[row * p.nparts + it.part] = lsum;
+                        p.part_m[row * p.slots + it.part] = M;
+                        p.part_l[row * p.slots + it.part] = lsum;
                     }
                 }
             }
-            named_bar_sync(1, NW * 32);
+            named_bar_sync(1 + grp, NW * 32);
         }
     }
 }
@@ -811,6 +865,84 @@ __global__ void __launch_bounds__(128) decode_combine_kernel(const float* __rest
 }
 
 // ---------------------------------------------------------------------------------------------
+// step a3 of a cascade call: one warp per (sequence, head) row merges the prefix pieces of the row's request / branch
+// group (slots [0, np_p)) with the suffix pieces of its own sequence (slots [nparts, nparts + np_s)) by log-sum-exp
+// in slot order (deterministic), normalises and rounds once.  Piece counts: fixed partitions -> from the lengths, the
+// arithmetic the split-K kernel used; balanced -> the counts it recorded per stream.
+template <int D>
+__global__ void __launch_bounds__(128) decode_combine_cascade_kernel(
+    const float* __restrict__ part_O, const float* __restrict__ part_m, const float* __restrict__ part_l,
+    const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ shared_lens, const int32_t* __restrict__ vpieces,
+    int32_t chunk, int32_t balanced, int32_t S, int32_t Hq, int32_t Hkv, int32_t G, int32_t B, int32_t bpg,
+    int32_t ng, int32_t nparts, void* __restrict__ out, float* __restrict__ lse, int32_t out_f32) {
+    constexpr int VEC = D / 32;
+    const int lane = threadIdx.x & 31;
+    const int64_t row = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (row >= (int64_t)S * Hq) return;
+    const int s = (int)(row / Hq), h = (int)(row - (int64_t)s * Hq);
+    const int L = seq_lens[s];
+    if (L <= 0) return;  // zero-filled by the split-K kernel
+    const int r = s / B, kvh = h / G;
+    const int sh = min(max(shared_lens[r], 0), L);
+    const int vp = r * ng + (s - r * B) / bpg, vs = (S / B) * ng + s;
+    int np_p = 0, np_s = 0;
+    if (sh > 0) np_p = balanced ? vpieces[(size_t)vp * Hkv + kvh] : (sh + chunk - 1) / chunk;
+    if (L - sh > 0) np_s = balanced ? vpieces[(size_t)vs * Hkv + kvh] : (L - sh + chunk - 1) / chunk;
+    const int slots = 2 * nparts;
+    const float* pm = part_m + row * slots;
+    const float* pl = part_l + row * slots;
+    const float* po = part_O + row * slots * D + lane * VEC;
+    // row maximum: lane i takes slot i of each set (at most 33 slots per set: one more round for lane 0)
+    float M = -INFINITY;
+    for (int i = lane; i < np_p; i += 32) M = fmaxf(M, pm[i]);
+    for (int i = lane; i < np_s; i += 32) M = fmaxf(M, pm[nparts + i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+    const float Mrow = M;
+    float acc[VEC];
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) acc[e] = 0.f;
+    float lsum = 0.f;
+    constexpr int PB = 4;  // pieces per batch: all loads of a batch are in flight before the first use
+    for (int i0 = 0; i0 < np_p + np_s; i0 += PB) {
+        float v[PB][VEC], mi[PB], li[PB];
+#pragma unroll
+        for (int u = 0; u < PB; ++u) {
+            const int i = i0 + u;
+            mi[u] = -INFINITY;
+            li[u] = 0.f;
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) v[u][e] = 0.f;
+            if (i < np_p + np_s) {
+                const int slot = i < np_p ? i : nparts + (i - np_p);
+                mi[u] = pm[slot];
+                li[u] = pl[slot];
+                if constexpr (VEC == 4) {
+                    const float4 t = *reinterpret_cast<const float4*>(po + (size_t)slot * D);
+                    v[u][0] = t.x; v[u][1] = t.y; v[u][2] = t.z; v[u][3] = t.w;
+                } else {
+                    const float2 t = *reinterpret_cast<const float2*>(po + (size_t)slot * D);
+                    v[u][0] = t.x; v[u][1] = t.y;
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < PB; ++u) {
+            const float a = (mi[u] == -INFINITY) ? 0.f : fast_exp2(mi[u] - Mrow);
+            lsum += a * li[u];
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) acc[e] += a * v[u][e];
+        }
+    }
+    const float inv = 1.f / lsum;
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) acc[e] *= inv;
+    store_out_vec(out, out_f32, (size_t)row * D + lane * VEC, acc, VEC);
+    if (lse && lane == 0) lse[row] = (M + log2f(lsum)) * 0.6931471805599453f;
+}
+
+// ---------------------------------------------------------------------------------------------
 static int32_t round_up(int32_t x, int32_t m) { return (x + m - 1) / m * m; }
 
 static int32_t auto_chunk(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t tok) {
@@ -854,16 +986,16 @@ static void partition_plan(int32_t S, int32_t Hkv, int32_t max_seq_len, int32_t 
     if (num_partitions > 0 && *nparts > num_partitions) *nparts = num_partitions;
 }
 
-template <int D, int PAGE, int GH, bool FP8, int NWARPS>
+template <int D, int PAGE, int GH, bool FP8, int NWARPS, int NB = 1>
 static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, cudaStream_t stream, int* grid_out) {
-    using SM = DecodeSmem<D, GH, FP8 ? 1 : 2, NWARPS>;
+    using SM = DecodeSmem<D, GH, FP8 ? 1 : 2, NWARPS, NB>;
     const int max_smem = device_max_smem_optin();
-    int nstages = (int)(((int64_t)max_smem - 1024 - SM::kFixed - (int64_t)(2 * p.S + 1) * 4 - 16) / SM::kStageBytes);
+    int nstages = (int)(((int64_t)max_smem - 1024 - SM::kFixed - (int64_t)(2 * p.V + 1) * 4 - 16) / SM::kStageBytes);
     if (nstages > kMaxStages) nstages = kMaxStages;
     if (nstages < 2) return MSTAR_ERR_UNSUPPORTED;
     p.nstages = nstages;
-    const size_t smem = SM::bytes(nstages, p.S);
-    auto kern = decode_splitk_kernel<D, PAGE, GH, FP8, NWARPS>;
+    const size_t smem = SM::bytes(nstages, p.V);
+    auto kern = decode_splitk_kernel<D, PAGE, GH, FP8, NWARPS, NB>;
     static PerDeviceOnce attr_once;  // per instantiation
     MSTAR_CUDA_OK(set_max_dynamic_smem(attr_once, kern, max_smem));
     int grid = device_sm_count();
@@ -873,7 +1005,7 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
     *grid_out = grid;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(decode_threads(NWARPS));
+    cfg.blockDim = dim3(decode_threads(NWARPS, NB));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
@@ -904,8 +1036,16 @@ extern "C" size_t mstar_paged_attn_decode_workspace_bytes(int32_t num_seqs, int3
     return 256 + rows * head_dim * 4 + 2 * rows * 4 + 256 + 16 + (size_t)mstar::kMaxDecodeGrid * 16;
 }
 
-// bf16 pool (k_scale == v_scale == NULL, fp8 false) or quantised pool
-static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, void* out, float* lse_out,
+// Workspace of a cascade call: two sets of partial slots per row + one piece count per (virtual sequence, kv head).
+static size_t cascade_workspace_bytes(int32_t num_seqs, int32_t num_q_heads, int32_t num_kv_heads, int32_t head_dim,
+                                      int32_t nparts) {
+    const size_t rows = (size_t)num_seqs * num_q_heads * 2 * (size_t)nparts;
+    return 256 + rows * head_dim * 4 + 2 * rows * 4 + 256 + 16 + (size_t)2 * num_seqs * num_kv_heads * 4 + 64;
+}
+
+// bf16 pool (k_scale == v_scale == NULL, fp8 false) or quantised pool; n_branches > 0: shared-prefix cascade
+static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, int32_t n_branches,
+                        const int32_t* shared_lens, void* out, float* lse_out,
                         const void* q, const mstar_kv_pool* pool, const int32_t* block_table,
                         int64_t block_table_stride, const int32_t* seq_lens, int32_t num_seqs, int32_t num_q_heads,
                         int32_t max_seq_len, float scale, int32_t num_partitions, uint32_t flags, void* workspace,
@@ -926,6 +1066,8 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
     const int G = num_q_heads / pool->num_kv_heads;
     if (G > 16) return MSTAR_ERR_UNSUPPORTED;
     if (num_seqs > 16384) return MSTAR_ERR_UNSUPPORTED;
+    const bool casc = n_branches > 0;
+    if (casc && (!shared_lens || !aligned(shared_lens, 4) || num_seqs % n_branches)) return MSTAR_ERR_INVALID_ARG;
     const int D = pool->head_dim, PAGE = pool->page_size;
 
     DecodeParams p{};
@@ -934,8 +1076,28 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
     partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, tok, &p.chunk, &p.nparts);
     if (num_partitions == 0)
         p.balanced = balanced_plan(max_seq_len > 0 ? max_seq_len : 1, tok, &p.nparts, &p.per_min) ? 1 : 0;
-    p.direct = (p.nparts == 1);
-    if (!p.direct) {
+    p.direct = (p.nparts == 1) && !casc;
+    p.slots = p.nparts;
+    p.V = num_seqs;
+    if (casc) {
+        // up to three branches share one pass over the prefix, one consumer warp group each (G <= 8; above that
+        // every branch reads the prefix itself)
+        p.casc_B = n_branches;
+        p.casc_bpg = G > 8 ? 1 : (n_branches < 3 ? n_branches : 3);
+        p.casc_ng = (n_branches + p.casc_bpg - 1) / p.casc_bpg;
+        p.casc_R = num_seqs / n_branches;
+        p.shared_lens = shared_lens;
+        p.V = p.casc_R * p.casc_ng + num_seqs;
+        p.slots = 2 * p.nparts;
+        const size_t need = cascade_workspace_bytes(num_seqs, num_q_heads, pool->num_kv_heads, D, p.nparts);
+        if (!workspace || !aligned(workspace, 16)) return MSTAR_ERR_INVALID_ARG;
+        if (workspace_bytes < need) return MSTAR_ERR_WORKSPACE_TOO_SMALL;
+        const size_t rows = (size_t)num_seqs * num_q_heads * p.slots;
+        p.part_O = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + 256);
+        p.part_m = p.part_O + rows * D;
+        p.part_l = p.part_m + rows;
+        p.vpieces = reinterpret_cast<int32_t*>((reinterpret_cast<uintptr_t>(p.part_l + rows + 64) + 15) & ~uintptr_t(15));
+    } else if (!p.direct) {
         const size_t need = mstar_paged_attn_decode_workspace_bytes(num_seqs, num_q_heads, D, p.nparts);
         if (!workspace || !aligned(workspace, 16)) return MSTAR_ERR_INVALID_ARG;
         if (workspace_bytes < need) return MSTAR_ERR_WORKSPACE_TOO_SMALL;
@@ -966,7 +1128,7 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
     rc = fp8 ? get_pool_maps_fp8(pool, &maps) : get_pool_maps(pool, &maps);
     if (rc != MSTAR_OK) return rc;
 
-    const int64_t max_items64 = (int64_t)num_seqs * p.nparts * pool->num_kv_heads;
+    const int64_t max_items64 = (int64_t)p.V * p.nparts * pool->num_kv_heads;
     const int max_items = max_items64 > (1 << 30) ? (1 << 30) : (int)max_items64;
     cudaStream_t st = (cudaStream_t)stream;
     const bool g16 = G > 8;
@@ -976,22 +1138,62 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, vo
         rc = g16 ? launch_decode<DD, PP, 16, F8, NWW>(maps, p, max_items, st, &grid)     \
                  : launch_decode<DD, PP, 8, F8, NWW>(maps, p, max_items, st, &grid);
     rc = MSTAR_ERR_UNSUPPORTED;
-    MSTAR_DECODE_CASE(128, 16, false, 4)
-    MSTAR_DECODE_CASE(128, 32, false, 4)
-    MSTAR_DECODE_CASE(64, 16, false, 4)
-    MSTAR_DECODE_CASE(64, 32, false, 4)
-    MSTAR_DECODE_CASE(128, 16, true, 8)
-    MSTAR_DECODE_CASE(128, 32, true, 8)
-    if (!g16) {  // 12 warps need the 111-register consumer of the G <= 8 form
-        if (D == 128 && PAGE == 16 && fp8 && nw == 12)
-            rc = launch_decode<128, 16, 8, true, 12>(maps, p, max_items, st, &grid);
-        if (D == 128 && PAGE == 32 && fp8 && nw == 12)
-            rc = launch_decode<128, 32, 8, true, 12>(maps, p, max_items, st, &grid);
+    const bool grouped = casc && p.casc_bpg > 1;  // cascade with several consumer warp groups: launched below
+    if (!grouped) {
+        MSTAR_DECODE_CASE(128, 16, false, 4)
+        MSTAR_DECODE_CASE(128, 32, false, 4)
+        MSTAR_DECODE_CASE(64, 16, false, 4)
+        MSTAR_DECODE_CASE(64, 32, false, 4)
+        MSTAR_DECODE_CASE(128, 16, true, 8)
+        MSTAR_DECODE_CASE(128, 32, true, 8)
+        if (!g16) {  // 12 warps need the 111-register consumer of the G <= 8 form
+            if (D == 128 && PAGE == 16 && fp8 && nw == 12)
+                rc = launch_decode<128, 16, 8, true, 12>(maps, p, max_items, st, &grid);
+            if (D == 128 && PAGE == 32 && fp8 && nw == 12)
+                rc = launch_decode<128, 32, 8, true, 12>(maps, p, max_items, st, &grid);
+        }
     }
 #undef MSTAR_DECODE_CASE
+    if (grouped) {  // bf16 pool, G <= 8: two or three consumer warp groups
+#define MSTAR_CASCADE_CASE(DD, PP)                                                                  \
+    if (D == DD && PAGE == PP)                                                                      \
+        rc = p.casc_bpg == 2 ? launch_decode<DD, PP, 8, false, 4, 2>(maps, p, max_items, st, &grid) \
+                             : launch_decode<DD, PP, 8, false, 4, 3>(maps, p, max_items, st, &grid);
+        rc = MSTAR_ERR_UNSUPPORTED;
+        MSTAR_CASCADE_CASE(128, 16)
+        MSTAR_CASCADE_CASE(128, 32)
+        MSTAR_CASCADE_CASE(64, 16)
+        MSTAR_CASCADE_CASE(64, 32)
+#undef MSTAR_CASCADE_CASE
+    }
     if (rc != MSTAR_OK) return rc;
 
-    if (!p.direct) {
+    if (casc) {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)(((int64_t)num_seqs * num_q_heads + 3) / 4));
+        cfg.blockDim = dim3(128);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        const float* cO = p.part_O;
+        const float* cm = p.part_m;
+        const float* cl = p.part_l;
+        const int32_t* vp = p.vpieces;
+        if (D == 128)
+            MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, decode_combine_cascade_kernel<128>, cO, cm, cl, seq_lens, shared_lens,
+                                             vp, p.chunk, p.balanced, num_seqs, num_q_heads, p.Hkv, (int32_t)G,
+                                             p.casc_B, p.casc_bpg, p.casc_ng, p.nparts, out, lse_out, p.out_f32));
+        else
+            MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, decode_combine_cascade_kernel<64>, cO, cm, cl, seq_lens, shared_lens,
+                                             vp, p.chunk, p.balanced, num_seqs, num_q_heads, p.Hkv, (int32_t)G,
+                                             p.casc_B, p.casc_bpg, p.casc_ng, p.nparts, out, lse_out, p.out_f32));
+        MSTAR_CUDA_OK(cudaGetLastError());
+        launch_count_add(1);
+    } else if (!p.direct) {
         // fixed partitions: one block per (sequence, head) row; balanced: one per (split-K CTA, head of the group)
         const int64_t blocks = p.balanced ? (int64_t)grid * G : (int64_t)num_seqs * num_q_heads;
         cudaLaunchConfig_t cfg{};
@@ -1025,7 +1227,7 @@ extern "C" int mstar_paged_attn_decode(void* out, float* lse_out, const void* q,
                                        const int32_t* seq_lens, int32_t num_seqs, int32_t num_q_heads,
                                        int32_t max_seq_len, float scale, int32_t num_partitions, uint32_t flags,
                                        void* workspace, size_t workspace_bytes, void* stream) {
-    return decode_entry(false, nullptr, nullptr, out, lse_out, q, pool, block_table, block_table_stride, seq_lens,
+    return decode_entry(false, nullptr, nullptr, 0, nullptr, out, lse_out, q, pool, block_table, block_table_stride, seq_lens,
                         num_seqs, num_q_heads, max_seq_len, scale, num_partitions, flags, workspace,
                         workspace_bytes, stream);
 }
@@ -1036,7 +1238,28 @@ extern "C" int mstar_paged_attn_decode_fp8(void* out, float* lse_out, const void
                                            int32_t num_q_heads, int32_t max_seq_len, float scale,
                                            int32_t num_partitions, uint32_t flags, void* workspace,
                                            size_t workspace_bytes, void* stream) {
-    return decode_entry(true, k_scale, v_scale, out, lse_out, q, pool8, block_table, block_table_stride, seq_lens,
+    return decode_entry(true, k_scale, v_scale, 0, nullptr, out, lse_out, q, pool8, block_table, block_table_stride, seq_lens,
                         num_seqs, num_q_heads, max_seq_len, scale, num_partitions, flags, workspace,
+                        workspace_bytes, stream);
+}
+
+extern "C" size_t mstar_paged_attn_decode_cascade_workspace_bytes(int32_t num_seqs, int32_t num_q_heads,
+                                                                  int32_t num_kv_heads, int32_t head_dim,
+                                                                  int32_t max_seq_len) {
+    if (num_seqs <= 0 || num_q_heads <= 0 || num_kv_heads <= 0 || head_dim <= 0) return 256;
+    int32_t chunk, nparts;
+    mstar::partition_plan(num_seqs, num_kv_heads, max_seq_len, 0, mstar::decode_tok(4), &chunk, &nparts);
+    return cascade_workspace_bytes(num_seqs, num_q_heads, num_kv_heads, head_dim, nparts);
+}
+
+extern "C" int mstar_paged_attn_decode_cascade(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool,
+                                               const int32_t* block_table, int64_t block_table_stride,
+                                               const int32_t* seq_lens, const int32_t* shared_lens, int32_t num_seqs,
+                                               int32_t n_branches, int32_t num_q_heads, int32_t max_seq_len,
+                                               float scale, uint32_t flags, void* workspace, size_t workspace_bytes,
+                                               void* stream) {
+    if (n_branches < 1) return MSTAR_ERR_INVALID_ARG;
+    return decode_entry(false, nullptr, nullptr, n_branches, shared_lens, out, lse_out, q, pool, block_table,
+                        block_table_stride, seq_lens, num_seqs, num_q_heads, max_seq_len, scale, 0, flags, workspace,
                         workspace_bytes, stream);
 }

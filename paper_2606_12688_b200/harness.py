@@ -75,6 +75,21 @@ class DeviceBatch:
                                 num_partitions=num_partitions, workspace=ws, lse_out=lse)
         return out, lse
 
+    def decode_cascade(self, n_branches, shared_lens, out_dtype=torch.bfloat16, want_lse=True):
+        """mstar_paged_attn_decode_cascade on the batch (request-major branches, shared_lens int32 per request)."""
+        b = self.b
+        S, Hq, D = b.num_seqs, b.num_q_heads, b.head_dim
+        dev = self.q_decode.device
+        out = torch.full((S, Hq, D), float("nan"), dtype=out_dtype, device=dev)
+        lse = torch.full((S, Hq), float("nan"), dtype=torch.float32, device=dev) if want_lse else None
+        ws = torch.empty(mstar.decode_cascade_workspace_bytes(S, Hq, b.num_kv_heads, D, b.max_seq_len),
+                         dtype=torch.uint8, device=dev)
+        ws.fill_(0xFF)
+        sh = torch.from_numpy(np.ascontiguousarray(shared_lens, dtype=np.int32)).to(dev)
+        mstar.paged_attn_decode_cascade(out, self.q_decode, self.pool, self.block_table, self.seq_lens, sh,
+                                        n_branches, b.max_seq_len, float(b.scale), workspace=ws, lse_out=lse)
+        return out, lse
+
     def prefill(self, causal=True, out_dtype=torch.bfloat16, want_lse=True, mma_sync=False):
         b = self.b
         T, Hq, D = b.total_q, b.num_q_heads, b.head_dim
@@ -158,60 +173,3 @@ class DeviceBatchFp8:
         """Pool codes of the used pages [U, Hkv, p, D] uint8 on the host."""
         idx = torch.from_numpy(self.b.used_pages).to(self.k_pool.device)
         return self.k_pool[idx].cpu().numpy(), self.v_pool[idx].cpu().numpy()
-
-
-class CascadeDecode:
-    """Shared-prefix ("cascade") decode for CFG branches on a DeviceBatch whose sequences are
-    request-major with ``n_branches`` branches per request sharing the pages of their first ``shared_tokens``
-    tokens: pass A = one decode over the shared prefix with the branches' queries stacked as grouped heads,
-    pass B = one decode over the private suffixes, then ``mstar_merge_attn_states``.  Argument marshalling only."""
-
-    def __init__(self, db: "DeviceBatch", n_branches: int, shared_tokens: int):
-        b = db.b
-        self.db, self.B = db, n_branches
-        S, Hq, Hkv, D, p = b.num_seqs, b.num_q_heads, b.num_kv_heads, b.head_dim, b.page_size
-        assert S % n_branches == 0 and shared_tokens % p == 0
-        R, G = S // n_branches, Hq // Hkv
-        dev = db.q_decode.device
-        self.R, self.HqA = R, Hq * n_branches
-        self.bt_a = db.block_table[::n_branches].contiguous()
-        self.len_a = torch.full((R,), shared_tokens, dtype=torch.int32, device=dev)
-        self.bt_b = db.block_table[:, shared_tokens // p:].contiguous()
-        self.len_b = (db.seq_lens - shared_tokens).to(torch.int32)
-        self.max_b = int(b.max_seq_len) - shared_tokens
-        self.shared = shared_tokens
-        # stacked query rows: [request][kv head][branch][g]
-        s_idx = torch.arange(S, device=dev).view(R, 1, n_branches, 1)
-        h_idx = (torch.arange(Hkv, device=dev).view(1, Hkv, 1, 1) * G + torch.arange(G, device=dev).view(1, 1, 1, G))
-        self.gather_rows = (s_idx * Hq + h_idx).reshape(-1)                       # stacked row -> (s, h) row
-        row_map = torch.empty(S * Hq, dtype=torch.int32, device=dev)
-        row_map[self.gather_rows] = torch.arange(S * Hq, dtype=torch.int32, device=dev)
-        self.row_map = row_map                                                    # (s, h) row -> stacked row
-        self.q_a = torch.empty((R, self.HqA, D), dtype=torch.bfloat16, device=dev)
-        self.out_a = torch.empty((R, self.HqA, D), dtype=torch.float32, device=dev)
-        self.lse_a = torch.empty((R, self.HqA), dtype=torch.float32, device=dev)
-        self.out_b = torch.empty((S, Hq, D), dtype=torch.float32, device=dev)
-        self.lse_b = torch.empty((S, Hq), dtype=torch.float32, device=dev)
-        self.out = torch.empty((S, Hq, D), dtype=torch.bfloat16, device=dev)
-        self.lse = torch.empty((S, Hq), dtype=torch.float32, device=dev)
-        pa = mstar.decode_auto_partitions(R, Hkv, shared_tokens)
-        pb = mstar.decode_auto_partitions(S, Hkv, self.max_b)
-        self.ws_a = torch.empty(mstar.decode_workspace_bytes(R, self.HqA, D, pa), dtype=torch.uint8, device=dev)
-        self.ws_b = torch.empty(mstar.decode_workspace_bytes(S, Hq, D, pb), dtype=torch.uint8, device=dev)
-        self.stack_queries()
-
-    def stack_queries(self):
-        """The branch queries in stacked order: an input layout (the caller's projection writes it), prepared here
-        once with a row gather, outside any timed region."""
-        D = self.db.b.head_dim
-        torch.index_select(self.db.q_decode.view(-1, D), 0, self.gather_rows, out=self.q_a.view(-1, D))
-
-    def run(self):
-        b, db = self.db.b, self.db
-        mstar.paged_attn_decode(self.out_a, self.q_a, db.pool, self.bt_a, self.len_a, self.shared, float(b.scale),
-                                num_partitions=0, workspace=self.ws_a, lse_out=self.lse_a)
-        mstar.paged_attn_decode(self.out_b, db.q_decode, db.pool, self.bt_b, self.len_b, self.max_b, float(b.scale),
-                                num_partitions=0, workspace=self.ws_b, lse_out=self.lse_b)
-        mstar.merge_attn_states(self.out, self.out_a, self.lse_a, self.out_b, self.lse_b, row_map_a=self.row_map,
-                                lse_out=self.lse)
-        return self.out, self.lse

@@ -1,3 +1,3 @@
 """Re-export of the device plumbing used by the GPU tests."""
 from paper_2606_12688_b200.harness import (  # noqa: F401
-    CascadeDecode, DeviceBatch, DeviceBatchFp8, bf16_tensor, bits_of, f64_of)
+    DeviceBatch, DeviceBatchFp8, bf16_tensor, bits_of, f64_of)
