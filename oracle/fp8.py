@@ -13,6 +13,8 @@ Definitions
                  saturation to +-448 ("satfinite"); NaN -> 0x7F.  The quantised code is an integer decided by
                  floating point, so both sides take the decision in the kernel's precision (fp32).
   DECODE_FP8     ORACLE_DECODE on the dequantised K and V.
+  PREFILL_FP8    ORACLE_PREFILL on the dequantised K and V: query row i of sequence s (n_s rows) sees
+                 positions j <= (L_s - n_s) + i when causal (R6), all L_s positions otherwise.
 Pools are uint8 ``[num_pages, Hkv, page_size, D]``; scales fp32 ``[num_pages, Hkv]`` (inputs, caller-owned).
 """
 from __future__ import annotations
@@ -116,4 +118,41 @@ def paged_decode_fp8(q, k_pool8, v_pool8, k_scale, v_scale, block_table, seq_len
             Z = w.sum()
             out[s, h] = (w @ V[:, g, :]) / Z
             lse[s, h] = M + np.log(Z)
+    return out, lse
+
+
+def paged_prefill_fp8(q, cu_seqlens_q, k_pool8, v_pool8, k_scale, v_scale, block_table, seq_lens, scale, causal=True,
+                      rows=None):
+    """PREFILL_FP8.  q bf16 bits uint16 [T, Hq, D], ragged by cu_seqlens_q; rows = ascending global row indices
+    (default all) -> (out fp64 [n_rows, Hq, D], lse fp64 [n_rows, Hq]).  Written out row by row: gather and dequantise
+    the sequence, logits over the visible positions, max, exp, sum, weighted sum."""
+    qf = bf16_bits_to_f32(q).astype(np.float64)
+    T, Hq, D = qf.shape
+    Hkv = k_pool8.shape[1]
+    G = Hq // Hkv
+    sc = float(np.float32(scale))
+    cu = np.asarray(cu_seqlens_q, dtype=np.int64)
+    rows = np.arange(T, dtype=np.int64) if rows is None else np.asarray(rows, dtype=np.int64)
+    out = np.zeros((len(rows), Hq, D), dtype=np.float64)
+    lse = np.full((len(rows), Hq), -np.inf, dtype=np.float64)
+    cache_s, K, V = -1, None, None
+    for idx, r in enumerate(rows):
+        s = int(np.searchsorted(cu, r, side="right") - 1)
+        n, L = int(cu[s + 1] - cu[s]), int(seq_lens[s])
+        i = int(r - cu[s])
+        if s != cache_s:
+            K = dequant_gather(k_pool8, k_scale, block_table[s], L)
+            V = dequant_gather(v_pool8, v_scale, block_table[s], L)
+            cache_s = s
+        vis = (L - n) + i + 1 if causal else L   # number of visible positions
+        if vis <= 0:
+            continue
+        for h in range(Hq):
+            g = h // G
+            x = sc * (K[:vis, g, :] @ qf[r, h])
+            M = x.max()
+            w = np.exp(x - M)
+            Z = w.sum()
+            out[idx, h] = (w @ V[:vis, g, :]) / Z
+            lse[idx, h] = M + np.log(Z)
     return out, lse

@@ -160,3 +160,87 @@ def test_append_fp8_quantisation_error_bound_and_saturation():
     assert np.all(np.abs(deq - xf[:, 0, :])[inr] <= np.maximum(np.abs(xf[:, 0, :])[inr] * 2.0 ** -4, 2.0 ** -10 * 0.01) * 1.0001)
     assert k8[0, 0, 0, 0] == 0x7E and k8[0, 0, 0, 1] == 0xFE and k8[0, 0, 0, 2] == 0x00
     assert np.array_equal(k8, v8)
+
+
+def _prefill_case(seed=13, Hq=8, Hkv=2, D=64, p=16, num_pages=40):
+    """Ragged prefill batch on an exactly representable quantised pool: (cu, seq_lens, bt, k8, v8, ks, vs, q)."""
+    rng = np.random.default_rng(seed)
+    q_lens = np.array([5, 1, 0, 33], dtype=np.int32)
+    prefix = np.array([20, 0, 7, 16], dtype=np.int32)
+    seq_lens = (prefix + q_lens).astype(np.int32)
+    S = len(q_lens)
+    cu = np.zeros(S + 1, dtype=np.int32)
+    cu[1:] = np.cumsum(q_lens)
+    perm = rng.permutation(num_pages)
+    bt = np.full((S, 6), -1, dtype=np.int32)
+    cur = 0
+    for s in range(S):
+        n = (int(seq_lens[s]) + p - 1) // p
+        bt[s, :n] = perm[cur:cur + n]
+        cur += n
+    finite = np.array([c for c in range(256) if c not in (0x7F, 0xFF)], dtype=np.uint8)
+    k8 = finite[rng.integers(0, 254, (num_pages, Hkv, p, D))]
+    v8 = finite[rng.integers(0, 254, (num_pages, Hkv, p, D))]
+    ks = (2.0 ** rng.integers(-6, 3, (num_pages, Hkv))).astype(np.float32)
+    vs = (2.0 ** rng.integers(-6, 3, (num_pages, Hkv))).astype(np.float32)
+    q = bf16_bits_from_f32(rng.normal(0, 0.05, (int(cu[-1]), Hq, D)).astype(np.float32))
+    return cu, seq_lens, bt, k8, v8, ks, vs, q
+
+
+@pytest.mark.parametrize("causal", [True, False])
+def test_prefill_fp8_equals_pinned_bf16_prefill_oracle_on_the_dequantised_pool(causal):
+    """PREFILL_FP8 against the pinned C prefill oracle (tests/test_oracle_pins.py) on a pool whose dequantised
+    values are exactly bf16 (power-of-two scales that differ per (page, head))."""
+    cu, seq_lens, bt, k8, v8, ks, vs, q = _prefill_case()
+    t = fp8.e4m3_decode_table()
+    kb = bf16_bits_from_f32((t[k8] * ks.astype(np.float64)[:, :, None, None]).astype(np.float32))
+    vb = bf16_bits_from_f32((t[v8] * vs.astype(np.float64)[:, :, None, None]).astype(np.float32))
+    scale = np.float32(1 / 8)
+    want, want_lse = oracle.paged_prefill(q, cu, kb, vb, bt, seq_lens, scale, causal=causal)
+    got, got_lse = fp8.paged_prefill_fp8(q, cu, k8, v8, ks, vs, bt, seq_lens, scale, causal=causal)
+    assert got.shape == want.shape
+    assert np.abs(got - want).max() <= 1e-12 * max(1.0, np.abs(want).max())
+    assert np.abs(got_lse - want_lse).max() <= 1e-12 * max(1.0, np.abs(want_lse).max())
+
+
+def test_prefill_fp8_one_row_is_decode_last_row_sees_everything_and_row_subset():
+    cu, seq_lens, bt, k8, v8, ks, vs, q = _prefill_case()
+    scale = np.float32(0.125)
+    full, full_lse = fp8.paged_prefill_fp8(q, cu, k8, v8, ks, vs, bt, seq_lens, scale)
+    # the last row of every sequence with rows = DECODE_FP8 with that row as the query
+    last = [int(cu[s + 1]) - 1 for s in range(len(seq_lens)) if cu[s + 1] > cu[s]]
+    seqs = [s for s in range(len(seq_lens)) if cu[s + 1] > cu[s]]
+    dec, dec_lse = fp8.paged_decode_fp8(q[last], k8, v8, ks, vs, bt[seqs], seq_lens[seqs], scale)
+    assert np.abs(full[last] - dec).max() < 1e-13 and np.abs(full_lse[last] - dec_lse).max() < 1e-13
+    # a subset of rows = the same rows of the full result
+    rows = np.array([0, 4, 5, 6, 20, 38])
+    sub, sub_lse = fp8.paged_prefill_fp8(q, cu, k8, v8, ks, vs, bt, seq_lens, scale, rows=rows)
+    assert np.array_equal(sub, full[rows]) and np.array_equal(sub_lse, full_lse[rows])
+    # first row of a sequence without prefix: the dequantised V row 0
+    t = fp8.e4m3_decode_table()
+    r = int(cu[1])   # sequence 1: prefix 0, one row
+    page = int(bt[1, 0])
+    for h in range(q.shape[1]):
+        g = h // (q.shape[1] // k8.shape[1])
+        assert np.array_equal(full[r, h], t[v8[page, g, 0]] * float(vs[page, g]))
+
+
+def test_prefill_fp8_causality_under_saturated_future_codes():
+    """Overwriting every position a row must not see with +-448 codes leaves that row unchanged (R6)."""
+    cu, seq_lens, bt, k8, v8, ks, vs, q = _prefill_case()
+    scale = np.float32(0.125)
+    s, p = 3, 16
+    n, L = int(cu[s + 1] - cu[s]), int(seq_lens[s])
+    i = 10
+    r = int(cu[s]) + i
+    base, _ = fp8.paged_prefill_fp8(q, cu, k8, v8, ks, vs, bt, seq_lens, scale, rows=[r])
+    k2, v2 = k8.copy(), v8.copy()
+    for j in range((L - n) + i + 1, L):
+        k2[bt[s, j // p], :, j % p, :] = 0x7E
+        v2[bt[s, j // p], :, j % p, :] = 0xFE
+    pois, _ = fp8.paged_prefill_fp8(q, cu, k2, v2, ks, vs, bt, seq_lens, scale, rows=[r])
+    assert np.array_equal(base, pois)
+    # and it is not a no-op: the non-causal result does change
+    a, _ = fp8.paged_prefill_fp8(q, cu, k8, v8, ks, vs, bt, seq_lens, scale, causal=False, rows=[r])
+    b, _ = fp8.paged_prefill_fp8(q, cu, k2, v2, ks, vs, bt, seq_lens, scale, causal=False, rows=[r])
+    assert np.abs(a - b).max() > 1e-3
