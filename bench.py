@@ -230,7 +230,7 @@ def run_reference(args):
 
 # ----------------------------------------------------------------------------- the CUDA arm
 
-def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15, b_long=None):
+def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15, b_long=None, bf16_peak=1590.0):
     """configs[1] (BAGEL-like CFG-pair decode) and configs[3] (thinker + talker decode): median call time with a
     cold L2, GB/s on logical and on unique K/V bytes (shared prefix pages counted once), sequences per second."""
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -400,6 +400,37 @@ def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15
                 "bf16_equivalent_GBps": b.kv_bytes_unique() / (ms * 1e-3) / 1e9,
                 "decode_tokens_per_s": S / (ms * 1e-3)}
 
+    def fp8_prefill_entry(b, causal, seed, peak_tf):
+        """append_fp8 of the step's new rows + mstar_paged_attn_prefill_fp8 (expand + plan + tcgen05 kernel)."""
+        ks, vs = W.fp8_page_scales(seed, b.num_pages, b.num_kv_heads)
+        d = DeviceBatchFp8(b, ks, vs, device=dev)
+        d.quantise_store()
+        T, Hq, Dh = b.total_q, b.num_q_heads, b.head_dim
+        from paper_2606_12688_b200.harness import bf16_tensor as _bt
+        q = _bt(b.q, dev)
+        cu = torch.from_numpy(b.cu_seqlens_q).to(dev)
+        out = torch.empty((T, Hq, Dh), dtype=torch.bfloat16, device=dev)
+        ws = torch.empty(mstar.prefill_fp8_workspace_bytes(b.num_seqs, T, Hq, b.num_kv_heads, b.page_size,
+                                                           b.max_seq_len), dtype=torch.uint8, device=dev)
+
+        def call():
+            mstar.kv_append_fp8(d.pool, d.k_new, d.v_new, d.slot_mapping)
+            mstar.paged_attn_prefill_fp8(out, q, cu, d.pool, d.block_table, d.seq_lens, b.max_q_len, b.max_seq_len,
+                                         float(b.scale), workspace=ws, causal=causal)
+
+        ms = median_ms([call])
+        n = b.q_lens.astype(np.float64)
+        Lf = b.seq_lens.astype(np.float64)
+        fl = float((4.0 * Hq * Dh * (n * (Lf - n) + n * (n + 1) / 2)).sum()) if causal else \
+            float((4.0 * Hq * Dh * n * Lf).sum())
+        return {"seqs": b.num_seqs, "ms": ms, "flops": fl, "TFLOPs": fl / (ms * 1e-3) / 1e12,
+                "frac_of_measured_bf16_burst": fl / (ms * 1e-3) / 1e12 / peak_tf,
+                "note": "quantising append of the new rows + expand (codes -> exact bf16 scratch pool) + plan + "
+                        "tcgen05 kernel with per-page scales; the MMAs are bf16 (kind::f16), so the bf16 peak applies"}
+
+    res["fp8 pool (SURVEY 8(f) rank 4): configs[2] causal prefill"] = fp8_prefill_entry(W.config3_prefill(), True, 84,
+                                                                                         bf16_peak)
+    res["fp8 pool (SURVEY 8(f) rank 4): flow step, causal = 0"] = fp8_prefill_entry(bf, False, 85, bf16_peak)
     res["fp8 pool (SURVEY 8(f) rank 4): configs[1] decode"] = fp8_entry(b2, 0, 81)
     res["fp8 pool (SURVEY 8(f) rank 4): configs[3] thinker decode"] = fp8_entry(bt, 0, 82)
     if b_long is not None:
@@ -551,7 +582,8 @@ def run_ours(args):
 
     other = None
     if rank == 0 and not args.no_other:
-        other = other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak=peaks["hbm_gbs"], b_long=bd)
+        other = other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak=peaks["hbm_gbs"], b_long=bd,
+                                bf16_peak=peaks["bf16_tflops"])
 
     if rank != 0:
         if dist is not None:

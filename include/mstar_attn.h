@@ -180,6 +180,26 @@ int mstar_paged_attn_decode_fp8(void* out, float* lse_out, const void* q, const 
                                 uint32_t flags, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * mstar_paged_attn_prefill_fp8: mstar_paged_attn_prefill (incl. causal = 0, the flow step) on the dequantised K and V
+ * of a quantised pool (same pool8 / k_scale / v_scale as above; the new tokens' codes must already be in the pool:
+ * mstar_kv_append_fp8 first).  All other arguments as mstar_paged_attn_prefill; flags: MSTAR_FLAG_OUT_F32 only.
+ * Prefill is bound by the tensor pipe, not by K/V bytes, and the bf16 MMA takes no E4M3 operand, so the call first
+ * writes the EXACT bf16 values of the referenced pages' codes to a compact scratch pool in the workspace
+ * (num_seqs * ceil(max_seq_len / page_size) pages: size the workspace with the function below; max_seq_len must be a
+ * true upper bound here) and then runs the tcgen05 kernel on it with the per-page scales applied in fp32: K scale on
+ * the raw scores of a page's keys, V scale on its probabilities before they are rounded to bf16 for P V.
+ *   workspace      device, >= mstar_paged_attn_prefill_fp8_workspace_bytes(...) bytes, 256-B aligned
+ */
+size_t mstar_paged_attn_prefill_fp8_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads,
+                                                    int32_t num_kv_heads, int32_t page_size, int32_t max_seq_len);
+int mstar_paged_attn_prefill_fp8(void* out, float* lse_out, const void* q, const int32_t* cu_seqlens_q,
+                                 const mstar_kv_pool* pool8, const float* k_scale, const float* v_scale,
+                                 const int32_t* block_table, int64_t block_table_stride, const int32_t* seq_lens,
+                                 int32_t num_seqs, int32_t total_q, int32_t max_q_len, int32_t max_seq_len,
+                                 int32_t num_q_heads, float scale, int32_t causal, uint32_t flags, void* workspace,
+                                 size_t workspace_bytes, void* stream);
+
+/*
  * mstar_merge_attn_states: log-sum-exp merge of two normalised attention states over
  * disjoint key sets, row by row -- the last step of a shared-prefix ("cascade") decode for CFG branches whose
  * labels reference the same prefix pages:

@@ -6,6 +6,7 @@ Python binding.  Names mirror the C entry points:
     kv_append            <- mstar_kv_append
     kv_append_fp8        <- mstar_kv_append_fp8        (quantising append into an E4M3 pool)
     paged_attn_decode_fp8 <- mstar_paged_attn_decode_fp8 (decode over the E4M3 pool)
+    paged_attn_prefill_fp8 <- mstar_paged_attn_prefill_fp8 (prefill / flow step over the E4M3 pool)
     paged_attn_decode    <- mstar_paged_attn_decode   (split-K + LSE combine)
     paged_attn_prefill   <- mstar_paged_attn_prefill  (causal over a cached prefix)
     build_slot_mapping   <- mstar_build_slot_mapping
@@ -40,6 +41,8 @@ from .binding import (  # noqa: F401
     paged_attn_decode_cascade,
     paged_attn_decode_fp8,
     paged_attn_prefill,
+    paged_attn_prefill_fp8,
+    prefill_fp8_workspace_bytes,
     prefill_workspace_bytes,
     status_string,
     version,

@@ -25,6 +25,8 @@ EXPORTS = (
     "mstar_kv_append",
     "mstar_kv_append_fp8",
     "mstar_paged_attn_decode_fp8",
+    "mstar_paged_attn_prefill_fp8_workspace_bytes",
+    "mstar_paged_attn_prefill_fp8",
     "mstar_kv_copy_pages",
     "mstar_kv_gather",
     "mstar_merge_attn_states",
@@ -85,6 +87,13 @@ def load_library() -> ctypes.CDLL:
         c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p, c.c_void_p, c.c_int64,
         c.c_void_p, c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_uint32, c.c_void_p, c.c_size_t,
         c.c_void_p]
+    lib.mstar_paged_attn_prefill_fp8_workspace_bytes.restype = c.c_size_t
+    lib.mstar_paged_attn_prefill_fp8_workspace_bytes.argtypes = [c.c_int32] * 6
+    lib.mstar_paged_attn_prefill_fp8.restype = c.c_int
+    lib.mstar_paged_attn_prefill_fp8.argtypes = [
+        c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p, c.c_void_p,
+        c.c_int64, c.c_void_p, c.c_int32, c.c_int32, c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_int32,
+        c.c_uint32, c.c_void_p, c.c_size_t, c.c_void_p]
     lib.mstar_kv_copy_pages.restype = c.c_int
     lib.mstar_kv_copy_pages.argtypes = [c.POINTER(_KvPoolStruct), c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p,
                                         c.c_int64, c.c_void_p]
@@ -406,6 +415,39 @@ def paged_attn_prefill(out: torch.Tensor, q: torch.Tensor, cu_seqlens_q: torch.T
         int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens), S, T, int(max_q_len),
         int(max_seq_len), Hq, float(scale), 1 if causal else 0, flags, _ptr(workspace), ws_bytes, _stream()),
         "mstar_paged_attn_prefill")
+
+
+def prefill_fp8_workspace_bytes(num_seqs: int, total_q: int, num_q_heads: int, num_kv_heads: int, page_size: int,
+                                max_seq_len: int) -> int:
+    return int(load_library().mstar_paged_attn_prefill_fp8_workspace_bytes(num_seqs, total_q, num_q_heads,
+                                                                            num_kv_heads, page_size, max_seq_len))
+
+
+def paged_attn_prefill_fp8(out: torch.Tensor, q: torch.Tensor, cu_seqlens_q: torch.Tensor, pool: "KVPoolFp8",
+                           block_table: torch.Tensor, seq_lens: torch.Tensor, max_q_len: int, max_seq_len: int,
+                           scale: float, workspace: torch.Tensor, causal: bool = True,
+                           lse_out: Optional[torch.Tensor] = None) -> None:
+    """mstar_paged_attn_prefill_fp8.  q/out [T,Hq,D]; the new tokens' codes must already be in the pool."""
+    _want(q, torch.bfloat16, "q"); _want(cu_seqlens_q, torch.int32, "cu_seqlens_q")
+    _want(block_table, torch.int32, "block_table"); _want(seq_lens, torch.int32, "seq_lens")
+    T, Hq, D = (int(x) for x in q.shape)
+    S = int(cu_seqlens_q.shape[0]) - 1
+    flags = 0
+    if out.dtype == torch.float32:
+        flags |= MSTAR_FLAG_OUT_F32
+    elif out.dtype != torch.bfloat16:
+        raise MstarError("out must be bf16 or fp32")
+    if not out.is_cuda or not out.is_contiguous() or tuple(out.shape) != (T, Hq, D):
+        raise MstarError("out must be a contiguous CUDA tensor [T, Hq, D]")
+    if lse_out is not None:
+        _want(lse_out, torch.float32, "lse_out")
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    lib = load_library()
+    _check(lib.mstar_paged_attn_prefill_fp8(
+        _ptr(out), _ptr(lse_out), _ptr(q), _ptr(cu_seqlens_q), ctypes.byref(pool.c), _ptr(pool.k_scale),
+        _ptr(pool.v_scale), _ptr(block_table), int(block_table.stride(0)) if block_table.dim() == 2 else 0,
+        _ptr(seq_lens), S, T, int(max_q_len), int(max_seq_len), Hq, float(scale), 1 if causal else 0, flags,
+        _ptr(workspace), ws_bytes, _stream()), "mstar_paged_attn_prefill_fp8")
 
 
 def build_slot_mapping(block_table: torch.Tensor, cu_seqlens_q: torch.Tensor, seq_lens: torch.Tensor,

@@ -1,0 +1,202 @@
+// prefill_fp8.cu -- mstar_paged_attn_prefill_fp8: paged prefill (and the flow step, causal = 0) over the quantised
+// (E4M3) K/V pool (R24-R26).
+//
+// Prefill is bound by the tensor pipe, not by K/V bytes (config 3 reads 28 MB of K/V for 0.14 TFLOP), and the
+// tcgen05 kind::f16 MMA takes no E4M3 operand next to a bf16 one.  So the call has two steps, both kernels of this
+// library:
+//   1. kv_expand_fp8_kernel   gathers the pages the batch's block table references and writes their codes as the
+//                             EXACT bf16 values of the codes (every E4M3 value is a bf16 value) into a compact bf16
+//                             scratch pool in the workspace -- page s * maxp + i for logical page i of sequence s --
+//                             together with the identity block table of that pool and the pages' scales by logical
+//                             page.  One read of the codes, one write of twice the bytes.
+//   2. prefill_plan_kernel + prefill_umma_kernel<PAGE, SCALED = true> over the scratch pool: the tcgen05 / TMEM kernel
+//      of prefill_umma.cu, whose softmax warps multiply the raw scores of a page's 16 or 32 keys by its K scale
+//      (fp32, before the mask and the max) and the probabilities by its V scale before they are rounded to bf16 for
+//      P V; the row sums keep the unscaled probabilities.  The roundings are those of the bf16 path (R26).
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include "host_common.h"
+#include "ptx.cuh"
+
+namespace mstar {
+
+struct ExpandParams {
+    const uint8_t* k8;
+    const uint8_t* v8;
+    int64_t stride_page, stride_head, stride_token;  // bytes
+    const float* k_scale;  // [num_pages][Hkv]
+    const float* v_scale;
+    const int32_t* block_table;
+    int64_t bt_stride;
+    const int32_t* seq_lens;
+    int32_t S, Hkv, page_size;
+    int32_t maxp;       // scratch pages per sequence
+    int32_t sc_stride;  // scale entries per (sequence, kv head): maxp rounded up to 8
+    uint16_t* k16;      // scratch pools [S * maxp][Hkv][page_size][128] bf16
+    uint16_t* v16;
+    int32_t* bt16;      // [S][maxp] identity table of the scratch pool
+    float* sc_k;        // [S][Hkv][sc_stride]
+    float* sc_v;
+};
+
+// two E4M3 codes (low 16 bits of w) -> two bf16, exact: e4m3x2 -> f16x2 (exact by definition of the conversion),
+// f16 -> f32 (exact), f32 -> bf16 (exact: four significant bits, exponents within [-9, 8])
+__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2_exact(uint32_t w) {
+    uint32_t h2;
+    asm("{\n\t.reg .b16 lo;\n\tcvt.u16.u32 lo, %1;\n\tcvt.rn.f16x2.e4m3x2 %0, lo;\n\t}" : "=r"(h2) : "r"(w));
+    const __half2 h = *reinterpret_cast<const __half2*>(&h2);
+    const float2 f = __half22float2(h);
+    return pack_bf16x2(f.x, f.y);
+}
+
+// One block per (sequence, logical page slot, kv head); 128 threads; K and V.  Thread t takes 16-byte chunk t of the
+// page's page_size x 128 bytes (page 32: two rounds).
+__global__ void __launch_bounds__(128) kv_expand_fp8_kernel(const ExpandParams p) {
+    const int i = blockIdx.x;  // logical page slot, < sc_stride
+    const int h = blockIdx.y;
+    const int s = blockIdx.z;
+    const int L = max(__ldg(p.seq_lens + s), 0);
+    const int npages = (L + p.page_size - 1) / p.page_size;
+    const bool live = i < npages;
+    int32_t page = 0;
+    if (live) page = __ldg(p.block_table + (size_t)s * p.bt_stride + i);
+    if (threadIdx.x == 0) {
+        const size_t o = ((size_t)s * p.Hkv + h) * p.sc_stride + i;
+        p.sc_k[o] = live ? __ldg(p.k_scale + (size_t)page * p.Hkv + h) : 1.f;
+        p.sc_v[o] = live ? __ldg(p.v_scale + (size_t)page * p.Hkv + h) : 1.f;
+        if (h == 0 && i < p.maxp) p.bt16[(size_t)s * p.maxp + i] = s * p.maxp + i;
+    }
+    if (!live) return;
+    const size_t src = (size_t)page * p.stride_page + (size_t)h * p.stride_head;
+    const size_t dst = (((size_t)s * p.maxp + i) * p.Hkv + h) * p.page_size * 128;
+    for (int c = threadIdx.x; c < p.page_size * 8; c += 128) {
+        const int tok = c >> 3, d0 = (c & 7) * 16;
+        const size_t so = src + (size_t)tok * p.stride_token + d0;
+        const uint4 a = *reinterpret_cast<const uint4*>(p.k8 + so);
+        const uint4 b = *reinterpret_cast<const uint4*>(p.v8 + so);
+        const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, bw[4] = {b.x, b.y, b.z, b.w};
+        uint32_t ko[8], vo[8];
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            ko[2 * w] = e4m3x2_to_bf16x2_exact(aw[w] & 0xffffu);
+            ko[2 * w + 1] = e4m3x2_to_bf16x2_exact(aw[w] >> 16);
+            vo[2 * w] = e4m3x2_to_bf16x2_exact(bw[w] & 0xffffu);
+            vo[2 * w + 1] = e4m3x2_to_bf16x2_exact(bw[w] >> 16);
+        }
+        uint4* kd = reinterpret_cast<uint4*>(p.k16 + dst + (size_t)tok * 128 + d0);
+        uint4* vd = reinterpret_cast<uint4*>(p.v16 + dst + (size_t)tok * 128 + d0);
+        kd[0] = make_uint4(ko[0], ko[1], ko[2], ko[3]);
+        kd[1] = make_uint4(ko[4], ko[5], ko[6], ko[7]);
+        vd[0] = make_uint4(vo[0], vo[1], vo[2], vo[3]);
+        vd[1] = make_uint4(vo[4], vo[5], vo[6], vo[7]);
+    }
+}
+
+struct Fp8PrefillLayout {
+    size_t plan, k16, v16, bt16, sc_k, sc_v, total;
+    int32_t maxp, sc_stride;
+};
+
+static Fp8PrefillLayout fp8_prefill_layout(int32_t S, int32_t total_q, int32_t Hq, int32_t Hkv, int32_t page_size,
+                                           int32_t max_seq_len) {
+    Fp8PrefillLayout l{};
+    auto up = [](size_t x, size_t a) { return (x + a - 1) / a * a; };
+    l.maxp = (max_seq_len + page_size - 1) / page_size;
+    if (l.maxp < 1) l.maxp = 1;
+    l.sc_stride = (l.maxp + 7) / 8 * 8;
+    const size_t pool_bytes = (size_t)S * l.maxp * Hkv * page_size * 128 * 2;
+    l.plan = 0;
+    l.k16 = up(prefill_umma_workspace_bytes(S, total_q, Hq), 1024);
+    l.v16 = up(l.k16 + pool_bytes, 1024);
+    l.bt16 = up(l.v16 + pool_bytes, 256);
+    l.sc_k = up(l.bt16 + (size_t)S * l.maxp * 4, 256);
+    l.sc_v = up(l.sc_k + (size_t)S * Hkv * l.sc_stride * 4, 256);
+    l.total = up(l.sc_v + (size_t)S * Hkv * l.sc_stride * 4, 256);
+    return l;
+}
+
+}  // namespace mstar
+
+extern "C" size_t mstar_paged_attn_prefill_fp8_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads,
+                                                               int32_t num_kv_heads, int32_t page_size,
+                                                               int32_t max_seq_len) {
+    if (num_seqs <= 0 || total_q < 0 || num_q_heads <= 0 || num_kv_heads <= 0 || page_size <= 0 || max_seq_len < 0)
+        return 0;
+    return mstar::fp8_prefill_layout(num_seqs, total_q, num_q_heads, num_kv_heads, page_size, max_seq_len).total;
+}
+
+extern "C" int mstar_paged_attn_prefill_fp8(void* out, float* lse_out, const void* q, const int32_t* cu_seqlens_q,
+                                            const mstar_kv_pool* pool8, const float* k_scale, const float* v_scale,
+                                            const int32_t* block_table, int64_t block_table_stride,
+                                            const int32_t* seq_lens, int32_t num_seqs, int32_t total_q,
+                                            int32_t max_q_len, int32_t max_seq_len, int32_t num_q_heads, float scale,
+                                            int32_t causal, uint32_t flags, void* workspace, size_t workspace_bytes,
+                                            void* stream) {
+    using namespace mstar;
+    launch_count_reset();
+    int rc = check_pool_fp8(pool8);
+    if (rc != MSTAR_OK) return rc;
+    if (!k_scale || !v_scale || !aligned(k_scale, 4) || !aligned(v_scale, 4)) return MSTAR_ERR_INVALID_ARG;
+    if (flags & ~MSTAR_FLAG_OUT_F32) return MSTAR_ERR_INVALID_ARG;
+    if (num_seqs < 0 || total_q < 0 || max_q_len < 0 || max_seq_len < 0 || num_q_heads <= 0)
+        return MSTAR_ERR_INVALID_ARG;
+    if (!(scale > 0.f) || !(scale < 3.0e38f)) return MSTAR_ERR_INVALID_ARG;
+    if (num_seqs == 0 || total_q == 0 || max_q_len == 0) return MSTAR_OK;
+    if (!out || !q || !cu_seqlens_q || !block_table || !seq_lens) return MSTAR_ERR_INVALID_ARG;
+    if (!aligned(out, 16) || !aligned(q, 16)) return MSTAR_ERR_INVALID_ARG;
+    const int32_t Hkv = pool8->num_kv_heads, PAGE = pool8->page_size;
+    if (num_q_heads % Hkv) return MSTAR_ERR_INVALID_ARG;
+    if (num_q_heads / Hkv > 128) return MSTAR_ERR_UNSUPPORTED;
+    const Fp8PrefillLayout l = fp8_prefill_layout(num_seqs, total_q, num_q_heads, Hkv, PAGE, max_seq_len);
+    if (!workspace || !aligned(workspace, 256)) return MSTAR_ERR_INVALID_ARG;
+    if (workspace_bytes < l.total) return MSTAR_ERR_WORKSPACE_TOO_SMALL;
+    if ((int64_t)num_seqs * l.maxp * Hkv * PAGE >= (int64_t(1) << 31)) return MSTAR_ERR_UNSUPPORTED;
+    if (num_seqs > 65535 || Hkv > 65535) return MSTAR_ERR_UNSUPPORTED;
+    uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+    cudaStream_t st = (cudaStream_t)stream;
+
+    ExpandParams e{};
+    e.k8 = reinterpret_cast<const uint8_t*>(pool8->k_pool);
+    e.v8 = reinterpret_cast<const uint8_t*>(pool8->v_pool);
+    e.stride_page = pool8->stride_page;
+    e.stride_head = pool8->stride_head;
+    e.stride_token = pool8->stride_token;
+    e.k_scale = k_scale;
+    e.v_scale = v_scale;
+    e.block_table = block_table;
+    e.bt_stride = block_table_stride;
+    e.seq_lens = seq_lens;
+    e.S = num_seqs;
+    e.Hkv = Hkv;
+    e.page_size = PAGE;
+    e.maxp = l.maxp;
+    e.sc_stride = l.sc_stride;
+    e.k16 = reinterpret_cast<uint16_t*>(ws + l.k16);
+    e.v16 = reinterpret_cast<uint16_t*>(ws + l.v16);
+    e.bt16 = reinterpret_cast<int32_t*>(ws + l.bt16);
+    e.sc_k = reinterpret_cast<float*>(ws + l.sc_k);
+    e.sc_v = reinterpret_cast<float*>(ws + l.sc_v);
+    kv_expand_fp8_kernel<<<dim3((unsigned)l.sc_stride, (unsigned)Hkv, (unsigned)num_seqs), 128, 0, st>>>(e);
+    MSTAR_CUDA_OK(cudaGetLastError());
+    launch_count_add(1);
+
+    // the scratch pool as an ordinary bf16 pool
+    mstar_kv_pool p16{};
+    p16.k_pool = e.k16;
+    p16.v_pool = e.v16;
+    p16.num_pages = (int64_t)num_seqs * l.maxp;
+    p16.page_size = PAGE;
+    p16.num_kv_heads = Hkv;
+    p16.head_dim = 128;
+    p16.stride_token = 128;
+    p16.stride_head = (int64_t)PAGE * 128;
+    p16.stride_page = (int64_t)Hkv * PAGE * 128;
+    PoolMaps maps;
+    rc = get_pool_maps(&p16, &maps);
+    if (rc != MSTAR_OK) return rc;
+    rc = launch_prefill_umma(maps, q, total_q, cu_seqlens_q, e.bt16, l.maxp, seq_lens, num_seqs, num_q_heads, Hkv, PAGE,
+                             max_q_len, scale, causal ? 1 : 0, out, lse_out, (flags & MSTAR_FLAG_OUT_F32) ? 1 : 0, 0,
+                             ws + l.plan, l.k16, st, e.sc_k, e.sc_v, l.sc_stride);
+    return rc;
+}

@@ -169,6 +169,20 @@ class DeviceBatchFp8:
                                     float(b.scale), num_partitions=num_partitions, workspace=ws, lse_out=lse)
         return out, lse
 
+    def prefill(self, causal=True, out_dtype=torch.bfloat16, want_lse=True):
+        b = self.b
+        T, Hq, D = b.total_q, b.num_q_heads, b.head_dim
+        q = bf16_tensor(b.q, self.device)
+        cu = torch.from_numpy(b.cu_seqlens_q).to(self.device)
+        out = torch.full((T, Hq, D), float("nan"), dtype=out_dtype, device=self.device)
+        lse = torch.full((T, Hq), float("nan"), dtype=torch.float32, device=self.device) if want_lse else None
+        ws = torch.empty(mstar.prefill_fp8_workspace_bytes(b.num_seqs, T, Hq, b.num_kv_heads, b.page_size,
+                                                           b.max_seq_len), dtype=torch.uint8, device=self.device)
+        ws.fill_(0xFF)
+        mstar.paged_attn_prefill_fp8(out, q, cu, self.pool, self.block_table, self.seq_lens, b.max_q_len,
+                                     b.max_seq_len, float(b.scale), workspace=ws, causal=causal, lse_out=lse)
+        return out, lse
+
     def store_codes(self):
         """Pool codes of the used pages [U, Hkv, p, D] uint8 on the host."""
         idx = torch.from_numpy(self.b.used_pages).to(self.k_pool.device)

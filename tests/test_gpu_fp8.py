@@ -255,3 +255,118 @@ def test_fp8_error_codes():
     sl = torch.ones(1, dtype=torch.int32, device=dev)
     with pytest.raises(mstar.MstarError, match="UNSUPPORTED"):
         mstar.paged_attn_decode_fp8(out, q, pool64, bt, sl, 1, 0.125, num_partitions=1)
+
+
+# ----------------------------------------------------------------------------- prefill / flow step over the fp8 pool
+
+def prefill_batch(seed, lens, q_lens, Hq=8, Hkv=2, p=16, **kw):
+    rng = np.random.default_rng(seed)
+    pages = sum((l + p - 1) // p for l in lens)
+    return W.make_batch(rng, "p8", lens, q_lens, Hq, Hkv, 128, p, max(2 * pages, 4), **kw)
+
+
+def run_prefill_case(b, causal=True, layout="HND", seed=2, rows=None, check_f32=True):
+    """mstar_kv_append_fp8 (store + new rows; codes bit-exact against APPEND_FP8) then
+    mstar_paged_attn_prefill_fp8 against PREFILL_FP8 on the oracle's codes (gates R11)."""
+    k_scale, v_scale = W.fp8_page_scales(seed, b.num_pages, b.num_kv_heads)
+    db = DeviceBatchFp8(b, k_scale, v_scale, layout=layout)
+    db.quantise_store()
+    db.append()
+    k8, v8, ks, vs = oracle_pool(b, k_scale, v_scale)
+    gk, gv = db.store_codes()
+    assert np.array_equal(gk, k8) and np.array_equal(gv, v8), "quantised codes differ from the oracle"
+    want, want_lse = ofp8.paged_prefill_fp8(b.q, b.cu_seqlens_q, k8, v8, ks, vs, b.compact_block_table, b.seq_lens,
+                                            b.scale, causal=causal, rows=rows)
+    sel = slice(None) if rows is None else np.asarray(rows)
+    out, lse = db.prefill(causal=causal)
+    stats = check_parity(f64_of(out)[sel], want, "%s fp8 prefill causal=%d" % (b.name, causal))
+    assert np.abs(f64_of(lse)[sel] - want_lse).max(initial=0.0) < 2e-3
+    if check_f32:
+        out32, _ = db.prefill(causal=causal, out_dtype=torch.float32)
+        _, r = check_parity(f64_of(out32)[sel], want, "%s fp8 prefill f32" % b.name)
+        assert r <= 6e-3
+    return stats
+
+
+@pytest.mark.parametrize("p", [16, 32])
+@pytest.mark.parametrize("G", [1, 4, 7, 8, 12])
+@pytest.mark.parametrize("causal", [True, False])
+def test_prefill_fp8_ragged_small(p, G, causal):
+    """Ragged batch with cached prefixes: rows per sequence 1 .. 200, prefixes 0 .. 300, an empty sequence."""
+    lens = [200 + 40, 64, 33 + 300, 1, 0, 129 + 16]
+    q_lens = [200, 64, 33, 1, 0, 129]
+    b = prefill_batch(40 + G, lens, q_lens, Hq=G * 2, Hkv=2, p=p)
+    run_prefill_case(b, causal=causal)
+
+
+def test_prefill_fp8_new_tokens_times_prefix_matrix_and_nhd_layout():
+    ns, Ps = [1, 2, 127, 128, 129], [0, 1, 15, 16, 255, 256]
+    lens, q_lens = [], []
+    for n in ns:
+        for P in Ps:
+            lens.append(n + P)
+            q_lens.append(n)
+    b = prefill_batch(77, lens, q_lens, Hq=8, Hkv=2, p=16)
+    run_prefill_case(b, causal=True, layout="NHD", check_f32=False)
+
+
+def test_prefill_fp8_kv_head_counts():
+    for Hkv, G in ((1, 8), (8, 4)):
+        b = prefill_batch(90 + Hkv, [150, 70, 260], [100, 70, 4], Hq=Hkv * G, Hkv=Hkv, p=16)
+        run_prefill_case(b, check_f32=False)
+
+
+def test_prefill_fp8_long_block_over_prefix_and_flow_step_sampled_rows():
+    """1024 new tokens over a 700-token prefix (causal) and a bidirectional 1024-token block over two label contexts
+    that share pages (the flow step, causal = 0), compared on sampled rows."""
+    b = prefill_batch(5, [1724, 1024 + 1], [1024, 1024], Hq=28, Hkv=4, p=16)
+    rows = np.unique(np.concatenate([np.random.default_rng(0).integers(0, 2048, 40), [0, 1023, 1024, 2047]]))
+    print("fp8 prefill causal", run_prefill_case(b, causal=True, rows=rows, check_f32=False))
+    bf = prefill_batch(6, [1024 + 64, 1024 + 64], [1024, 1024], Hq=28, Hkv=4, p=16, share_with=[-1, 0],
+                       shared_tokens=64)
+    print("fp8 flow step", run_prefill_case(bf, causal=False, rows=rows, check_f32=False))
+
+
+def test_prefill_fp8_deterministic_graph_capturable_and_error_codes():
+    b = prefill_batch(8, [300, 90], [128, 90], Hq=8, Hkv=2, p=16)
+    k_scale, v_scale = W.fp8_page_scales(3, b.num_pages, b.num_kv_heads)
+    db = DeviceBatchFp8(b, k_scale, v_scale)
+    db.quantise_store()
+    db.append()
+    o1, _ = db.prefill()
+    o2, _ = db.prefill()
+    assert torch.equal(o1.view(torch.int16), o2.view(torch.int16))
+    T, Hq, D = b.total_q, b.num_q_heads, b.head_dim
+    q = bf16_tensor(b.q)
+    cu = torch.from_numpy(b.cu_seqlens_q).cuda()
+    ws = torch.empty(mstar.prefill_fp8_workspace_bytes(b.num_seqs, T, Hq, b.num_kv_heads, b.page_size, b.max_seq_len),
+                     dtype=torch.uint8, device="cuda")
+    og = torch.empty_like(o1)
+    call = lambda: mstar.paged_attn_prefill_fp8(og, q, cu, db.pool, db.block_table, db.seq_lens, b.max_q_len,
+                                                b.max_seq_len, float(b.scale), workspace=ws)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        call()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            call()
+    torch.cuda.synchronize()
+    og.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(o1.view(torch.int16), og.view(torch.int16))
+    with pytest.raises(mstar.MstarError, match="WORKSPACE_TOO_SMALL"):
+        mstar.paged_attn_prefill_fp8(og, q, cu, db.pool, db.block_table, db.seq_lens, b.max_q_len, b.max_seq_len,
+                                     float(b.scale), workspace=ws[:4096])
+    with pytest.raises(mstar.MstarError, match="INVALID_ARG"):
+        mstar.paged_attn_prefill_fp8(og, q, cu, db.pool, db.block_table, db.seq_lens, b.max_q_len, b.max_seq_len,
+                                     -1.0, workspace=ws)
+
+
+def test_prefill_fp8_config3_full_size_sampled_rows_every_sequence():
+    """BASELINE configs[2] (8 x 1024 new tokens over cached prefixes, 28q / 4kv) on the quantised pool, the launch
+    configuration bench.py times: sampled rows of every sequence incl. first and last rows."""
+    b = W.config3_prefill()
+    rng = np.random.default_rng(11)
+    rows = np.unique(np.concatenate([rng.integers(0, b.total_q, 48), b.cu_seqlens_q[:-1], b.cu_seqlens_q[1:] - 1]))
+    print("fp8 prefill config 3", run_prefill_case(b, causal=True, rows=rows, check_f32=False))
