@@ -183,11 +183,13 @@ int mstar_paged_attn_decode_fp8(void* out, float* lse_out, const void* q, const 
  * mstar_paged_attn_prefill_fp8: mstar_paged_attn_prefill (incl. causal = 0, the flow step) on the dequantised K and V
  * of a quantised pool (same pool8 / k_scale / v_scale as above; the new tokens' codes must already be in the pool:
  * mstar_kv_append_fp8 first).  All other arguments as mstar_paged_attn_prefill; flags: MSTAR_FLAG_OUT_F32 only.
- * Prefill is bound by the tensor pipe, not by K/V bytes, and the bf16 MMA takes no E4M3 operand, so the call first
- * writes the EXACT bf16 values of the referenced pages' codes to a compact scratch pool in the workspace
- * (num_seqs * ceil(max_seq_len / page_size) pages: size the workspace with the function below; max_seq_len must be a
- * true upper bound here) and then runs the tcgen05 kernel on it with the per-page scales applied in fp32: K scale on
- * the raw scores of a page's keys, V scale on its probabilities before they are rounded to bf16 for P V.
+ * Prefill is bound by the tensor pipe, not by K/V bytes, and the 16-bit MMA takes no E4M3 operand, so the call first
+ * writes the referenced pages DEQUANTISED to fp16 -- e4m3(code) * scale, the product exact in fp32, rounded once to
+ * nearest even (11 significant bits; magnitudes above 65504 saturate, below 2^-14 round to multiples of 2^-24) -- to a
+ * compact scratch pool in the workspace (num_seqs * ceil(max_seq_len / page_size) pages: size the workspace with the
+ * function below; max_seq_len must be a true upper bound here) and then runs the tcgen05 kernel of
+ * mstar_paged_attn_prefill on it with fp16 operands (Q converted from bf16 in shared memory, P rounded to fp16).
+ * Tolerances as the bf16 path.
  *   workspace      device, >= mstar_paged_attn_prefill_fp8_workspace_bytes(...) bytes, 256-B aligned
  */
 size_t mstar_paged_attn_prefill_fp8_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads,

@@ -44,8 +44,7 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
                         const int32_t* block_table, int64_t bt_stride, const int32_t* seq_lens, int32_t S,
                         int32_t Hq, int32_t Hkv, int32_t page_size, int32_t max_q_len, float scale, int32_t causal,
                         void* out, float* lse, int32_t out_f32, int32_t reuse_plan, void* workspace,
-                        size_t workspace_bytes, cudaStream_t stream, const float* sc_k = nullptr,
-                        const float* sc_v = nullptr, int32_t sc_stride = 0);
+                        size_t workspace_bytes, cudaStream_t stream, int32_t kv_f16 = 0);
 size_t prefill_umma_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads);
 
 // Properties of the CURRENT device (cudaGetDevice), cached per device ordinal; thread-safe.

@@ -1,18 +1,26 @@
 // prefill_fp8.cu -- mstar_paged_attn_prefill_fp8: paged prefill (and the flow step, causal = 0) over the quantised
-// (E4M3) K/V pool (R24-R26).
+// (E4M3) K/V pool (R24-R27).
 //
 // Prefill is bound by the tensor pipe, not by K/V bytes (config 3 reads 28 MB of K/V for 0.14 TFLOP), and the
 // tcgen05 kind::f16 MMA takes no E4M3 operand next to a bf16 one.  So the call has two steps, both kernels of this
 // library:
-//   1. kv_expand_fp8_kernel   gathers the pages the batch's block table references and writes their codes as the
-//                             EXACT bf16 values of the codes (every E4M3 value is a bf16 value) into a compact bf16
-//                             scratch pool in the workspace -- page s * maxp + i for logical page i of sequence s --
-//                             together with the identity block table of that pool and the pages' scales by logical
-//                             page.  One read of the codes, one write of twice the bytes.
-//   2. prefill_plan_kernel + prefill_umma_kernel<PAGE, SCALED = true> over the scratch pool: the tcgen05 / TMEM kernel
-//      of prefill_umma.cu, whose softmax warps multiply the raw scores of a page's 16 or 32 keys by its K scale
-//      (fp32, before the mask and the max) and the probabilities by its V scale before they are rounded to bf16 for
-//      P V; the row sums keep the unscaled probabilities.  The roundings are those of the bf16 path (R26).
+//   1. kv_expand_fp8_kernel   gathers the pages the batch's block table references and writes them DEQUANTISED to
+//                             fp16 -- e4m3(code) * scale[page][kv head], the product taken in fp32 (exact: 4 x 24
+//                             significant bits), rounded once to nearest even (11 significant bits; saturating at
+//                             +-65504, multiples of 2^-24 below 2^-14) -- into a compact scratch pool in the
+//                             workspace (page s * maxp + i for logical page i of sequence s), together with the
+//                             identity block table of that pool.  One read of the codes, one write of twice the bytes.
+//   2. prefill_plan_kernel + prefill_umma_kernel<PAGE, F16 = true> over the scratch pool: the tcgen05 / TMEM kernel of
+//      prefill_umma.cu with f16 x f16 MMAs: its two idle warps convert the Q tiles from bf16 to fp16 in shared memory
+//      (exact for normal magnitudes), P is rounded to fp16 instead of bf16.
+// Against PREFILL_FP8 (fp64 on the exact dequantised values) the roundings are fp16's 2^-12 on K, V and P where the
+// bf16 path has 2^-9 on P: the gates of the bf16 path (R11) hold with more margin (R27).
+// Measured and dropped: (i) codes kept exact in the scratch pool and the scales applied in fp32 inside the softmax
+// warps (a page's K scale on its scores, its V scale folded into the exponent): parity green but 50 % slower than the
+// bf16 kernel -- 16 more live registers on warps that already hold a 128-column row, 90 local-memory instructions per
+// stage; (ii) K in fp16 with Q left in bf16: a kind::f16 MMA with operands of two formats faults; (iii) K and V both
+// rounded to bf16: the stacked bf16 roundings of V, P and the output exceed the 1e-2 row gate on rows with few keys
+// (1.0-1.2e-2); (iv) K to bf16, V and P to fp16: inside the gate, but the key rounding alone costs up to 8e-3.
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
@@ -32,42 +40,35 @@ struct ExpandParams {
     const int32_t* seq_lens;
     int32_t S, Hkv, page_size;
     int32_t maxp;       // scratch pages per sequence
-    int32_t sc_stride;  // scale entries per (sequence, kv head): maxp rounded up to 8
-    uint16_t* k16;      // scratch pools [S * maxp][Hkv][page_size][128] bf16
+    uint16_t* k16;      // scratch pools [S * maxp][Hkv][page_size][128] fp16
     uint16_t* v16;
     int32_t* bt16;      // [S][maxp] identity table of the scratch pool
-    float* sc_k;        // [S][Hkv][sc_stride]
-    float* sc_v;
 };
 
-// two E4M3 codes (low 16 bits of w) -> two bf16, exact: e4m3x2 -> f16x2 (exact by definition of the conversion),
-// f16 -> f32 (exact), f32 -> bf16 (exact: four significant bits, exponents within [-9, 8])
-__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2_exact(uint32_t w) {
+// two E4M3 codes (low 16 bits of w) times the page's scale -> two fp16: e4m3x2 -> f16x2 and f16 -> f32 are exact, the
+// fp32 product of a 4-bit and a 24-bit significand is exact, one rounding to fp16 (nearest even, saturating)
+__device__ __forceinline__ uint32_t e4m3x2_dequant_f16x2(uint32_t w, float scale) {
     uint32_t h2;
     asm("{\n\t.reg .b16 lo;\n\tcvt.u16.u32 lo, %1;\n\tcvt.rn.f16x2.e4m3x2 %0, lo;\n\t}" : "=r"(h2) : "r"(w));
     const __half2 h = *reinterpret_cast<const __half2*>(&h2);
     const float2 f = __half22float2(h);
-    return pack_bf16x2(f.x, f.y);
+    uint32_t r;
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(f.y * scale), "f"(f.x * scale));
+    return r;
 }
 
 // One block per (sequence, logical page slot, kv head); 128 threads; K and V.  Thread t takes 16-byte chunk t of the
 // page's page_size x 128 bytes (page 32: two rounds).
 __global__ void __launch_bounds__(128) kv_expand_fp8_kernel(const ExpandParams p) {
-    const int i = blockIdx.x;  // logical page slot, < sc_stride
+    const int i = blockIdx.x;  // logical page of the sequence, < maxp
     const int h = blockIdx.y;
     const int s = blockIdx.z;
     const int L = max(__ldg(p.seq_lens + s), 0);
-    const int npages = (L + p.page_size - 1) / p.page_size;
-    const bool live = i < npages;
-    int32_t page = 0;
-    if (live) page = __ldg(p.block_table + (size_t)s * p.bt_stride + i);
-    if (threadIdx.x == 0) {
-        const size_t o = ((size_t)s * p.Hkv + h) * p.sc_stride + i;
-        p.sc_k[o] = live ? __ldg(p.k_scale + (size_t)page * p.Hkv + h) : 1.f;
-        p.sc_v[o] = live ? __ldg(p.v_scale + (size_t)page * p.Hkv + h) : 1.f;
-        if (h == 0 && i < p.maxp) p.bt16[(size_t)s * p.maxp + i] = s * p.maxp + i;
-    }
-    if (!live) return;
+    if (h == 0 && threadIdx.x == 0) p.bt16[(size_t)s * p.maxp + i] = s * p.maxp + i;
+    if (i >= (L + p.page_size - 1) / p.page_size) return;
+    const int32_t page = __ldg(p.block_table + (size_t)s * p.bt_stride + i);
+    const float ks = __ldg(p.k_scale + (size_t)page * p.Hkv + h);
+    const float vs = __ldg(p.v_scale + (size_t)page * p.Hkv + h);
     const size_t src = (size_t)page * p.stride_page + (size_t)h * p.stride_head;
     const size_t dst = (((size_t)s * p.maxp + i) * p.Hkv + h) * p.page_size * 128;
     for (int c = threadIdx.x; c < p.page_size * 8; c += 128) {
@@ -79,10 +80,10 @@ __global__ void __launch_bounds__(128) kv_expand_fp8_kernel(const ExpandParams p
         uint32_t ko[8], vo[8];
 #pragma unroll
         for (int w = 0; w < 4; ++w) {
-            ko[2 * w] = e4m3x2_to_bf16x2_exact(aw[w] & 0xffffu);
-            ko[2 * w + 1] = e4m3x2_to_bf16x2_exact(aw[w] >> 16);
-            vo[2 * w] = e4m3x2_to_bf16x2_exact(bw[w] & 0xffffu);
-            vo[2 * w + 1] = e4m3x2_to_bf16x2_exact(bw[w] >> 16);
+            ko[2 * w] = e4m3x2_dequant_f16x2(aw[w] & 0xffffu, ks);
+            ko[2 * w + 1] = e4m3x2_dequant_f16x2(aw[w] >> 16, ks);
+            vo[2 * w] = e4m3x2_dequant_f16x2(bw[w] & 0xffffu, vs);
+            vo[2 * w + 1] = e4m3x2_dequant_f16x2(bw[w] >> 16, vs);
         }
         uint4* kd = reinterpret_cast<uint4*>(p.k16 + dst + (size_t)tok * 128 + d0);
         uint4* vd = reinterpret_cast<uint4*>(p.v16 + dst + (size_t)tok * 128 + d0);
@@ -94,8 +95,8 @@ __global__ void __launch_bounds__(128) kv_expand_fp8_kernel(const ExpandParams p
 }
 
 struct Fp8PrefillLayout {
-    size_t plan, k16, v16, bt16, sc_k, sc_v, total;
-    int32_t maxp, sc_stride;
+    size_t plan, k16, v16, bt16, total;
+    int32_t maxp;
 };
 
 static Fp8PrefillLayout fp8_prefill_layout(int32_t S, int32_t total_q, int32_t Hq, int32_t Hkv, int32_t page_size,
@@ -104,15 +105,12 @@ static Fp8PrefillLayout fp8_prefill_layout(int32_t S, int32_t total_q, int32_t H
     auto up = [](size_t x, size_t a) { return (x + a - 1) / a * a; };
     l.maxp = (max_seq_len + page_size - 1) / page_size;
     if (l.maxp < 1) l.maxp = 1;
-    l.sc_stride = (l.maxp + 7) / 8 * 8;
     const size_t pool_bytes = (size_t)S * l.maxp * Hkv * page_size * 128 * 2;
     l.plan = 0;
     l.k16 = up(prefill_umma_workspace_bytes(S, total_q, Hq), 1024);
     l.v16 = up(l.k16 + pool_bytes, 1024);
     l.bt16 = up(l.v16 + pool_bytes, 256);
-    l.sc_k = up(l.bt16 + (size_t)S * l.maxp * 4, 256);
-    l.sc_v = up(l.sc_k + (size_t)S * Hkv * l.sc_stride * 4, 256);
-    l.total = up(l.sc_v + (size_t)S * Hkv * l.sc_stride * 4, 256);
+    l.total = up(l.bt16 + (size_t)S * l.maxp * 4, 256);
     return l;
 }
 
@@ -171,17 +169,14 @@ extern "C" int mstar_paged_attn_prefill_fp8(void* out, float* lse_out, const voi
     e.Hkv = Hkv;
     e.page_size = PAGE;
     e.maxp = l.maxp;
-    e.sc_stride = l.sc_stride;
     e.k16 = reinterpret_cast<uint16_t*>(ws + l.k16);
     e.v16 = reinterpret_cast<uint16_t*>(ws + l.v16);
     e.bt16 = reinterpret_cast<int32_t*>(ws + l.bt16);
-    e.sc_k = reinterpret_cast<float*>(ws + l.sc_k);
-    e.sc_v = reinterpret_cast<float*>(ws + l.sc_v);
-    kv_expand_fp8_kernel<<<dim3((unsigned)l.sc_stride, (unsigned)Hkv, (unsigned)num_seqs), 128, 0, st>>>(e);
+    kv_expand_fp8_kernel<<<dim3((unsigned)l.maxp, (unsigned)Hkv, (unsigned)num_seqs), 128, 0, st>>>(e);
     MSTAR_CUDA_OK(cudaGetLastError());
     launch_count_add(1);
 
-    // the scratch pool as an ordinary bf16 pool
+    // the scratch pool, described like a bf16 pool (16-bit elements; the tensor maps move bytes)
     mstar_kv_pool p16{};
     p16.k_pool = e.k16;
     p16.v_pool = e.v16;
@@ -197,6 +192,6 @@ extern "C" int mstar_paged_attn_prefill_fp8(void* out, float* lse_out, const voi
     if (rc != MSTAR_OK) return rc;
     rc = launch_prefill_umma(maps, q, total_q, cu_seqlens_q, e.bt16, l.maxp, seq_lens, num_seqs, num_q_heads, Hkv, PAGE,
                              max_q_len, scale, causal ? 1 : 0, out, lse_out, (flags & MSTAR_FLAG_OUT_F32) ? 1 : 0, 0,
-                             ws + l.plan, l.k16, st, e.sc_k, e.sc_v, l.sc_stride);
+                             ws + l.plan, l.k16, st, /*kv_f16=*/1);
     return rc;
 }

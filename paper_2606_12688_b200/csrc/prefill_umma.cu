@@ -68,13 +68,6 @@ struct PrefillUmmaParams {
     float* lse;
     int32_t out_f32;
     int32_t causal;
-    // SCALED instantiations (mstar_paged_attn_prefill_fp8): the pool holds the exact bf16 values of E4M3 codes; the
-    // logits of a page's keys take its K scale, its probabilities its V scale.  sc_k / sc_v: [S][Hkv][sc_stride] fp32
-    // by LOGICAL page of the sequence (entries past the last page are 1).
-    const float* sc_k;
-    const float* sc_v;
-    int32_t sc_stride;
-    int32_t Hkv;
 };
 
 
@@ -150,7 +143,7 @@ constexpr int kPuO = 12 * kPuHT;            // 2 tiles x one 64-column half of t
 constexpr int kPuBars = 14 * kPuHT;         // barriers
 enum { B_QFULL0 = 0, B_QFULL1, B_QEMPTY0, B_QEMPTY1, B_KFULL0, B_KFULL1, B_KEMPTY0, B_KEMPTY1, B_VFULL0, B_VFULL1,
        B_VEMPTY0, B_VEMPTY1, B_SFULL0, B_SFULL1, B_PFULL00, B_PFULL01, B_PFULL10, B_PFULL11, B_OFULL0, B_OFULL1,
-       B_OEMPTY0, B_OEMPTY1, B_UFULL0, B_UFULL1, B_UEMPTY0, B_UEMPTY1, B_COUNT };
+       B_OEMPTY0, B_OEMPTY1, B_UFULL0, B_UFULL1, B_UEMPTY0, B_UEMPTY1, B_QCONV0, B_QCONV1, B_COUNT };
 constexpr int kPuDesc = kPuBars + 256;      // 2 unit descriptors (32 B each)
 constexpr int kPuTmemSlot = kPuDesc + 64;
 constexpr int kPuSmemBytes = 14 * kPuHT + 512 + 1024;
@@ -186,7 +179,12 @@ __device__ __forceinline__ PuDesc pu_read_desc(const uint8_t* gbase, int uslot) 
     return d;
 }
 
-template <int PAGE, bool SCALED>
+// F16 (mstar_paged_attn_prefill_fp8): the pool tiles hold fp16 instead of bf16 (the dequantised E4M3 scratch pool).
+// Both operands of a kind::f16 MMA must have one format (a bf16 x f16 instruction raises an illegal-instruction
+// fault, measured), so warps 10 and 11 -- idle in the bf16 kernel -- convert the Q tiles of every unit from bf16 to
+// fp16 in shared memory as soon as they land (exact for |q| in [2^-14, 65504]) and hand them to the MMA warp, and P
+// is rounded to fp16: Q K^T and P V are f16 x f16 MMAs.
+template <int PAGE, bool F16>
 __global__ void __launch_bounds__(kPuThreads, 1)
 prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUtensorMap kmap,
                     const __grid_constant__ CUtensorMap vmap, const __grid_constant__ CUtensorMap omap,
@@ -215,7 +213,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             mbar_init(bar(B_OFULL0 + i), 1);
             mbar_init(bar(B_OEMPTY0 + i), 4);
             mbar_init(bar(B_UFULL0 + i), 1);
-            mbar_init(bar(B_UEMPTY0 + i), 9);  // MMA warp + 8 softmax warps
+            mbar_init(bar(B_UEMPTY0 + i), F16 ? 11 : 9);  // MMA warp + 8 softmax warps (+ 2 Q converters)
+            mbar_init(bar(B_QCONV0 + i), 1);
         }
         fence_mbar_init();
     }
@@ -350,8 +349,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             }
         } else if (warp == kPuMmaWarp) {
             // =============================== MMA ISSUER ===============================
-            const uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
-            const uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
+            const uint32_t fmt = F16 ? 0u : 1u;  // operand format of Q, K, P and V
+            const uint32_t idesc_qk = umma_idesc_f16(128, 128, fmt, fmt, 0, 0);
+            const uint32_t idesc_pv = umma_idesc_f16(128, 128, fmt, fmt, 0, 1);
             uint32_t qph[2] = {0, 0}, kph = 0, vph = 0, pph[2] = {0, 0}, oeph = 0, uph = 0;
             int ks = 0, vs = 0, uslot = 0;
             // Descriptors differ only in the 14-bit start-address field (bytes >> 4) of their low word: the bases are
@@ -399,7 +399,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 mbar_wait(bar(B_KFULL0 + ks), kph);
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
-                    mbar_wait(bar(B_QFULL0 + t), qph[t]);
+                    mbar_wait(bar((F16 ? B_QCONV0 : B_QFULL0) + t), qph[t]);
                     qph[t] ^= 1;
                     tc_fence_after();
                     issue_qk(t, ks);
@@ -455,6 +455,35 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 }
                 oeph ^= 1;
             }
+        } else if (F16) {
+            // =============================== Q CONVERTERS (warps 10, 11; fp16 pool only) ===============================
+            // warp 10 + t: Q tile t of every unit, bf16 -> fp16 in place (the conversion is elementwise, so the
+            // swizzled layout does not matter), then a fence towards the tensor core's proxy and the hand-over
+            const int t = warp - 10;
+            uint32_t qph = 0, uph = 0;
+            int uslot = 0;
+            while (true) {
+                mbar_wait(bar(B_UFULL0 + uslot), uph);
+                const PuDesc x = pu_read_desc(gbase, uslot);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_UEMPTY0 + uslot));
+                uslot ^= 1;
+                if (uslot == 0) uph ^= 1;
+                if (x.T == 0) break;
+                mbar_wait(bar(B_QFULL0 + t), qph);
+                qph ^= 1;
+                const uint32_t qt = base + kPuQ + t * 2 * kPuHT;
+#pragma unroll 4
+                for (int c = lane; c < 2 * kPuHT / 16; c += 32) {
+                    uint32_t w0, w1, w2, w3;
+                    ld_shared_v4(qt + c * 16, w0, w1, w2, w3);
+                    st_shared_v4(qt + c * 16, bf16x2_to_f16x2(w0), bf16x2_to_f16x2(w1), bf16x2_to_f16x2(w2),
+                                 bf16x2_to_f16x2(w3));
+                }
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_QCONV0 + t));
+            }
         }
     } else {
         // =============================== SOFTMAX / EPILOGUE WARPGROUPS ===============================
@@ -481,13 +510,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             // last visible KV position of this row (rows that are not stored follow the unit bound)
             const int lim = p.causal ? min(x.P + tok, x.kv_end - 1) : x.kv_end - 1;
             float m_ref = -INFINITY, l = 0.f;
-            const float* sc_ku = nullptr;
-            const float* sc_vu = nullptr;
-            if constexpr (SCALED) {
-                const size_t o = ((size_t)x.s * p.Hkv + x.kvh) * p.sc_stride;
-                sc_ku = p.sc_k + o;
-                sc_vu = p.sc_v + o;
-            }
             for (int j = 0; j < x.T; ++j) {
                 const int j0 = j * kPuTok;
                 mbar_wait(bar(B_SFULL0 + t), sph);
@@ -505,20 +527,6 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     tmem_ld_32x32b_x32(s_addr + 96, r3);
                     tmem_wait_ld();
                 }
-                // SCALED: the stage's PPS consecutive logical pages.  A page's K scale multiplies the raw scores of
-                // its keys: it goes into the page's maximum and into the multiplier of the exponent's FFMA.  Its V
-                // scale multiplies the probabilities P V sees: log2 of it goes into the FFMA's addend, and the row
-                // sum, which wants the unscaled probabilities, divides each page's partial sum by it.
-                float ksc[PPS], vsc[PPS];
-                if constexpr (SCALED) {
-#pragma unroll
-                    for (int i = 0; i < PPS; i += 4) {
-                        const float4 a = __ldg(reinterpret_cast<const float4*>(sc_ku + j * PPS + i));
-                        const float4 b = __ldg(reinterpret_cast<const float4*>(sc_vu + j * PPS + i));
-                        ksc[i] = a.x; ksc[i + 1] = a.y; ksc[i + 2] = a.z; ksc[i + 3] = a.w;
-                        vsc[i] = b.x; vsc[i + 1] = b.y; vsc[i + 2] = b.z; vsc[i + 3] = b.w;
-                    }
-                }
                 // ---- mask (diagonal / last stages only; warp-uniform branch)
                 if (__any_sync(0xffffffffu, j0 + kPuTok - 1 > lim)) {
                     const int rel = lim - j0;  // columns i > rel are invisible to this row
@@ -526,41 +534,21 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     for (int i = 0; i < 128; ++i)
                         if (i > rel) r[i] = 0xff800000u;  // -inf
                 }
-                float mx;
-                if constexpr (SCALED) {
-                    // ---- row max of the scaled scores: maximum of every page's raw scores times the page's K scale
-                    mx = -INFINITY;
+                // ---- row max (3-input max, four chains)
+                float mx0 = fmax3(__uint_as_float(r[0]), __uint_as_float(r[1]), __uint_as_float(r[2]));
+                float mx1 = fmax3(__uint_as_float(r[3]), __uint_as_float(r[4]), __uint_as_float(r[5]));
+                float mx2 = fmax3(__uint_as_float(r[6]), __uint_as_float(r[7]), __uint_as_float(r[8]));
+                float mx3 = fmax3(__uint_as_float(r[9]), __uint_as_float(r[10]), __uint_as_float(r[11]));
 #pragma unroll
-                    for (int g = 0; g < PPS; ++g) {
-                        float a0 = fmax3(__uint_as_float(r[g * PAGE]), __uint_as_float(r[g * PAGE + 1]),
-                                         __uint_as_float(r[g * PAGE + 2]));
-                        float a1 = fmax3(__uint_as_float(r[g * PAGE + 3]), __uint_as_float(r[g * PAGE + 4]),
-                                         __uint_as_float(r[g * PAGE + 5]));
-#pragma unroll
-                        for (int i = 6; i < PAGE - 2; i += 4) {
-                            a0 = fmax3(a0, __uint_as_float(r[g * PAGE + i]), __uint_as_float(r[g * PAGE + i + 1]));
-                            a1 = fmax3(a1, __uint_as_float(r[g * PAGE + i + 2]), __uint_as_float(r[g * PAGE + i + 3]));
-                        }
-                        a0 = fmax3(a0, __uint_as_float(r[g * PAGE + PAGE - 2]), __uint_as_float(r[g * PAGE + PAGE - 1]));
-                        mx = fmaxf(mx, fmaxf(a0, a1) * ksc[g]);
-                    }
-                } else {
-                    // ---- row max (3-input max, four chains)
-                    float mx0 = fmax3(__uint_as_float(r[0]), __uint_as_float(r[1]), __uint_as_float(r[2]));
-                    float mx1 = fmax3(__uint_as_float(r[3]), __uint_as_float(r[4]), __uint_as_float(r[5]));
-                    float mx2 = fmax3(__uint_as_float(r[6]), __uint_as_float(r[7]), __uint_as_float(r[8]));
-                    float mx3 = fmax3(__uint_as_float(r[9]), __uint_as_float(r[10]), __uint_as_float(r[11]));
-    #pragma unroll
-                    for (int i = 12; i < 124; i += 8) {
-                        mx0 = fmax3(mx0, __uint_as_float(r[i]), __uint_as_float(r[i + 1]));
-                        mx1 = fmax3(mx1, __uint_as_float(r[i + 2]), __uint_as_float(r[i + 3]));
-                        mx2 = fmax3(mx2, __uint_as_float(r[i + 4]), __uint_as_float(r[i + 5]));
-                        mx3 = fmax3(mx3, __uint_as_float(r[i + 6]), __uint_as_float(r[i + 7]));
-                    }
-                    mx0 = fmax3(mx0, __uint_as_float(r[124]), __uint_as_float(r[125]));
-                    mx1 = fmax3(mx1, __uint_as_float(r[126]), __uint_as_float(r[127]));
-                    mx = fmax3(fmaxf(mx0, mx1), mx2, mx3);
+                for (int i = 12; i < 124; i += 8) {
+                    mx0 = fmax3(mx0, __uint_as_float(r[i]), __uint_as_float(r[i + 1]));
+                    mx1 = fmax3(mx1, __uint_as_float(r[i + 2]), __uint_as_float(r[i + 3]));
+                    mx2 = fmax3(mx2, __uint_as_float(r[i + 4]), __uint_as_float(r[i + 5]));
+                    mx3 = fmax3(mx3, __uint_as_float(r[i + 6]), __uint_as_float(r[i + 7]));
                 }
+                mx0 = fmax3(mx0, __uint_as_float(r[124]), __uint_as_float(r[125]));
+                mx1 = fmax3(mx1, __uint_as_float(r[126]), __uint_as_float(r[127]));
+                const float mx = fmax3(fmaxf(mx0, mx1), mx2, mx3);
                 // ---- running max with lazy rescale of O (TMEM) and l
                 if (j == 0) {
                     m_ref = mx;
@@ -589,27 +577,16 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 // ---- p = 2^(s*c - m_ref*c), P -> bf16 -> TMEM (over the columns of S), handed over in two parts:
                 // the first kPuSplit keys, then the rest, so that little P V work is left after the last hand-off
                 const float nmc = -m_ref * c;
-                float ck[PPS], nk[PPS];
-                if constexpr (SCALED) {
-#pragma unroll
-                    for (int g = 0; g < PPS; ++g) {
-                        ck[g] = c * ksc[g];
-                        nk[g] = nmc + log2f(vsc[g]);
-                    }
-                }
                 {
                     uint32_t pk[kPuSplit / 2];
 #pragma unroll
                     for (int i = 0; i < kPuSplit; i += 2) {
                         float x0, x1;
-                        if constexpr (SCALED)
-                            ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), ck[i / PAGE], nk[i / PAGE]);
-                        else
-                            ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), c, nmc);
+                        ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), c, nmc);
                         const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
                         r[i] = __float_as_uint(p0);
                         r[i + 1] = __float_as_uint(p1);
-                        pk[i >> 1] = pack_bf16x2(p0, p1);
+                        pk[i >> 1] = F16 ? pack_f16x2(p0, p1) : pack_bf16x2(p0, p1);
                     }
                     tmem_st_32x32b_x32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
                     tmem_st_32x32b_x16(s_addr + 32, *reinterpret_cast<uint32_t(*)[16]>(&pk[32]));
@@ -623,14 +600,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
 #pragma unroll
                     for (int i = kPuSplit; i < 128; i += 2) {
                         float x0, x1;
-                        if constexpr (SCALED)
-                            ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), ck[i / PAGE], nk[i / PAGE]);
-                        else
-                            ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), c, nmc);
+                        ffma2_bcast(x0, x1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]), c, nmc);
                         const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
                         r[i] = __float_as_uint(p0);
                         r[i + 1] = __float_as_uint(p1);
-                        pk[(i - kPuSplit) >> 1] = pack_bf16x2(p0, p1);
+                        pk[(i - kPuSplit) >> 1] = F16 ? pack_f16x2(p0, p1) : pack_bf16x2(p0, p1);
                     }
                     tmem_st_32x32b_x16(s_addr + kPuSplit / 2, pk);
                     tmem_wait_st();
@@ -638,35 +612,15 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(B_PFULL00 + 2 * t + 1));
                 }
-                if constexpr (SCALED) {
-                    // ---- row sum of the UNSCALED probabilities: every page's partial sum over its V scale
+                // ---- row sum, after the hand-off (packed adds, four chains)
+                float s0 = __uint_as_float(r[0]), s1 = __uint_as_float(r[1]);
+                float s2 = __uint_as_float(r[2]), s3 = __uint_as_float(r[3]);
 #pragma unroll
-                    for (int g = 0; g < PPS; ++g) {
-                        if ((g & 3) == 0) {  // re-read (L1 hit): not kept in registers across the exponentials
-                            const float4 b = __ldg(reinterpret_cast<const float4*>(sc_vu + j * PPS + g));
-                            vsc[g] = b.x; vsc[g + 1] = b.y; vsc[g + 2] = b.z; vsc[g + 3] = b.w;
-                        }
-                        float s0 = __uint_as_float(r[g * PAGE]), s1 = __uint_as_float(r[g * PAGE + 1]);
-                        float s2 = __uint_as_float(r[g * PAGE + 2]), s3 = __uint_as_float(r[g * PAGE + 3]);
-#pragma unroll
-                        for (int i = 4; i < PAGE; i += 4) {
-                            fadd2(s0, s1, s0, s1, __uint_as_float(r[g * PAGE + i]), __uint_as_float(r[g * PAGE + i + 1]));
-                            fadd2(s2, s3, s2, s3, __uint_as_float(r[g * PAGE + i + 2]),
-                                  __uint_as_float(r[g * PAGE + i + 3]));
-                        }
-                        l += __fdividef((s0 + s1) + (s2 + s3), vsc[g]);
-                    }
-                } else {
-                    // ---- row sum, after the hand-off (packed adds, four chains)
-                    float s0 = __uint_as_float(r[0]), s1 = __uint_as_float(r[1]);
-                    float s2 = __uint_as_float(r[2]), s3 = __uint_as_float(r[3]);
-    #pragma unroll
-                    for (int i = 4; i < 128; i += 4) {
-                        fadd2(s0, s1, s0, s1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]));
-                        fadd2(s2, s3, s2, s3, __uint_as_float(r[i + 2]), __uint_as_float(r[i + 3]));
-                    }
-                    l += (s0 + s1) + (s2 + s3);
+                for (int i = 4; i < 128; i += 4) {
+                    fadd2(s0, s1, s0, s1, __uint_as_float(r[i]), __uint_as_float(r[i + 1]));
+                    fadd2(s2, s3, s2, s3, __uint_as_float(r[i + 2]), __uint_as_float(r[i + 3]));
                 }
+                l += (s0 + s1) + (s2 + s3);
             }
             // ---- epilogue: O / l -> out
             mbar_wait(bar(B_OFULL0 + t), oph);
@@ -789,13 +743,8 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
                         const int32_t* block_table, int64_t bt_stride, const int32_t* seq_lens, int32_t S,
                         int32_t Hq, int32_t Hkv, int32_t page_size, int32_t max_q_len, float scale, int32_t causal,
                         void* out, float* lse, int32_t out_f32, int32_t reuse_plan, void* workspace,
-                        size_t workspace_bytes, cudaStream_t stream, const float* sc_k, const float* sc_v,
-                        int32_t sc_stride) {
+                        size_t workspace_bytes, cudaStream_t stream, int32_t kv_f16) {
     PrefillUmmaParams p{};
-    p.sc_k = sc_k;
-    p.sc_v = sc_v;
-    p.sc_stride = sc_stride;
-    p.Hkv = Hkv;
     p.block_table = block_table;
     p.bt_stride = bt_stride;
     p.plan = reinterpret_cast<int32_t*>(workspace);
@@ -832,12 +781,11 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
     int grid = device_sm_count();
     if (grid > max_units) grid = (int)max_units;
     if (grid < 1) grid = 1;
-    const bool scaled = sc_k != nullptr;
-    auto k16 = scaled ? prefill_umma_kernel<16, true> : prefill_umma_kernel<16, false>;
-    auto k32 = scaled ? prefill_umma_kernel<32, true> : prefill_umma_kernel<32, false>;
-    static PerDeviceOnce once16, once32, once16s, once32s;
-    MSTAR_CUDA_OK(set_max_dynamic_smem(scaled ? once16s : once16, k16, kPuSmemBytes));
-    MSTAR_CUDA_OK(set_max_dynamic_smem(scaled ? once32s : once32, k32, kPuSmemBytes));
+    auto k16 = kv_f16 ? prefill_umma_kernel<16, true> : prefill_umma_kernel<16, false>;
+    auto k32 = kv_f16 ? prefill_umma_kernel<32, true> : prefill_umma_kernel<32, false>;
+    static PerDeviceOnce once16, once32, once16h, once32h;
+    MSTAR_CUDA_OK(set_max_dynamic_smem(kv_f16 ? once16h : once16, k16, kPuSmemBytes));
+    MSTAR_CUDA_OK(set_max_dynamic_smem(kv_f16 ? once32h : once32, k32, kPuSmemBytes));
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3(kPuThreads);

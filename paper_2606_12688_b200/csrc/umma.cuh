@@ -41,9 +41,14 @@ __device__ __forceinline__ uint64_t umma_desc_mnmajor_sw128(uint32_t addr, uint3
     return (uint64_t)((addr >> 4) & 0x3fffu) | ((uint64_t)((mn_stride_bytes >> 4) & 0x3fffu) << 16) |
            ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
 }
-__device__ __forceinline__ uint32_t umma_idesc_bf16(uint32_t M, uint32_t N, uint32_t a_mn_major, uint32_t b_mn_major) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | (a_mn_major << 15) | (b_mn_major << 16) | ((N >> 3) << 17) |
+// a_fmt / b_fmt: 1 = bf16, 0 = f16 (the two operands of a kind::f16 MMA carry their formats separately)
+__device__ __forceinline__ uint32_t umma_idesc_f16(uint32_t M, uint32_t N, uint32_t a_fmt, uint32_t b_fmt,
+                                                   uint32_t a_mn_major, uint32_t b_mn_major) {
+    return (1u << 4) | (a_fmt << 7) | (b_fmt << 10) | (a_mn_major << 15) | (b_mn_major << 16) | ((N >> 3) << 17) |
            ((M >> 4) << 24);
+}
+__device__ __forceinline__ uint32_t umma_idesc_bf16(uint32_t M, uint32_t N, uint32_t a_mn_major, uint32_t b_mn_major) {
+    return umma_idesc_f16(M, N, 1u, 1u, a_mn_major, b_mn_major);
 }
 
 // ---------------------------------------------------------------- MMA issue (one thread)
