@@ -39,11 +39,40 @@ if ROOT not in sys.path:
 METRIC = "paged_decode_attn_GBps"
 UNIT = "GB/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r1f_full_summary.csv: split-K read + write, combine read; prefill read + write); valid for the
-# full-size workloads only.
-NCU_TRAFFIC = {"decode": 2147743000 + 5533952 + 4272000, "prefill": 87985000 + 12952064,
-               "source": "profiles/r1f_full_summary.csv"}
+# `traffic` of the roofline blocks: dram__bytes_read.sum + dram__bytes_write.sum per launch, read at run time from
+# the committed summary of the `ncu --set full` capture (profiles/, one row per kernel of a whole step); valid for the
+# full-size workloads only, None when the file or a row is missing.
+NCU_SUMMARY = os.path.join("profiles", "r2_full_summary.csv")
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+
+
+def load_ncu_traffic(path=None):
+    """{'decode': bytes, 'prefill': bytes, 'source': file} from the summary CSV (header row, unit row, data rows)."""
+    import csv
+    path = os.path.join(ROOT, NCU_SUMMARY) if path is None else path
+    out = {"decode": None, "prefill": None, "source": None}
+    try:
+        with open(path, newline="") as f:
+            rows = list(csv.reader(f))
+        head, units = rows[0], rows[1]
+        ik, ir, iw = head.index("Kernel Name"), head.index("dram__bytes_read.sum"), head.index("dram__bytes_write.sum")
+
+        def traffic(row):
+            return float(row[ir]) * _UNIT[units[ir]] + float(row[iw]) * _UNIT[units[iw]]
+
+        def first(sub):
+            for r in rows[2:]:
+                if sub in r[ik]:
+                    return traffic(r)
+            return None
+        sk, cb = first("decode_splitk_kernel<128, 32, 8, 0, 4"), first("decode_combine_kernel")
+        out["decode"] = None if sk is None or cb is None else int(sk + cb)
+        pf = first("prefill_umma_kernel<16")
+        out["prefill"] = None if pf is None else int(pf)
+        out["source"] = os.path.relpath(path, ROOT)
+    except Exception:
+        pass
+    return out
 
 
 def load_peaks():
@@ -451,6 +480,7 @@ def run_ours(args):
     import workloads as W
     mstar.load_library()
     peaks = load_peaks()
+    ncu_traffic = load_ncu_traffic()
 
     # ---- inputs (seeded, host-generated, uploaded once)
     free, _ = torch.cuda.mem_get_info()
@@ -618,14 +648,14 @@ def run_ours(args):
         "roofline": {"kernel": "decode_splitk_kernel + decode_combine_kernel (one mstar_paged_attn_decode call)",
                      "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak, "unit": "GB/s",
                      "frac": dec_gbs / hbm_peak,
-                     "traffic": NCU_TRAFFIC["decode"] if pool_pages == 491520 else None,
-                     "traffic_source": NCU_TRAFFIC["source"], "peak_source": peaks["source"],
+                     "traffic": ncu_traffic["decode"] if pool_pages == 491520 else None,
+                     "traffic_source": ncu_traffic["source"], "peak_source": peaks["source"],
                      "frac_of_nominal_8TBps": dec_gbs / 8000.0, "ms": t_dec_max, "bytes": dec_bytes,
                      "hbm_read_ceiling": read_ceiling,
                      "frac_of_read_ceiling": (dec_gbs / read_ceiling["GBps"]) if read_ceiling else None},
         "roofline_prefill": {"kernel": "prefill kernel (one mstar_paged_attn_prefill call)", "bound": "tensor",
                              "achieved": pre_tfs, "peak": tf_peak, "unit": "TFLOP/s", "frac": pre_tfs / tf_peak,
-                             "traffic": NCU_TRAFFIC["prefill"], "traffic_source": NCU_TRAFFIC["source"],
+                             "traffic": ncu_traffic["prefill"], "traffic_source": ncu_traffic["source"],
                              "peak_source": peaks["source"] + ", burst",
                              "frac_of_sustained": pre_tfs / peaks["bf16_tflops_sustained"],
                              "frac_of_nominal_2250": pre_tfs / 2250.0, "ms": t_pre_max, "flops": flops},
@@ -659,7 +689,26 @@ def main(argv=None):
     args = ap.parse_args(argv)
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: become N ranks (one per GPU) under torchrun on this node
+        return respawn_under_torchrun(args.gpus, sys.argv[1:] if argv is None else list(argv))
     return run_ours(args)
+
+
+def torchrun_command(n_gpus: int, argv, port=None):
+    """The command line `python bench.py --gpus N` turns itself into when it is not already under torchrun."""
+    if port is None:
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n_gpus),
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
+
+
+def respawn_under_torchrun(n_gpus: int, argv):
+    import subprocess
+    return subprocess.call(torchrun_command(n_gpus, argv))
 
 
 if __name__ == "__main__":

@@ -1,6 +1,7 @@
 """Build ``libmstar_attn.so`` (and the bench-only ``bench_aux/libmstar_benchaux.so``) in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_2606_12688_b200.build [--force] [--verbose]
+    python -m paper_2606_12688_b200.build --sass-counts      # per-kernel counts of the Blackwell SASS mnemonics (markdown)
 
 The shared library travels to the GPU box with the repo snapshot; nothing is JIT-compiled there.
 """
@@ -79,5 +80,45 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     return LIB_PATH
 
 
+SASS_MNEMONICS = ["UTCHMMA", "UTCQMMA", "LDTM", "STTM", "UTMALDG", "UTMASTG", "UBLKCP", "UTCBAR", "HMMA", "LDSM",
+                  "MUFU.EX2", "SYNCS", "STL", "LDL"]
+
+
+def sass_counts() -> str:
+    """Markdown table: how often each mnemonic of interest occurs in every kernel of the built library
+    (`cuobjdump -sass`; the evidence table of B200_PROFILING.md: tcgen05.mma = UTC*MMA, tcgen05.ld/st = LDTM/STTM,
+    TMA = UTMALDG/UTMASTG/UBLKCP, mma.sync = HMMA; STL/LDL = register spills)."""
+    import re
+    build_library()
+    cuobjdump = os.path.join(os.environ.get("CUDA_HOME", "/usr/local/cuda"), "bin", "cuobjdump")
+    out = subprocess.run([cuobjdump, "-sass", LIB_PATH], capture_output=True, text=True, check=True).stdout
+    demangle = os.path.join(os.environ.get("CUDA_HOME", "/usr/local/cuda"), "bin", "cu++filt")
+    rows, name, counts = [], None, None
+    for line in out.splitlines():
+        m = re.match(r"\s*Function : (\S+)", line)
+        if m:
+            if name:
+                rows.append((name, counts))
+            name, counts = m.group(1), dict.fromkeys(SASS_MNEMONICS, 0)
+            continue
+        if name and re.match(r"\s+/\*[0-9a-f]{4,}\*/", line):
+            body = line.split("*/", 1)[1]
+            for mn in SASS_MNEMONICS:
+                if re.search(r"(?<![A-Z0-9_.])" + re.escape(mn) + r"(?![A-Z0-9_])", body):
+                    counts[mn] += 1
+    if name:
+        rows.append((name, counts))
+    names = subprocess.run([demangle] + [r[0] for r in rows], capture_output=True, text=True).stdout.splitlines()
+    lines = ["| kernel | " + " | ".join(SASS_MNEMONICS) + " |", "|---|" + "---|" * len(SASS_MNEMONICS)]
+    for (_, c), nm in sorted(zip(rows, names), key=lambda x: x[1]):
+        short = nm[:nm.index(">(") + 1] if ">(" in nm else nm.split("(")[0]
+        short = short.replace("mstar::", "").replace("void ", "").replace("(int)", "").replace("(bool)", "")
+        lines.append("| `%s` | " % short + " | ".join(str(c[m]) for m in SASS_MNEMONICS) + " |")
+    return "\n".join(lines)
+
+
 if __name__ == "__main__":
-    print(build_library(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--sass-counts" in sys.argv:
+        print(sass_counts())
+    else:
+        print(build_library(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

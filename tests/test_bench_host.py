@@ -75,3 +75,35 @@ def test_reference_arm_prints_contract_line():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference"],
                          env=dict(env, RANK="1", WORLD_SIZE="2"), capture_output=True, text=True, timeout=60)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_gpus_flag_respawns_under_torchrun(monkeypatch):
+    """`python bench.py --gpus N` without torchrun becomes N ranks (one per GPU) on this node; under torchrun
+    (WORLD_SIZE set) it runs as the rank it is."""
+    import bench
+    cmd = bench.torchrun_command(4, ["--gpus", "4", "--steps", "3"], port=29999)
+    assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node" in cmd
+    assert cmd[cmd.index("--nproc-per-node") + 1] == "4" and cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
+    assert cmd[-5:] == [os.path.join(ROOT, "bench.py"), "--gpus", "4", "--steps", "3"]
+    seen = {}
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    monkeypatch.setattr(bench, "respawn_under_torchrun", lambda n, argv: seen.update(n=n, argv=argv) or 0)
+    monkeypatch.setattr(bench, "run_ours", lambda args: seen.update(direct=args.gpus) or 0)
+    assert bench.main(["--gpus", "2", "--steps", "1"]) == 0 and seen == {"n": 2, "argv": ["--gpus", "2", "--steps", "1"]}
+    seen.clear()
+    monkeypatch.setenv("WORLD_SIZE", "2")
+    assert bench.main(["--gpus", "2"]) == 0 and seen == {"direct": 2}
+    seen.clear()
+    monkeypatch.delenv("WORLD_SIZE")
+    assert bench.main(["--gpus", "1"]) == 0 and seen == {"direct": 1}
+
+
+def test_ncu_traffic_is_read_from_the_committed_summary(tmp_path):
+    import bench
+    f = tmp_path / "s.csv"
+    f.write_text('Kernel Name,gpu__time_duration.sum,dram__bytes_read.sum,dram__bytes_write.sum\n,us,Gbyte,Mbyte\n'
+                 '"void prefill_umma_kernel<16, 0>(X)",1,0.5,2\n'
+                 '"void decode_splitk_kernel<128, 32, 8, 0, 4, 1>(X)",1,2,1\n"void decode_combine_kernel<128>(X)",1,0.004,0\n')
+    t = bench.load_ncu_traffic(str(f))
+    assert t["prefill"] == 502000000 and t["decode"] == 2005000000
+    assert bench.load_ncu_traffic(str(tmp_path / "missing.csv"))["decode"] is None
