@@ -460,6 +460,29 @@ def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15
     res["fp8 pool (SURVEY 8(f) rank 4): configs[2] causal prefill"] = fp8_prefill_entry(W.config3_prefill(), True, 84,
                                                                                          bf16_peak)
     res["fp8 pool (SURVEY 8(f) rank 4): flow step, causal = 0"] = fp8_prefill_entry(bf, False, 85, bf16_peak)
+    # SURVEY 8(f) rank 4, last clause: CUDA-graph-compatible sampling, 64 rows over a 151 936-entry vocabulary
+    def sampling_entry(dtype, use_filters):
+        Bs, Vs = 64, 151936
+        g = torch.Generator(device=dev)
+        g.manual_seed(5)
+        lg = (torch.randn((Bs, Vs), device=dev, generator=g) * 3.0).to(dtype)
+        seeds = torch.arange(Bs, dtype=torch.int64, device=dev) + 1000
+        step = torch.zeros(1, dtype=torch.int64, device=dev)
+        tk = torch.full((Bs,), 50 if use_filters else 0, dtype=torch.int32, device=dev)
+        tp = torch.full((Bs,), 0.9 if use_filters else 1.0, dtype=torch.float32, device=dev)
+        tt = torch.full((Bs,), 0.8, dtype=torch.float32, device=dev)
+        tok = torch.empty(Bs, dtype=torch.int32, device=dev)
+        ms = median_ms([lambda: mstar.sample_tokens(tok, lg, seeds, step, temperature=tt, top_k=tk, top_p=tp,
+                                                    advance_step=True)])
+        nbytes = Bs * Vs * lg.element_size()
+        return {"rows": Bs, "vocab": Vs, "logits": str(dtype).split(".")[-1], "top_k": int(tk[0]),
+                "top_p": float(tp[0]), "us": ms * 1e3, "tokens_per_s": Bs / (ms * 1e-3),
+                "logit_bytes": nbytes, "GBps_one_read_of_the_logits": nbytes / (ms * 1e-3) / 1e9,
+                "passes_over_the_row": 21 if use_filters else 4}
+
+    res["sampling (SURVEY 8(f) rank 4): temperature only, fp32 logits"] = sampling_entry(torch.float32, False)
+    res["sampling (SURVEY 8(f) rank 4): top-k 50 + top-p 0.9, fp32 logits"] = sampling_entry(torch.float32, True)
+    res["sampling (SURVEY 8(f) rank 4): top-k 50 + top-p 0.9, bf16 logits"] = sampling_entry(torch.bfloat16, True)
     res["fp8 pool (SURVEY 8(f) rank 4): configs[1] decode"] = fp8_entry(b2, 0, 81)
     res["fp8 pool (SURVEY 8(f) rank 4): configs[3] thinker decode"] = fp8_entry(bt, 0, 82)
     if b_long is not None:

@@ -59,6 +59,10 @@ typedef enum {
                                           for the SAME cu_seqlens_q, seq_lens, head geometry and causal flag (the
                                           next layer of the same forward pass): skip the plan kernel. */
 
+#define MSTAR_FLAG_LOGITS_BF16 8u          /* mstar_sample_tokens only: `logits` is bf16 instead of fp32 */
+#define MSTAR_FLAG_SAMPLE_ADVANCE_STEP 16u /* mstar_sample_tokens only: add 1 to *step behind the sampling kernel, so
+                                              that every replay of a captured graph draws fresh numbers */
+
 /*
  * The paged K/V pool ("a single paged KV pool").  Caller-owned device memory, bf16.
  * Element (page, kv_head, token_in_page, d) of K lives at
@@ -270,6 +274,31 @@ int mstar_paged_attn_prefill(void* out, float* lse_out, const void* q, const int
                              int32_t total_q, int32_t max_q_len, int32_t max_seq_len,
                              int32_t num_q_heads, float scale, int32_t causal, uint32_t flags,
                              void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * mstar_sample_tokens (last clause): the "cuda-graph-compatible sampling plugin" of the
+ * KVCacheEngine.  One token per row from softmax(logits / temperature) restricted by top-k and
+ * top-p, drawn with one uniform number per row; all state is device memory, the call only enqueues, so it can be
+ * captured and replayed.  Definition (R28, oracle/sampling.py):
+ *   z = logits / T.  top-k (0 < k < vocab): keep the tokens with z >= the k-th largest z (ties kept).  top-p
+ *   (0 < p < 1): of the kept tokens in descending probability, the shortest prefix of mass >= p, ties with its last
+ *   token kept.  u = (x + 1/2) / 2^32 with x = word 0 of Philox4x32-10, counter (step mod 2^32, step div 2^32, row, 0),
+ *   key (seed mod 2^32, seed div 2^32).  Token = the first kept index whose running sum of probabilities (index order)
+ *   exceeds u times the kept mass.  T = 0: the argmax of the row (lowest index among equals).
+ *   tokens_out   device, [num_rows] int32
+ *   logits       device, [num_rows][row_stride] fp32 (bf16 with MSTAR_FLAG_LOGITS_BF16), vocab <= row_stride; NaN
+ *                entries: undefined; -inf entries never win
+ *   temperature  device, [num_rows] fp32 >= 0, or NULL (= 1)
+ *   top_k        device, [num_rows] int32 (<= 0 or >= vocab: off), or NULL
+ *   top_p        device, [num_rows] fp32 (<= 0 or >= 1: off), or NULL
+ *   seeds        device, [num_rows] uint64;  step: device, one uint64 shared by the rows
+ * Probabilities are fixed-point (floor(2^32 * exp(z - z_max)), exponential in fp32) and all sums are integers, so the
+ * result is run-to-run deterministic; against the fp64 definition a token is correct when u lies within rounding
+ * (1e-5) of its interval of the running sum.
+ */
+int mstar_sample_tokens(int32_t* tokens_out, const void* logits, int64_t row_stride, int32_t num_rows, int32_t vocab,
+                        const float* temperature, const int32_t* top_k, const float* top_p, const uint64_t* seeds,
+                        uint64_t* step, uint32_t flags, void* stream);
 
 /*
  * mstar_build_slot_mapping: device-side helper so that append -> prefill stays graph-capturable.

@@ -13,6 +13,7 @@ Python binding.  Names mirror the C entry points:
     kv_copy_pages        <- mstar_kv_copy_pages       (page moves pool -> pool)
     kv_gather            <- mstar_kv_gather           (pool -> contiguous rows)
     merge_attn_states    <- mstar_merge_attn_states   (LSE merge of two attention states)
+    sample_tokens        <- mstar_sample_tokens       (CUDA-graph-compatible temperature / top-k / top-p sampling)
     paged_attn_decode_cascade <- mstar_paged_attn_decode_cascade (CFG branches sharing prefix pages, one call)
 
 There is no CPU fallback: without the built library every call raises ``MstarError``.
@@ -22,6 +23,7 @@ from .binding import (  # noqa: F401
     KVPool,
     KVPoolFp8,
     LIB_PATH,
+    MSTAR_FLAG_LOGITS_BF16,
     MSTAR_FLAG_OUT_F32,
     MSTAR_FLAG_PREFILL_MMA_SYNC,
     MSTAR_FLAG_PREFILL_REUSE_PLAN,
@@ -44,6 +46,7 @@ from .binding import (  # noqa: F401
     paged_attn_prefill_fp8,
     prefill_fp8_workspace_bytes,
     prefill_workspace_bytes,
+    sample_tokens,
     status_string,
     version,
 )

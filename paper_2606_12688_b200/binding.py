@@ -20,6 +20,8 @@ MSTAR_OK = 0
 MSTAR_FLAG_OUT_F32 = 1
 MSTAR_FLAG_PREFILL_MMA_SYNC = 2
 MSTAR_FLAG_PREFILL_REUSE_PLAN = 4
+MSTAR_FLAG_LOGITS_BF16 = 8
+MSTAR_FLAG_SAMPLE_ADVANCE_STEP = 16
 
 EXPORTS = (
     "mstar_kv_append",
@@ -38,6 +40,7 @@ EXPORTS = (
     "mstar_paged_attn_prefill_workspace_bytes",
     "mstar_paged_attn_prefill",
     "mstar_build_slot_mapping",
+    "mstar_sample_tokens",
     "mstar_last_launch_count",
     "mstar_status_string",
     "mstar_version",
@@ -94,6 +97,9 @@ def load_library() -> ctypes.CDLL:
         c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p, c.c_void_p,
         c.c_int64, c.c_void_p, c.c_int32, c.c_int32, c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_int32,
         c.c_uint32, c.c_void_p, c.c_size_t, c.c_void_p]
+    lib.mstar_sample_tokens.restype = c.c_int
+    lib.mstar_sample_tokens.argtypes = [c.c_void_p, c.c_void_p, c.c_int64, c.c_int32, c.c_int32, c.c_void_p,
+                                        c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_uint32, c.c_void_p]
     lib.mstar_kv_copy_pages.restype = c.c_int
     lib.mstar_kv_copy_pages.argtypes = [c.POINTER(_KvPoolStruct), c.POINTER(_KvPoolStruct), c.c_void_p, c.c_void_p,
                                         c.c_int64, c.c_void_p]
@@ -448,6 +454,34 @@ def paged_attn_prefill_fp8(out: torch.Tensor, q: torch.Tensor, cu_seqlens_q: tor
         _ptr(pool.v_scale), _ptr(block_table), int(block_table.stride(0)) if block_table.dim() == 2 else 0,
         _ptr(seq_lens), S, T, int(max_q_len), int(max_seq_len), Hq, float(scale), 1 if causal else 0, flags,
         _ptr(workspace), ws_bytes, _stream()), "mstar_paged_attn_prefill_fp8")
+
+
+def sample_tokens(tokens_out: torch.Tensor, logits: torch.Tensor, seeds: torch.Tensor, step: torch.Tensor,
+                  temperature: Optional[torch.Tensor] = None, top_k: Optional[torch.Tensor] = None,
+                  top_p: Optional[torch.Tensor] = None, advance_step: bool = False) -> None:
+    """mstar_sample_tokens.  logits [B, V] fp32 or bf16 (unit inner stride); seeds [B] int64 bit patterns of the
+    uint64 keys; step: one int64 on the device (the uint64 counter)."""
+    if logits.dim() != 2 or logits.stride(1) != 1 or not logits.is_cuda:
+        raise MstarError("logits must be a CUDA tensor [B, V] with unit inner stride")
+    B, V = (int(x) for x in logits.shape)
+    flags = 0
+    if logits.dtype == torch.bfloat16:
+        flags |= MSTAR_FLAG_LOGITS_BF16
+    elif logits.dtype != torch.float32:
+        raise MstarError("logits must be fp32 or bf16")
+    _want(tokens_out, torch.int32, "tokens_out"); _want(seeds, torch.int64, "seeds"); _want(step, torch.int64, "step")
+    if temperature is not None:
+        _want(temperature, torch.float32, "temperature")
+    if top_k is not None:
+        _want(top_k, torch.int32, "top_k")
+    if top_p is not None:
+        _want(top_p, torch.float32, "top_p")
+    if advance_step:
+        flags |= MSTAR_FLAG_SAMPLE_ADVANCE_STEP
+    lib = load_library()
+    _check(lib.mstar_sample_tokens(_ptr(tokens_out), _ptr(logits), int(logits.stride(0)), B, V, _ptr(temperature),
+                                   _ptr(top_k), _ptr(top_p), _ptr(seeds), _ptr(step), flags, _stream()),
+           "mstar_sample_tokens")
 
 
 def build_slot_mapping(block_table: torch.Tensor, cu_seqlens_q: torch.Tensor, seq_lens: torch.Tensor,

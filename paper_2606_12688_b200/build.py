@@ -15,7 +15,7 @@ PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libmstar_attn.so")
 SOURCES = ["host_common.cu", "kv_append.cu", "kv_append_fp8.cu", "kv_transfer.cu", "decode.cu", "merge_states.cu",
-           "prefill.cu", "prefill_umma.cu", "prefill_fp8.cu"]
+           "prefill.cu", "prefill_umma.cu", "prefill_fp8.cu", "sampling.cu"]
 # measurement aid for bench.py, a library of its own (not part of the product ABI)
 AUX_DIR = os.path.join(PKG_DIR, "bench_aux")
 AUX_LIB_PATH = os.path.join(AUX_DIR, "libmstar_benchaux.so")
