@@ -430,21 +430,35 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                         mbar_wait(bar(B_PFULL00 + 2 * t), pph[t]);
                         tc_fence_after();
                         issue_pv(t, vs, j > 0, false);
+                        // the next K stage landed long ago: checked here, off the chain that follows the last hand-off
+                        if (t == 0 && j + 1 < T) mbar_wait(bar(B_KFULL0 + ks), kph);
                         mbar_wait(bar(B_PFULL00 + 2 * t + 1), pph[t]);
                         pph[t] ^= 1;
                         tc_fence_after();
-                        issue_pv(t, vs, true, true);
-                        commit_if(t == 1, B_VEMPTY0 + vs);
-                        commit_if(j == T - 1, B_OFULL0 + t);
-                        if (j + 1 < T) {
-                            if (t == 0) {
-                                mbar_wait(bar(B_KFULL0 + ks), kph);
-                                tc_fence_after();
+                        // one elected region for everything behind the last hand-off: the rest of P V, its commits,
+                        // the next Q K^T and its commits (each elect / __syncwarp pair sits on the per-tile chain)
+                        if (elect_one()) {
+                            const uint64_t bv = dv + (uint64_t)(vs * 2 * (kPuHT >> 4));
+#pragma unroll
+                            for (int k = kPuSplit / 16; k < 8; ++k)
+                                umma_ts(tmem + 256 + t * 128, tmem + t * 128 + k * 8, bv + (uint64_t)(k * 16 * 128 >> 4),
+                                        idesc_pv, 1u);
+                            if (t == 1) umma_commit(bar(B_VEMPTY0 + vs));
+                            if (j == T - 1) umma_commit(bar(B_OFULL0 + t));
+                            if (j + 1 < T) {
+                                const uint64_t a0 = dq + (uint64_t)(t * 2 * (kPuHT >> 4));
+                                const uint64_t b0 = dk + (uint64_t)(ks * 2 * (kPuHT >> 4));
+#pragma unroll
+                                for (int k = 0; k < 8; ++k) {
+                                    const uint32_t off = (uint32_t)((k >> 2) * (kPuHT >> 4) + (k & 3) * 2);
+                                    umma_ss(tmem + t * 128, a0 + off, b0 + off, idesc_qk, k > 0);
+                                }
+                                umma_commit(bar(B_SFULL0 + t));
+                                if (j + 1 == T - 1) umma_commit(bar(B_QEMPTY0 + t));
+                                if (t == 1) umma_commit(bar(B_KEMPTY0 + ks));
                             }
-                            issue_qk(t, ks);
-                            commit_if(j + 1 == T - 1, B_QEMPTY0 + t);
-                            commit_if(t == 1, B_KEMPTY0 + ks);
                         }
+                        __syncwarp();
                     }
                     if (j + 1 < T) {
                         ks ^= 1;
