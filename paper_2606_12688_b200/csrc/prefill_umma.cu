@@ -531,14 +531,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 tc_fence_after();
                 uint32_t r[128];
                 {
-                    uint32_t(&r0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[0]);
-                    uint32_t(&r1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[32]);
-                    uint32_t(&r2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[64]);
-                    uint32_t(&r3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[96]);
-                    tmem_ld_32x32b_x32(s_addr, r0);
-                    tmem_ld_32x32b_x32(s_addr + 32, r1);
-                    tmem_ld_32x32b_x32(s_addr + 64, r2);
-                    tmem_ld_32x32b_x32(s_addr + 96, r3);
+                    tmem_ld_32x32b_x64(s_addr, *reinterpret_cast<uint32_t(*)[64]>(&r[0]));
+                    tmem_ld_32x32b_x64(s_addr + 64, *reinterpret_cast<uint32_t(*)[64]>(&r[64]));
                     tmem_wait_ld();
                 }
                 // ---- mask (diagonal / last stages only; warp-uniform branch)
