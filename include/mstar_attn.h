@@ -62,6 +62,10 @@ typedef enum {
 #define MSTAR_FLAG_LOGITS_BF16 8u          /* mstar_sample_tokens only: `logits` is bf16 instead of fp32 */
 #define MSTAR_FLAG_SAMPLE_ADVANCE_STEP 16u /* mstar_sample_tokens only: add 1 to *step behind the sampling kernel, so
                                               that every replay of a captured graph draws fresh numbers */
+#define MSTAR_FLAG_SAMPLE_ONE_CTA 32u      /* mstar_sample_tokens only: one CTA per row re-reading the row from L2 (the
+                                              path of vocabularies beyond the cluster kernel's capacity of 8 x 49 152
+                                              tokens) instead of a cluster per row that keeps the row in shared
+                                              memory; same token either way */
 
 /*
  * The paged K/V pool ("a single paged KV pool").  Caller-owned device memory, bf16.

@@ -22,6 +22,7 @@ MSTAR_FLAG_PREFILL_MMA_SYNC = 2
 MSTAR_FLAG_PREFILL_REUSE_PLAN = 4
 MSTAR_FLAG_LOGITS_BF16 = 8
 MSTAR_FLAG_SAMPLE_ADVANCE_STEP = 16
+MSTAR_FLAG_SAMPLE_ONE_CTA = 32
 
 EXPORTS = (
     "mstar_kv_append",
@@ -458,9 +459,10 @@ def paged_attn_prefill_fp8(out: torch.Tensor, q: torch.Tensor, cu_seqlens_q: tor
 
 def sample_tokens(tokens_out: torch.Tensor, logits: torch.Tensor, seeds: torch.Tensor, step: torch.Tensor,
                   temperature: Optional[torch.Tensor] = None, top_k: Optional[torch.Tensor] = None,
-                  top_p: Optional[torch.Tensor] = None, advance_step: bool = False) -> None:
+                  top_p: Optional[torch.Tensor] = None, advance_step: bool = False, one_cta: bool = False) -> None:
     """mstar_sample_tokens.  logits [B, V] fp32 or bf16 (unit inner stride); seeds [B] int64 bit patterns of the
-    uint64 keys; step: one int64 on the device (the uint64 counter)."""
+    uint64 keys; step: one int64 on the device (the uint64 counter).  ``one_cta=True`` sets
+    MSTAR_FLAG_SAMPLE_ONE_CTA (the single-CTA-per-row kernel; same tokens)."""
     if logits.dim() != 2 or logits.stride(1) != 1 or not logits.is_cuda:
         raise MstarError("logits must be a CUDA tensor [B, V] with unit inner stride")
     B, V = (int(x) for x in logits.shape)
@@ -478,6 +480,8 @@ def sample_tokens(tokens_out: torch.Tensor, logits: torch.Tensor, seeds: torch.T
         _want(top_p, torch.float32, "top_p")
     if advance_step:
         flags |= MSTAR_FLAG_SAMPLE_ADVANCE_STEP
+    if one_cta:
+        flags |= MSTAR_FLAG_SAMPLE_ONE_CTA
     lib = load_library()
     _check(lib.mstar_sample_tokens(_ptr(tokens_out), _ptr(logits), int(logits.stride(0)), B, V, _ptr(temperature),
                                    _ptr(top_k), _ptr(top_p), _ptr(seeds), _ptr(step), flags, _stream()),

@@ -315,6 +315,397 @@ __global__ void __launch_bounds__(kSmpThreads) sample_tokens_kernel(const Sample
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Cluster kernel (the default path).  A row is split over the CTAs of a thread-block cluster (1, 2, 4 or 8 CTAs by
+// vocabulary size); each CTA reads its slice from HBM exactly once and keeps it in shared memory as order-preserving
+// integer keys of z, so every later pass is a pass over shared memory, and every reduction crosses the cluster through
+// distributed shared memory behind one cluster barrier.  The arithmetic is the single-CTA kernel's (same keys, same
+// fixed-point weights, same index-order inversion), so the two return the same token.
+//   radix select: level 0 bins a token by x = z_max - z (256 bins over [0, 23); past 23 the fixed-point weight is 0),
+//   which spreads the tokens that matter over the bins where the top byte of a float key would put them into two or
+//   three; levels 1-4 are the four bytes of the key among the tokens of the chosen bin.  Histograms are 16-bit limbs of
+//   the weights added with 32-bit shared-memory reductions (a slice has < 2^16 tokens, so a limb sum fits; sm_100 has
+//   no native 64-bit shared atomic add).
+constexpr int kCsThreads = 512;
+constexpr int kCsWarps = kCsThreads / 32;
+constexpr int kCsBins = 256;
+constexpr int kCsMaxCluster = 8;
+constexpr int kCsMaxSlice = 49152;          // tokens per CTA: 192 KB of keys (and < 2^16, see above)
+constexpr uint32_t kKeyNegInf = 0x007fffffu;  // order_key(-inf): padding, weight 0
+constexpr int kCsCand = 1024;
+constexpr int kCsLoads = 8;                 // 16-byte loads in flight per thread in the pass over HBM
+
+struct CsShared {
+    uint32_t hist[2][3][kCsBins];  // [exchange parity][16-bit limb][digit]
+    uint64_t xchg[2];              // [exchange parity]: the value this CTA publishes
+    uint64_t gath[kCsMaxCluster];  // the published values of all ranks
+    uint64_t wred[kCsWarps];
+    uint64_t pick[3];              // crossing search: digit, weight above it, weight of it
+    uint32_t ncand;                // tokens of the slice in the level-0 bin of the cut (counted at level 1)
+    uint32_t cand[kCsCand];        // their keys, when they fit: levels 2-4 walk this list instead of the slice
+};
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t cluster_nctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+    return r;
+}
+// all threads of all CTAs of the cluster; orders shared-memory writes before it against DSMEM reads after it
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t map_to_rank(uint32_t smem_addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ uint32_t ld_cluster_u32(uint32_t a) {
+    uint32_t v;
+    asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint64_t ld_cluster_u64(uint32_t a) {
+    uint64_t v;
+    asm volatile("ld.shared::cluster.u64 %0, [%1];" : "=l"(v) : "r"(a) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ float key_to_float(uint32_t k) {
+    return __uint_as_float(k ^ ((k >> 31) ? 0x80000000u : 0xffffffffu));
+}
+
+// level-0 digit: 255 - floor((zmax - z) * 255 / 23), clamped; larger z, larger (or equal) digit; digit 0 = weight 0
+__device__ __forceinline__ uint32_t cs_digit0(float z, float zmax) {
+    int b = __float2int_rz((zmax - z) * (255.f / 23.f));  // saturates; NaN -> 0
+    b = min(max(b, 0), kCsBins - 1);
+    return (uint32_t)(kCsBins - 1 - b);
+}
+
+// The fixed-point weight floor(2^32 e), e = 2^((z - zmax) log2 e) as in weight_of, as hi = floor(2^16 e) (0 .. 2^16) and
+// lo = floor(2^32 e) - 2^16 hi (0 .. 2^16 - 1): two round-toward-zero additions of 2^23 leave the integer parts in the
+// significand, the remainder between them is exact (it is a subset of the bits of e).  FMA-pipe instructions only; the
+// one-CTA kernel gets the same integer from the bits of e with 64-bit shifts.
+__device__ __forceinline__ void cs_weight(float z, float zmax, uint32_t& hi, uint32_t& lo) {
+    const float e = fast_exp2((z - zmax) * 1.4426950408889634f);
+    const float hf = __fadd_rz(e * 65536.f, 8388608.f);
+    hi = __float_as_uint(hf) & 0x007fffffu;
+    const float r = fmaf(8388608.f - hf, 65536.f, e * 4294967296.f);
+    lo = __float_as_uint(__fadd_rz(r, 8388608.f)) & 0x007fffffu;
+}
+
+__device__ __forceinline__ uint64_t warp_scan_u64(uint64_t v, int lane) {
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint64_t t = __shfl_up_sync(0xffffffffu, v, o);
+        if (lane >= o) v += t;
+    }
+    return v;
+}
+
+// Every CTA publishes thread 0's `mine`; afterwards sh.gath[r] holds rank r's value in every CTA.
+__device__ __forceinline__ void cs_allgather(CsShared& sh, uint32_t& gen, uint64_t mine, uint32_t CS) {
+    if (threadIdx.x == 0) sh.xchg[gen & 1] = mine;
+    cluster_sync_all();
+    if (threadIdx.x < CS) sh.gath[threadIdx.x] = ld_cluster_u64(map_to_rank(smem_u32(&sh.xchg[gen & 1]), threadIdx.x));
+    __syncthreads();
+    ++gen;
+}
+
+// As radix_select, over the cluster.  COUNT: target = k.  Otherwise target = ceil(tp * kept mass), the kept mass
+// being the total of level 0.  Returns theta (0 = keep everything: the k-th largest token has weight 0).
+template <bool COUNT>
+__device__ uint32_t cs_select(CsShared& sh, const uint32_t* keys, int plen, float zmax, uint32_t floor_key,
+                              uint64_t k_target, float tp, uint32_t CS, uint32_t& gen) {
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    uint32_t theta = 0, d0 = 0;
+    uint64_t above = 0, target = k_target;
+    bool listed = false;
+    for (int level = 0; level < 5; ++level) {
+        const int shift = 32 - 8 * level;  // levels 1..4: 24, 16, 8, 0
+        uint32_t* h = &sh.hist[gen & 1][0][0];
+        for (int i = tid; i < 3 * kCsBins; i += kCsThreads) h[i] = 0;
+        if (level == 1 && tid == 0) sh.ncand = 0;
+        __syncthreads();
+        if (tid == 0) sh.pick[0] = ~0ull;
+        auto add = [&](uint32_t d, uint32_t key) {
+            if (COUNT) {
+                atomicAdd(&h[d], 1u);
+            } else {
+                uint32_t hi, lo;
+                cs_weight(key_to_float(key), zmax, hi, lo);
+                if (lo) atomicAdd(&h[d], lo);
+                if (hi & 0xffffu) atomicAdd(&h[kCsBins + d], hi & 0xffffu);
+                if (hi >> 16) atomicAdd(&h[2 * kCsBins + d], 1u);
+            }
+        };
+        if (listed) {
+            const int nc = (int)sh.ncand;
+            for (int i = tid; i < nc; i += kCsThreads) {
+                const uint32_t key = sh.cand[i];
+                if ((key >> (shift + 8)) == (theta >> (shift + 8))) add((key >> shift) & 255u, key);
+            }
+        } else {
+            const uint4* k4 = reinterpret_cast<const uint4*>(keys);
+            const int n4 = plen >> 2;
+            for (int c0 = warp * 32; c0 < n4; c0 += kCsThreads) {  // the same trip count in every lane of a warp
+                const bool valid = c0 + lane < n4;
+                const uint4 q = valid ? k4[c0 + lane] : make_uint4(0u, 0u, 0u, 0u);
+                const uint32_t kk[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const uint32_t key = kk[e];
+                    uint32_t d = cs_digit0(key_to_float(key), zmax);
+                    bool pass = valid && key >= floor_key;
+                    if (level > 0) {
+                        pass = pass && d == d0;
+                        if (level == 1) {  // the tokens of the bin, appended with one atomic per warp
+                            const unsigned m = __ballot_sync(0xffffffffu, pass);
+                            if (m) {
+                                uint32_t pos = 0;
+                                if (lane == __ffs(m) - 1) pos = atomicAdd(&sh.ncand, (uint32_t)__popc(m));
+                                pos = __shfl_sync(0xffffffffu, pos, __ffs(m) - 1) + __popc(m & ((1u << lane) - 1u));
+                                if (pass && pos < (uint32_t)kCsCand) sh.cand[pos] = key;
+                            }
+                        } else {
+                            pass = pass && (key >> (shift + 8)) == (theta >> (shift + 8));
+                        }
+                        d = (key >> shift) & 255u;
+                    }
+                    if (pass) add(d, key);
+                }
+            }
+        }
+        cluster_sync_all();
+        if (level == 1) listed = sh.ncand <= (uint32_t)kCsCand;  // per CTA: the histograms are the same either way
+        // thread t < 256 owns digit 255 - t: its total over the cluster, then a prefix sum from the top digit down
+        uint64_t tot = 0;
+        if (tid < kCsBins) {
+            const uint32_t a = smem_u32(&h[kCsBins - 1 - tid]);
+            uint32_t l0[kCsMaxCluster], l1[kCsMaxCluster], l2[kCsMaxCluster];  // all loads of the 215-cycle path in flight
+#pragma unroll
+            for (uint32_t r = 0; r < (uint32_t)kCsMaxCluster; ++r) {
+                const uint32_t ra = map_to_rank(a, r < CS ? r : 0u);
+                l0[r] = ld_cluster_u32(ra);
+                l1[r] = COUNT ? 0u : ld_cluster_u32(ra + 4 * kCsBins);
+                l2[r] = COUNT ? 0u : ld_cluster_u32(ra + 8 * kCsBins);
+            }
+#pragma unroll
+            for (uint32_t r = 0; r < (uint32_t)kCsMaxCluster; ++r)
+                if (r < CS) tot += (uint64_t)l0[r] + ((uint64_t)l1[r] << 16) + ((uint64_t)l2[r] << 32);
+        }
+        uint64_t incl = warp_scan_u64(tot, lane);
+        if (lane == 31) sh.wred[warp] = incl;
+        __syncthreads();
+        uint64_t base = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < kCsBins / 32; ++w) {
+            const uint64_t t = sh.wred[w];
+            if (w < warp) base += t;
+            total += t;
+        }
+        if (!COUNT && level == 0) {
+            uint64_t tgt = (uint64_t)ceil((double)tp * (double)total);
+            target = tgt < 1 ? 1 : (tgt > total ? total : tgt);
+        }
+        incl += base;
+        if (tid < kCsBins && above + incl >= target && above + (incl - tot) < target) {
+            sh.pick[0] = (uint64_t)(kCsBins - 1 - tid);
+            sh.pick[1] = above + (incl - tot);
+            sh.pick[2] = tot;
+        }
+        __syncthreads();
+        ++gen;
+        const uint64_t pd = sh.pick[0];
+        uint32_t d = 0;
+        if (pd != ~0ull) {  // always, for target <= total
+            d = (uint32_t)pd;
+            above = sh.pick[1];
+        }
+        if (level == 0) {
+            d0 = d;
+            if (d0 == 0) return 0u;  // the cut falls among tokens of weight 0: keeping all of them changes nothing
+        } else {
+            theta |= d << shift;
+        }
+    }
+    return theta;
+}
+
+__global__ void __launch_bounds__(kCsThreads, 2) sample_tokens_cluster_kernel(const SampleParams p, const int slice) {
+    extern __shared__ __align__(16) unsigned char cs_smem[];
+    CsShared& sh = *reinterpret_cast<CsShared*>(cs_smem);
+    uint32_t* keys = reinterpret_cast<uint32_t*>(cs_smem + ((sizeof(CsShared) + 15) & ~(size_t)15));
+    const uint32_t rank = cluster_ctarank(), CS = cluster_nctarank();
+    const int row = blockIdx.x / CS, V = p.vocab;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int lo = min(V, (int)rank * slice), len = min(V, lo + slice) - lo, plen = (len + 3) & ~3;
+    // every per-row parameter is requested here, in front of the pass over HBM (each is a cold miss of its own)
+    const float T = p.temperature ? p.temperature[row] : 1.f;
+    const int k = p.top_k ? p.top_k[row] : 0;
+    const float tp = p.top_p ? p.top_p[row] : 1.f;
+    const uint64_t seed = p.seeds ? p.seeds[row] : 0ull, step = p.step ? *p.step : 0ull;
+    const float inv_t = T > 0.f ? 1.f / T : 1.f;
+    uint32_t gen = 0;
+
+    // ---- the one pass over HBM: z -> key into shared memory; maximum and its lowest index as max of (key << 32 | ~i)
+    uint64_t best = 0;
+    auto put = [&](int i, float logit) -> uint32_t {  // i: index in the slice
+        const uint32_t key = order_key(logit * inv_t);
+        const uint64_t c = ((uint64_t)key << 32) | (uint32_t)(~(uint32_t)(lo + i));
+        best = c > best ? c : best;
+        return key;
+    };
+    if (!p.bf16) {
+        const float* f = reinterpret_cast<const float*>(p.logits) + (size_t)row * p.row_stride + lo;
+        if ((reinterpret_cast<uintptr_t>(f) & 15) == 0) {
+            const float4* b = reinterpret_cast<const float4*>(f);
+            const int n4 = len >> 2;
+            for (int c0 = tid; c0 < n4; c0 += kCsLoads * kCsThreads) {
+                float4 a[kCsLoads];
+#pragma unroll
+                for (int u = 0; u < kCsLoads; ++u)
+                    if (c0 + u * kCsThreads < n4) a[u] = __ldcs(b + c0 + u * kCsThreads);
+#pragma unroll
+                for (int u = 0; u < kCsLoads; ++u) {
+                    const int c = c0 + u * kCsThreads;
+                    if (c < n4) {
+                        uint4 k;
+                        k.x = put(4 * c, a[u].x); k.y = put(4 * c + 1, a[u].y);
+                        k.z = put(4 * c + 2, a[u].z); k.w = put(4 * c + 3, a[u].w);
+                        reinterpret_cast<uint4*>(keys)[c] = k;
+                    }
+                }
+            }
+            for (int i = 4 * n4 + tid; i < len; i += kCsThreads) keys[i] = put(i, f[i]);
+        } else {
+            for (int i = tid; i < len; i += kCsThreads) keys[i] = put(i, f[i]);
+        }
+    } else {
+        const __nv_bfloat16* hp = reinterpret_cast<const __nv_bfloat16*>(p.logits) + (size_t)row * p.row_stride + lo;
+        if ((reinterpret_cast<uintptr_t>(hp) & 15) == 0) {
+            const uint4* b = reinterpret_cast<const uint4*>(hp);
+            const int n8 = len >> 3;
+            for (int c0 = tid; c0 < n8; c0 += kCsLoads * kCsThreads) {
+                uint4 a[kCsLoads];
+#pragma unroll
+                for (int u = 0; u < kCsLoads; ++u)
+                    if (c0 + u * kCsThreads < n8) a[u] = __ldcs(b + c0 + u * kCsThreads);
+#pragma unroll
+                for (int u = 0; u < kCsLoads; ++u) {
+                    const int c = c0 + u * kCsThreads;
+                    if (c < n8) {
+                        const uint32_t w[4] = {a[u].x, a[u].y, a[u].z, a[u].w};
+                        uint32_t k[8];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            k[2 * j] = put(8 * c + 2 * j, __uint_as_float(w[j] << 16));
+                            k[2 * j + 1] = put(8 * c + 2 * j + 1, __uint_as_float(w[j] & 0xffff0000u));
+                        }
+                        reinterpret_cast<uint4*>(keys)[2 * c] = make_uint4(k[0], k[1], k[2], k[3]);
+                        reinterpret_cast<uint4*>(keys)[2 * c + 1] = make_uint4(k[4], k[5], k[6], k[7]);
+                    }
+                }
+            }
+            for (int i = 8 * n8 + tid; i < len; i += kCsThreads) keys[i] = put(i, __bfloat162float(hp[i]));
+        } else {
+            for (int i = tid; i < len; i += kCsThreads) keys[i] = put(i, __bfloat162float(hp[i]));
+        }
+    }
+    if (tid < plen - len) keys[len + tid] = kKeyNegInf;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const uint64_t other = __shfl_xor_sync(0xffffffffu, best, o);
+        best = other > best ? other : best;
+    }
+    if (lane == 0) sh.wred[warp] = best;
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int w = 1; w < kCsWarps; ++w) best = sh.wred[w] > best ? sh.wred[w] : best;
+    }
+    cs_allgather(sh, gen, best, CS);
+    best = sh.gath[0];
+    for (uint32_t r = 1; r < CS; ++r) best = sh.gath[r] > best ? sh.gath[r] : best;
+    const int argmax = (int)(~(uint32_t)best);
+    const float zmax = key_to_float((uint32_t)(best >> 32));
+
+    if (!(T > 0.f)) {  // greedy (the same branch in every CTA of the cluster)
+        if (rank == 0 && tid == 0) p.tokens[row] = argmax;
+    } else {
+        uint32_t floor_key = 0;
+        if (k > 0 && k < V) floor_key = cs_select<true>(sh, keys, plen, zmax, 0u, (uint64_t)k, 0.f, CS, gen);
+        if (tp > 0.f && tp < 1.f) floor_key = cs_select<false>(sh, keys, plen, zmax, floor_key, 0ull, tp, CS, gen);
+
+        // ---- invert the running sum in index order; thread t owns tokens [t n, (t + 1) n) of the slice, n odd
+        // (consecutive lanes on distinct banks)
+        const int n = ((slice + kCsThreads - 1) / kCsThreads) | 1;
+        const int i0 = min(plen, tid * n), i1 = min(plen, i0 + n);
+        uint32_t sum_hi = 0, sum_lo = 0;  // n < 2^7 tokens: no overflow
+#pragma unroll 8
+        for (int j = 0; j < n; ++j) {
+            const int i = i0 + j;
+            const uint32_t key = i < i1 ? keys[i] : 0u;
+            uint32_t wh, wl;
+            cs_weight(key_to_float(key), zmax, wh, wl);
+            if (i < i1 && key >= floor_key) {
+                sum_hi += wh;
+                sum_lo += wl;
+            }
+        }
+        const uint64_t mine = ((uint64_t)sum_hi << 16) + sum_lo;
+        uint64_t incl = warp_scan_u64(mine, lane);
+        __syncthreads();  // wred may still be read (select or the maximum)
+        if (lane == 31) sh.wred[warp] = incl;
+        __syncthreads();
+        uint64_t base = 0, cta_total = 0;
+#pragma unroll
+        for (int w = 0; w < kCsWarps; ++w) {
+            const uint64_t t = sh.wred[w];
+            if (w < warp) base += t;
+            cta_total += t;
+        }
+        cs_allgather(sh, gen, cta_total, CS);
+        uint64_t W = 0, before = 0;
+        for (uint32_t r = 0; r < CS; ++r) {
+            const uint64_t t = sh.gath[r];
+            if (r < rank) before += t;
+            W += t;
+        }
+        uint32_t c[4] = {(uint32_t)step, (uint32_t)(step >> 32), (uint32_t)row, 0u};
+        philox4x32_10(c, (uint32_t)seed, (uint32_t)(seed >> 32));
+        const uint64_t target = __umul64hi(((uint64_t)c[0] << 32) | 0x80000000ull, W);
+        const uint64_t run = before + base + incl - mine;
+        if (W == 0 && rank == 0 && tid == 0) p.tokens[row] = argmax;  // cannot happen (the maximum weighs 2^32); guard
+        // exactly one thread of the cluster owns the target; its warp scans that thread's tokens together
+        const unsigned own = __ballot_sync(0xffffffffu, W != 0 && mine > 0 && run <= target && target < run + mine);
+        if (own) {
+            const int src = __ffs(own) - 1;
+            const int b0 = __shfl_sync(0xffffffffu, i0, src), b1 = __shfl_sync(0xffffffffu, i1, src);
+            uint64_t r0 = __shfl_sync(0xffffffffu, run, src);
+            for (int base_i = b0; base_i < b1; base_i += 32) {
+                const int i = base_i + lane;
+                const uint32_t key = i < b1 ? keys[i] : 0u;
+                uint32_t wh, wl;
+                cs_weight(key_to_float(key), zmax, wh, wl);
+                const uint64_t w = (i < b1 && key >= floor_key) ? ((uint64_t)wh << 16) + wl : 0ull;
+                const uint64_t inc = warp_scan_u64(w, lane);
+                const unsigned hit = __ballot_sync(0xffffffffu, w > 0 && r0 + inc > target);
+                if (hit) {
+                    if (lane == 0) p.tokens[row] = lo + base_i + __ffs(hit) - 1;
+                    break;
+                }
+                r0 += __shfl_sync(0xffffffffu, inc, 31);
+            }
+        }
+    }
+    cluster_sync_all();  // no CTA leaves while a peer may still read its shared memory
+}
+
 __global__ void sample_advance_kernel(uint64_t* step) { *step += 1; }
 
 }  // namespace mstar
@@ -324,7 +715,8 @@ extern "C" int mstar_sample_tokens(int32_t* tokens_out, const void* logits, int6
                                    const uint64_t* seeds, uint64_t* step, uint32_t flags, void* stream) {
     using namespace mstar;
     launch_count_reset();
-    if (flags & ~(MSTAR_FLAG_LOGITS_BF16 | MSTAR_FLAG_SAMPLE_ADVANCE_STEP)) return MSTAR_ERR_INVALID_ARG;
+    if (flags & ~(MSTAR_FLAG_LOGITS_BF16 | MSTAR_FLAG_SAMPLE_ADVANCE_STEP | MSTAR_FLAG_SAMPLE_ONE_CTA))
+        return MSTAR_ERR_INVALID_ARG;
     if (num_rows < 0 || vocab <= 0 || row_stride < vocab) return MSTAR_ERR_INVALID_ARG;
     if (num_rows == 0) return MSTAR_OK;
     if (!tokens_out || !logits || !seeds || !step) return MSTAR_ERR_INVALID_ARG;
@@ -343,10 +735,33 @@ extern "C" int mstar_sample_tokens(int32_t* tokens_out, const void* logits, int6
     p.step = step;
     p.tokens = tokens_out;
     cudaStream_t st = (cudaStream_t)stream;
-    static PerDeviceOnce once;
-    MSTAR_CUDA_OK(set_max_dynamic_smem(once, sample_tokens_kernel, 16 * kSmpThreads * 8));
-    sample_tokens_kernel<<<(unsigned)num_rows, kSmpThreads, 16 * kSmpThreads * 8, st>>>(p);
-    MSTAR_CUDA_OK(cudaGetLastError());
+    // cluster size by vocabulary: slices of at most 4096 tokens up to 4 CTAs, then 8 CTAs with whatever slice results
+    const int cs = vocab <= 4096 ? 1 : vocab <= 8192 ? 2 : vocab <= 16384 ? 4 : kCsMaxCluster;
+    const int slice = ((vocab + cs - 1) / cs + 7) & ~7;
+    if (!(flags & MSTAR_FLAG_SAMPLE_ONE_CTA) && slice <= kCsMaxSlice) {
+        const size_t smem = ((sizeof(CsShared) + 15) & ~(size_t)15) + (size_t)slice * 4;
+        static PerDeviceOnce once_cs;
+        MSTAR_CUDA_OK(set_max_dynamic_smem(once_cs, sample_tokens_cluster_kernel,
+                                           (int)(((sizeof(CsShared) + 15) & ~(size_t)15) + (size_t)kCsMaxSlice * 4)));
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)num_rows * cs);
+        cfg.blockDim = dim3(kCsThreads);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = cs;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        MSTAR_CUDA_OK(cudaLaunchKernelEx(&cfg, sample_tokens_cluster_kernel, p, slice));
+    } else {
+        static PerDeviceOnce once;
+        MSTAR_CUDA_OK(set_max_dynamic_smem(once, sample_tokens_kernel, 16 * kSmpThreads * 8));
+        sample_tokens_kernel<<<(unsigned)num_rows, kSmpThreads, 16 * kSmpThreads * 8, st>>>(p);
+        MSTAR_CUDA_OK(cudaGetLastError());
+    }
     launch_count_add(1);
     if (flags & MSTAR_FLAG_SAMPLE_ADVANCE_STEP) {
         sample_advance_kernel<<<1, 1, 0, st>>>(step);

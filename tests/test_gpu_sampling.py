@@ -33,15 +33,20 @@ def unambiguous(lg, T, k, p):
     return True
 
 
-def run(logits, T, K, P, seeds, step, dtype=torch.float32, advance=False):
+def run(logits, T, K, P, seeds, step, dtype=torch.float32, advance=False, one_cta=False, pad=0):
     B, V = logits.shape
     lg = torch.from_numpy(logits.astype(np.float32)).cuda().to(dtype)
+    if pad:   # rows that start off a 16-byte boundary, with a stride that is not a multiple of the vector width
+        big = torch.full((B, V + 2 * pad + 1), float("nan"), dtype=dtype, device="cuda")
+        big[:, pad:pad + V] = lg
+        lg = big[:, pad:pad + V]
     out = torch.full((B,), -1, dtype=torch.int32, device="cuda")
     st = torch.tensor([step], dtype=torch.int64, device="cuda")
     mstar.sample_tokens(out, lg, torch.from_numpy(np.asarray(seeds, dtype=np.int64)).cuda(), st,
                         temperature=torch.from_numpy(np.asarray(T, np.float32)).cuda(),
                         top_k=torch.from_numpy(np.asarray(K, np.int32)).cuda(),
-                        top_p=torch.from_numpy(np.asarray(P, np.float32)).cuda(), advance_step=advance)
+                        top_p=torch.from_numpy(np.asarray(P, np.float32)).cuda(), advance_step=advance,
+                        one_cta=one_cta)
     torch.cuda.synchronize()
     return out.cpu().numpy(), lg.float().cpu().numpy().astype(np.float64), int(st.item())
 
@@ -92,6 +97,32 @@ def test_sample_tokens_random_rows_all_filters(V, dtype):
         tok, lg64, _ = run(lg, T, K, P, seeds, step, dtype=dtype)
         exact = check_rows(tok, lg64, T, K, P, seeds, step)
         assert exact >= 0.95 * (T != 0).sum()   # away from interval boundaries the token is the oracle's own
+
+
+@pytest.mark.parametrize("V", [1, 7, 4096, 4099, 8200, 16390, 40001, 151936])
+@pytest.mark.parametrize("dtype", [torch.float32, torch.bfloat16])
+def test_sample_tokens_cluster_kernel_equals_one_cta_kernel(V, dtype):
+    """The cluster kernel (1, 2, 4, 8 CTAs per row by vocabulary size; the default) and the one-CTA kernel compute the
+    same keys, fixed-point weights and index-order inversion: the same token on rows of every kind -- ties at the
+    top-k / top-p cut, -inf entries, a cut among tokens of weight 0, greedy rows, unaligned rows."""
+    rng = np.random.default_rng(900 + V)
+    B = 24
+    lg = np.float32(rng.normal(0, 3.0, (B, V)))
+    lg[:, ::5] = np.round(lg[:, ::5] * 4) / 4          # many exact ties
+    lg[B // 2:, 1::7] = -np.inf
+    lg[3] = 1.25                                       # all equal
+    lg[4, :] = -40.0
+    lg[4, V // 2] = 0.0                                # every other token has weight 0
+    T = np.float32(rng.choice([0.0, 0.3, 0.8, 1.0, 2.5], B))
+    K = rng.choice([0, 1, 2, 50, max(1, V // 2), max(1, V - 1), V], B).astype(np.int32)
+    P = np.float32(rng.choice([1.0, 0.999, 0.9, 0.5, 1e-6], B))
+    T[3], T[4] = 1.0, 1.0
+    seeds = rng.integers(0, 2 ** 62, B)
+    for step, pad in ((0, 0), (7, 0), (3, 3)):
+        a, _, _ = run(lg, T, K, P, seeds, step, dtype=dtype, pad=pad)
+        b, _, _ = run(lg, T, K, P, seeds, step, dtype=dtype, pad=pad, one_cta=True)
+        assert np.array_equal(a, b), (V, step, pad, np.flatnonzero(a != b), a[a != b], b[a != b])
+        assert np.all((a >= 0) & (a < V))
 
 
 def test_sample_tokens_vocab_of_a_real_tokenizer_size():
