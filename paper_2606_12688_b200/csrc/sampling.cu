@@ -332,7 +332,8 @@ constexpr int kCsBins = 256;
 constexpr int kCsMaxCluster = 8;
 constexpr int kCsMaxSlice = 49152;          // tokens per CTA: 192 KB of keys (and < 2^16, see above)
 constexpr uint32_t kKeyNegInf = 0x007fffffu;  // order_key(-inf): padding, weight 0
-constexpr int kCsCand = 1024;
+constexpr int kCsCand = 512;     // listed tokens per CTA
+constexpr int kCsGather = 2048;  // and per cluster, for the select to finish on the gathered list
 constexpr int kCsLoads = 8;                 // 16-byte loads in flight per thread in the pass over HBM
 
 struct CsShared {
@@ -341,8 +342,10 @@ struct CsShared {
     uint64_t gath[kCsMaxCluster];  // the published values of all ranks
     uint64_t wred[kCsWarps];
     uint64_t pick[3];              // crossing search: digit, weight above it, weight of it
-    uint32_t ncand;                // tokens of the slice in the level-0 bin of the cut (counted at level 1)
-    uint32_t cand[kCsCand];        // their keys, when they fit: levels 2-4 walk this list instead of the slice
+    uint32_t ncand;                // tokens of the slice in the level-0 bin of the cut
+    uint32_t cand[kCsCand];        // their keys, when they fit
+    uint32_t range[2];             // the bin as a key range: first key of the bin, first key of the next bin
+    uint32_t gl[kCsGather];        // the lists of all CTAs of the cluster
 };
 
 __device__ __forceinline__ uint32_t cluster_ctarank() {
@@ -416,6 +419,176 @@ __device__ __forceinline__ void cs_allgather(CsShared& sh, uint32_t& gen, uint64
     ++gen;
 }
 
+template <bool COUNT>
+__device__ __forceinline__ void cs_hist_add(uint32_t* h, uint32_t d, uint32_t key, float zmax) {
+    if (COUNT) {
+        atomicAdd(&h[d], 1u);
+    } else {
+        uint32_t hi, lo;
+        cs_weight(key_to_float(key), zmax, hi, lo);
+        if (lo) atomicAdd(&h[d], lo);
+        if (hi & 0xffffu) atomicAdd(&h[kCsBins + d], hi & 0xffffu);
+        if (hi >> 16) atomicAdd(&h[2 * kCsBins + d], 1u);
+    }
+}
+
+// Crossing search of one level.  tot = the level's total of digit 255 - tid in the threads tid < 256 (0 elsewhere).
+// Finds the largest digit d with above + (total of the digits >= d) >= target, moves `above` to the weight above d
+// and returns d.  set_target: target = ceil(tp * total of the level), clamped to [1, total], first.  Called by all
+// threads; sh.pick[0] must hold ~0 (set behind a barrier that follows the previous call).
+__device__ __forceinline__ uint32_t cs_cross(CsShared& sh, uint64_t tot, uint64_t& above, uint64_t& target,
+                                             bool set_target, float tp) {
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    uint64_t incl = warp_scan_u64(tot, lane);
+    if (lane == 31) sh.wred[warp] = incl;
+    __syncthreads();
+    uint64_t base = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kCsBins / 32; ++w) {
+        const uint64_t t = sh.wred[w];
+        if (w < warp) base += t;
+        total += t;
+    }
+    if (set_target) {
+        const uint64_t tgt = (uint64_t)ceil((double)tp * (double)total);
+        target = tgt < 1 ? 1 : (tgt > total ? total : tgt);
+    }
+    incl += base;
+    if (tid < kCsBins && above + incl >= target && above + (incl - tot) < target) {
+        sh.pick[0] = (uint64_t)(kCsBins - 1 - tid);
+        sh.pick[1] = above + (incl - tot);
+    }
+    __syncthreads();
+    const uint64_t pd = sh.pick[0];
+    if (pd == ~0ull) return 0u;  // never, for target <= total
+    above = sh.pick[1];
+    return (uint32_t)pd;
+}
+
+// The rest of a select behind level 0, when the tokens of bin d0 are few (the usual case): the bin is a key range
+// (the level-0 digit is monotone in the key; its two ends by a 32-way search in one warp each), every CTA lists the
+// keys of its slice in the range, all lists are gathered into every CTA through distributed shared memory, and the
+// four key bytes are resolved on the gathered list with no further cluster traffic.  False (nothing decided) when a
+// list overflows; the decision is the same in every CTA of the cluster.
+template <bool COUNT>
+__device__ bool cs_finish_on_list(CsShared& sh, const uint32_t* keys, int plen, float zmax, uint32_t floor_key,
+                                  uint32_t d0, uint64_t above, uint64_t target, uint32_t CS, uint32_t& gen,
+                                  uint32_t& theta_out) {
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (warp < 2) {  // warp 0: the first key of bin d0; warp 1: the first key of bin d0 + 1
+        const uint32_t D = d0 + warp;
+        uint32_t lo = kKeyNegInf, hi = 0xff800000u;  // the keys of -inf and +inf; digit(+inf) = 255
+        if (D < (uint32_t)kCsBins) {
+            while (lo < hi) {
+                const uint32_t span = hi - lo, step = (span + 30u) / 31u;  // lane 31 probes hi
+                const bool t = cs_digit0(key_to_float(lo + min(span, (uint32_t)lane * step)), zmax) >= D;
+                const int L = __ffs(__ballot_sync(0xffffffffu, t)) - 1;
+                hi = lo + min(span, (uint32_t)L * step);
+                lo = L == 0 ? hi : lo + min(span, (uint32_t)(L - 1) * step) + 1u;
+            }
+        } else {
+            lo = 0u;  // no bin above: the range is open
+        }
+        if (lane == 0) sh.range[warp] = lo;
+    }
+    if (tid == 0) sh.ncand = 0;
+    __syncthreads();
+    const uint32_t bin_lo = sh.range[0], khi = sh.range[1] - 1u, klo = max(bin_lo, floor_key);
+    const uint4* k4 = reinterpret_cast<const uint4*>(keys);
+    const int n4 = plen >> 2;
+    for (int c0 = warp * 32; c0 < n4; c0 += kCsThreads) {  // the same trip count in every lane of a warp
+        const bool valid = c0 + lane < n4;
+        const uint4 q = valid ? k4[c0 + lane] : make_uint4(0u, 0u, 0u, 0u);
+        const uint32_t kk[4] = {q.x, q.y, q.z, q.w};
+        bool ps[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) ps[e] = valid && kk[e] >= klo && kk[e] <= khi;
+        if (!__ballot_sync(0xffffffffu, ps[0] || ps[1] || ps[2] || ps[3])) continue;  // the usual case
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const unsigned m = __ballot_sync(0xffffffffu, ps[e]);
+            if (m) {  // one atomic per warp
+                uint32_t pos = 0;
+                if (lane == __ffs(m) - 1) pos = atomicAdd(&sh.ncand, (uint32_t)__popc(m));
+                pos = __shfl_sync(0xffffffffu, pos, __ffs(m) - 1) + __popc(m & ((1u << lane) - 1u));
+                if (ps[e] && pos < (uint32_t)kCsCand) sh.cand[pos] = kk[e];
+            }
+        }
+    }
+    __syncthreads();
+    cs_allgather(sh, gen, (uint64_t)sh.ncand, CS);  // its barrier also publishes cand[]
+    uint32_t total = 0, offs[kCsMaxCluster + 1];
+    bool fits = true;
+#pragma unroll
+    for (uint32_t r = 0; r < (uint32_t)kCsMaxCluster; ++r) {
+        const uint64_t cnt = r < CS ? sh.gath[r] : 0ull;
+        fits = fits && cnt <= (uint64_t)kCsCand;
+        offs[r] = total;
+        total += (uint32_t)min(cnt, (uint64_t)kCsGather);
+    }
+    offs[kCsMaxCluster] = total;
+    if (!fits || total > (uint32_t)kCsGather) return false;
+    for (uint32_t g = tid; g < total; g += kCsThreads) {  // all remote loads of a thread in flight together
+        uint32_t r = 0;
+#pragma unroll
+        for (uint32_t j = 1; j < (uint32_t)kCsMaxCluster; ++j) r += g >= offs[j];
+        sh.gl[g] = ld_cluster_u32(map_to_rank(smem_u32(&sh.cand[0]), r) + 4u * (g - offs[r]));
+    }
+    __syncthreads();
+    // One warp resolves the key bytes on the gathered list (peers read hist[] of level 0 before they arrive at the
+    // barrier above, so both copies are free here).  All keys of the list lie in [bin_lo, khi]: the bytes above the
+    // highest bit in which the two ends differ are common to all and are skipped.
+    if (warp == 0) {
+        uint32_t* h = &sh.hist[0][0][0];
+        const uint32_t diff = bin_lo ^ khi;
+        const int nb = diff ? 32 - __clz(diff) : 0;  // the low nb bits vary
+        uint32_t theta = nb < 32 ? (bin_lo >> nb) << nb : 0u;
+        for (int shift = ((nb + 7) / 8 - 1) * 8; shift >= 0; shift -= 8) {
+            for (int i = lane; i < (COUNT ? 1 : 3) * kCsBins / 4; i += 32)
+                reinterpret_cast<uint4*>(h)[i] = make_uint4(0u, 0u, 0u, 0u);
+            __syncwarp();
+            for (uint32_t i = lane; i < total; i += 32) {
+                const uint32_t key = sh.gl[i];
+                if (shift == 24 || (key >> (shift + 8)) == (theta >> (shift + 8)))
+                    cs_hist_add<COUNT>(h, (key >> shift) & 255u, key, zmax);
+            }
+            __syncwarp();
+            // lane l owns the digits 255 - 8 l down to 248 - 8 l
+            uint64_t t[8], sum = 0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int d = kCsBins - 1 - 8 * lane - j;
+                t[j] = (uint64_t)h[d];
+                if (!COUNT) t[j] += ((uint64_t)h[kCsBins + d] << 16) + ((uint64_t)h[2 * kCsBins + d] << 32);
+                sum += t[j];
+            }
+            const uint64_t incl = warp_scan_u64(sum, lane);
+            uint64_t run = above + incl - sum;
+            const unsigned hit = __ballot_sync(0xffffffffu, above + incl >= target && run < target);
+            uint32_t d = 0;
+            if (hit) {  // always, for target <= total
+                bool found = false;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    if (!found && run + t[j] >= target) {
+                        d = kCsBins - 1 - 8 * lane - j;
+                        found = true;
+                    }
+                    if (!found) run += t[j];
+                }
+                d = __shfl_sync(0xffffffffu, d, __ffs(hit) - 1);
+                above = __shfl_sync(0xffffffffu, run, __ffs(hit) - 1);
+            }
+            theta |= d << shift;
+            __syncwarp();
+        }
+        if (lane == 0) sh.range[0] = theta;
+    }
+    __syncthreads();
+    theta_out = sh.range[0];
+    return true;
+}
+
 // As radix_select, over the cluster.  COUNT: target = k.  Otherwise target = ceil(tp * kept mass), the kept mass
 // being the total of level 0.  Returns theta (0 = keep everything: the k-th largest token has weight 0).
 template <bool COUNT>
@@ -432,22 +605,12 @@ __device__ uint32_t cs_select(CsShared& sh, const uint32_t* keys, int plen, floa
         if (level == 1 && tid == 0) sh.ncand = 0;
         __syncthreads();
         if (tid == 0) sh.pick[0] = ~0ull;
-        auto add = [&](uint32_t d, uint32_t key) {
-            if (COUNT) {
-                atomicAdd(&h[d], 1u);
-            } else {
-                uint32_t hi, lo;
-                cs_weight(key_to_float(key), zmax, hi, lo);
-                if (lo) atomicAdd(&h[d], lo);
-                if (hi & 0xffffu) atomicAdd(&h[kCsBins + d], hi & 0xffffu);
-                if (hi >> 16) atomicAdd(&h[2 * kCsBins + d], 1u);
-            }
-        };
         if (listed) {
             const int nc = (int)sh.ncand;
             for (int i = tid; i < nc; i += kCsThreads) {
                 const uint32_t key = sh.cand[i];
-                if ((key >> (shift + 8)) == (theta >> (shift + 8))) add((key >> shift) & 255u, key);
+                if ((key >> (shift + 8)) == (theta >> (shift + 8)))
+                    cs_hist_add<COUNT>(h, (key >> shift) & 255u, key, zmax);
             }
         } else {
             const uint4* k4 = reinterpret_cast<const uint4*>(keys);
@@ -476,7 +639,7 @@ __device__ uint32_t cs_select(CsShared& sh, const uint32_t* keys, int plen, floa
                         }
                         d = (key >> shift) & 255u;
                     }
-                    if (pass) add(d, key);
+                    if (pass) cs_hist_add<COUNT>(h, d, key, zmax);
                 }
             }
         }
@@ -498,37 +661,13 @@ __device__ uint32_t cs_select(CsShared& sh, const uint32_t* keys, int plen, floa
             for (uint32_t r = 0; r < (uint32_t)kCsMaxCluster; ++r)
                 if (r < CS) tot += (uint64_t)l0[r] + ((uint64_t)l1[r] << 16) + ((uint64_t)l2[r] << 32);
         }
-        uint64_t incl = warp_scan_u64(tot, lane);
-        if (lane == 31) sh.wred[warp] = incl;
-        __syncthreads();
-        uint64_t base = 0, total = 0;
-#pragma unroll
-        for (int w = 0; w < kCsBins / 32; ++w) {
-            const uint64_t t = sh.wred[w];
-            if (w < warp) base += t;
-            total += t;
-        }
-        if (!COUNT && level == 0) {
-            uint64_t tgt = (uint64_t)ceil((double)tp * (double)total);
-            target = tgt < 1 ? 1 : (tgt > total ? total : tgt);
-        }
-        incl += base;
-        if (tid < kCsBins && above + incl >= target && above + (incl - tot) < target) {
-            sh.pick[0] = (uint64_t)(kCsBins - 1 - tid);
-            sh.pick[1] = above + (incl - tot);
-            sh.pick[2] = tot;
-        }
-        __syncthreads();
+        const uint32_t d = cs_cross(sh, tot, above, target, !COUNT && level == 0, tp);
         ++gen;
-        const uint64_t pd = sh.pick[0];
-        uint32_t d = 0;
-        if (pd != ~0ull) {  // always, for target <= total
-            d = (uint32_t)pd;
-            above = sh.pick[1];
-        }
         if (level == 0) {
             d0 = d;
             if (d0 == 0) return 0u;  // the cut falls among tokens of weight 0: keeping all of them changes nothing
+            if (cs_finish_on_list<COUNT>(sh, keys, plen, zmax, floor_key, d0, above, target, CS, gen, theta))
+                return theta;
         } else {
             theta |= d << shift;
         }
