@@ -478,7 +478,7 @@ def other_workloads(torch, mstar, DeviceBatch, W, dev, flush, hbm_peak, iters=15
         return {"rows": Bs, "vocab": Vs, "logits": str(dtype).split(".")[-1], "top_k": int(tk[0]),
                 "top_p": float(tp[0]), "us": ms * 1e3, "tokens_per_s": Bs / (ms * 1e-3),
                 "logit_bytes": nbytes, "GBps_one_read_of_the_logits": nbytes / (ms * 1e-3) / 1e9,
-                "passes_over_the_row": 21 if use_filters else 4}
+                "kernel": "cluster of 8 CTAs per row, the row read from HBM once and kept in shared memory"}
 
     res["sampling (SURVEY 8(f) rank 4): temperature only, fp32 logits"] = sampling_entry(torch.float32, False)
     res["sampling (SURVEY 8(f) rank 4): top-k 50 + top-p 0.9, fp32 logits"] = sampling_entry(torch.float32, True)

@@ -1,16 +1,20 @@
 // sampling.cu -- mstar_sample_tokens: CUDA-graph-compatible token sampling (last clause;
 // PAPER.md:134 "a cuda-graph-compatible sampling plugin", :230; definition: DESIGN.md R28, oracle/sampling.py).
 //
-// One CTA per row of logits.  Everything after the exponential is INTEGER arithmetic, so the result does not depend on
-// the order in which threads add: token weights are fixed-point, w_i = floor(2^32 * 2^((z_i - z_max) log2 e)), sums are
-// 64-bit integers, the uniform number is the 64-bit fraction (x + 1/2) / 2^32 of a Philox4x32-10 word and the running
-// sum is inverted in index order.  No state on the host: seeds and the step counter are device memory, so a replayed
-// CUDA graph draws fresh numbers (MSTAR_FLAG_SAMPLE_ADVANCE_STEP adds 1 to the counter behind the sampling kernel).
+// Everything after the exponential is INTEGER arithmetic, so the result does not depend on the order in which threads
+// (or CTAs) add: token weights are fixed-point, w_i = floor(2^32 * 2^((z_i - z_max) log2 e)), sums are 64-bit integers,
+// the uniform number is the 64-bit fraction (x + 1/2) / 2^32 of a Philox4x32-10 word and the running sum is inverted
+// in index order.  No state on the host: seeds and the step counter are device memory, so a replayed CUDA graph draws
+// fresh numbers (MSTAR_FLAG_SAMPLE_ADVANCE_STEP adds 1 to the counter behind the sampling kernel).
 //
-// Passes over the row (all L2 hits after the first): maximum / argmax; [top-k: 8 radix-select passes on the order-
-// preserving integer image of z, 4 bits each, counting]; total weight; [top-p: 8 radix-select passes, weighing; total
-// weight of the nucleus]; weight per warp segment; scan of the one segment that holds the target.  A radix-select
-// pass keeps one private 16-bin histogram per thread in shared memory (no atomics) and reduces it afterwards.
+// Two kernels that return the same token:
+//   sample_tokens_cluster_kernel (default): a thread-block cluster per row, the row read from HBM once and kept in
+//     shared memory, reductions over distributed shared memory;
+//   sample_tokens_kernel (MSTAR_FLAG_SAMPLE_ONE_CTA, and vocabularies past the cluster kernel's capacity): one CTA per
+//     row, the row re-read from L2 in every pass: maximum / argmax; [top-k: 8 radix-select passes on the order-
+//     preserving integer image of z, 4 bits each, counting]; total weight; [top-p: 8 radix-select passes, weighing];
+//     weight per warp segment; scan of the one segment that holds the target.  A radix-select pass keeps one private
+//     16-bin histogram per thread in shared memory (no atomics) and reduces it afterwards.
 #include <cuda_bf16.h>
 
 #include "host_common.h"
