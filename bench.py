@@ -701,6 +701,93 @@ def run_ours(args):
     return 0
 
 
+def run_sustained(args):
+    """--sustained: each kernel of the path launched back to back for a few seconds while NVML samples board power,
+    SM clock and throttle reasons, next to a cuBLAS bf16 GEMM and a device copy under the same regime.  Not the bench
+    line: it shows which limit (power cap, clock) the measured rates sit under.  One JSON object on stdout."""
+    import pynvml as nv
+    import torch
+    import paper_2606_12688_b200 as mstar
+    import workloads as W
+    from paper_2606_12688_b200.harness import DeviceBatch
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    mstar.load_library()
+    nv.nvmlInit()
+    h = nv.nvmlDeviceGetHandleByIndex(0)
+    out = {"mode": "sustained", "seconds_per_kernel": args.sustained,
+           "power_limit_w": nv.nvmlDeviceGetEnforcedPowerLimit(h) / 1e3,
+           "sm_max_mhz": int(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)), "kernels": {}}
+    names = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+             0x80: "hw_power_brake_slowdown"}
+
+    def sustained(name, call, work, unit):
+        stop, samples = threading.Event(), []
+
+        def sampler():
+            while not stop.is_set():
+                samples.append((nv.nvmlDeviceGetPowerUsage(h) / 1e3, nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM),
+                                nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)))
+                time.sleep(0.02)
+        th = threading.Thread(target=sampler, daemon=True)
+        call()
+        torch.cuda.synchronize()
+        th.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0, n = time.time(), 0
+        e0.record()
+        while time.time() - t0 < args.sustained:
+            for _ in range(50):
+                call()
+            n += 50
+            torch.cuda.synchronize()
+        e1.record()
+        torch.cuda.synchronize()
+        stop.set()
+        th.join()
+        smp = samples[len(samples) // 3:] or samples
+        bits = 0
+        for x in smp:
+            bits |= x[2]
+        us = e0.elapsed_time(e1) * 1e3 / n
+        out["kernels"][name] = {"us_per_call": us, "rate": work / (us * 1e-6), "unit": unit,
+                                "power_w_median": float(np.median([x[0] for x in smp])),
+                                "sm_mhz_median": float(np.median([x[1] for x in smp])),
+                                "reasons": [v for k, v in names.items() if bits & k]}
+
+    def prefill_call(b, causal):
+        d = DeviceBatch(b, device=dev)
+        d.append()
+        o = torch.empty((b.total_q, b.num_q_heads, b.head_dim), dtype=torch.bfloat16, device=dev)
+        ws = torch.empty(mstar.prefill_workspace_bytes(b.num_seqs, b.total_q, b.num_q_heads, b.head_dim),
+                         dtype=torch.uint8, device=dev)
+        return lambda: mstar.paged_attn_prefill(o, d.q, d.cu_seqlens_q, d.pool, d.block_table, d.seq_lens, b.max_q_len,
+                                                b.max_seq_len, float(b.scale), causal=causal, workspace=ws)
+
+    b3 = W.config3_prefill()
+    sustained("prefill configs[2] (plan + attention)", prefill_call(b3, True), prefill_flops(b3) / 1e12, "TFLOP/s")
+    bf = W.flow_step_bagel()
+    n, L = bf.q_lens.astype(np.float64), bf.seq_lens.astype(np.float64)
+    sustained("prefill flow step, causal = 0", prefill_call(bf, False),
+              float((4.0 * bf.num_q_heads * bf.head_dim * n * L).sum()) / 1e12, "TFLOP/s")
+    a = torch.randn(8192, 8192, device=dev, dtype=torch.bfloat16)
+    bm = torch.randn(8192, 8192, device=dev, dtype=torch.bfloat16)
+    c = torch.empty(8192, 8192, device=dev, dtype=torch.bfloat16)
+    sustained("cuBLAS bf16 GEMM 8192^3", lambda: torch.matmul(a, bm, out=c), 2 * 8192.0 ** 3 / 1e12, "TFLOP/s")
+    del a, bm, c
+    x = torch.empty(1 << 30, dtype=torch.uint8, device=dev)
+    y = torch.empty_like(x)
+    sustained("device copy 1 GiB", lambda: y.copy_(x), 2 * float(1 << 30) / 1e9, "GB/s read + write")
+    del x, y
+    b2 = W.config2_bagel_cfg_decode()
+    d2 = DeviceBatch(b2, device=dev)
+    d2.append()
+    sustained("decode configs[1] (warm L2)", lambda: d2.decode(num_partitions=0), b2.kv_bytes_unique() / 1e9,
+              "GB/s of unique K/V")
+    print(json.dumps(out))
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -709,9 +796,13 @@ def main(argv=None):
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other", action="store_true", help="skip the configs[1] / configs[3] decode timings")
+    ap.add_argument("--sustained", type=float, default=0.0, metavar="SECONDS",
+                    help="instead of the bench line: power / clock of each kernel launched back to back for SECONDS")
     args = ap.parse_args(argv)
     if args.impl == "reference":
         return run_reference(args)
+    if args.sustained > 0:
+        return run_sustained(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # plain `python bench.py --gpus N`: become N ranks (one per GPU) under torchrun on this node
         return respawn_under_torchrun(args.gpus, sys.argv[1:] if argv is None else list(argv))
