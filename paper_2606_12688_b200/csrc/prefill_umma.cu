@@ -530,7 +530,15 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 sph ^= 1;
                 tc_fence_after();
                 uint32_t r[128];
-                {
+                if constexpr (F16) {
+                    // four 32-column loads: with the converter warps resident, the two 64-column loads of the bf16
+                    // instantiation measured 6.5 % slower here (152.6 -> 162.8 us on config 3, A/B on one box)
+                    tmem_ld_32x32b_x32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
+                    tmem_ld_32x32b_x32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
+                    tmem_ld_32x32b_x32(s_addr + 64, *reinterpret_cast<uint32_t(*)[32]>(&r[64]));
+                    tmem_ld_32x32b_x32(s_addr + 96, *reinterpret_cast<uint32_t(*)[32]>(&r[96]));
+                    tmem_wait_ld();
+                } else {
                     tmem_ld_32x32b_x64(s_addr, *reinterpret_cast<uint32_t(*)[64]>(&r[0]));
                     tmem_ld_32x32b_x64(s_addr + 64, *reinterpret_cast<uint32_t(*)[64]>(&r[64]));
                     tmem_wait_ld();

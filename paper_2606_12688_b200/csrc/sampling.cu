@@ -52,9 +52,11 @@ __device__ __forceinline__ void philox4x32_10(uint32_t (&c)[4], uint32_t k0, uin
     }
 }
 
-// order-preserving map float -> uint32 (larger float, larger key; -0 < +0)
+// order-preserving map float -> uint32 (larger float, larger key; -0 and +0 share the key of +0: they are equal
+// values, and the argmax takes the lowest index among equals)
 __device__ __forceinline__ uint32_t order_key(float z) {
-    const uint32_t b = __float_as_uint(z);
+    uint32_t b = __float_as_uint(z);
+    b = b == 0x80000000u ? 0u : b;
     return b ^ ((b >> 31) ? 0xffffffffu : 0x80000000u);
 }
 
@@ -521,7 +523,7 @@ __device__ bool cs_finish_on_list(CsShared& sh, const uint32_t* keys, int plen, 
     }
     __syncthreads();
     cs_allgather(sh, gen, (uint64_t)sh.ncand, CS);  // its barrier also publishes cand[]
-    uint32_t total = 0, offs[kCsMaxCluster + 1];
+    uint32_t total = 0, offs[kCsMaxCluster];
     bool fits = true;
 #pragma unroll
     for (uint32_t r = 0; r < (uint32_t)kCsMaxCluster; ++r) {
@@ -530,13 +532,16 @@ __device__ bool cs_finish_on_list(CsShared& sh, const uint32_t* keys, int plen, 
         offs[r] = total;
         total += (uint32_t)min(cnt, (uint64_t)kCsGather);
     }
-    offs[kCsMaxCluster] = total;
     if (!fits || total > (uint32_t)kCsGather) return false;
     for (uint32_t g = tid; g < total; g += kCsThreads) {  // all remote loads of a thread in flight together
-        uint32_t r = 0;
+        uint32_t r = 0, first = 0;  // constant indices only: offs[] stays in registers
 #pragma unroll
-        for (uint32_t j = 1; j < (uint32_t)kCsMaxCluster; ++j) r += g >= offs[j];
-        sh.gl[g] = ld_cluster_u32(map_to_rank(smem_u32(&sh.cand[0]), r) + 4u * (g - offs[r]));
+        for (uint32_t j = 1; j < (uint32_t)kCsMaxCluster; ++j)
+            if (g >= offs[j]) {
+                r = j;
+                first = offs[j];
+            }
+        sh.gl[g] = ld_cluster_u32(map_to_rank(smem_u32(&sh.cand[0]), r) + 4u * (g - first));
     }
     __syncthreads();
     // One warp resolves the key bytes on the gathered list (peers read hist[] of level 0 before they arrive at the

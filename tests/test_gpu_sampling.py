@@ -51,7 +51,8 @@ def run(logits, T, K, P, seeds, step, dtype=torch.float32, advance=False, one_ct
     return out.cpu().numpy(), lg.float().cpu().numpy().astype(np.float64), int(st.item())
 
 
-def check_rows(tok, lg64, T, K, P, seeds, step):
+def check_rows(tok, lg64, T, K, P, seeds, step, rows=None):
+    """rows: the row numbers the entries had in the call (the Philox counter holds the row); default 0, 1, ..."""
     exact = 0
     for r in range(len(tok)):
         t = int(tok[r])
@@ -59,7 +60,7 @@ def check_rows(tok, lg64, T, K, P, seeds, step):
         if T[r] == 0:
             assert t == int(np.argmax(lg64[r]))
             continue
-        u = smp.uniform(int(seeds[r]), step, r)
+        u = smp.uniform(int(seeds[r]), step, r if rows is None else int(rows[r]))
         ok, lo, hi = smp.cdf_interval(lg64[r], float(np.float32(T[r])), int(K[r]), float(np.float32(P[r])), t)
         assert ok, "row %d: token %d outside the support" % (r, t)
         assert lo - DELTA <= u <= hi + DELTA, "row %d: u = %.9f not in [%.9f, %.9f]" % (r, u, lo, hi)
@@ -148,6 +149,12 @@ def test_sample_tokens_closed_forms_exact():
     tok, _, _ = run(np.zeros((B, V)), np.ones(B), np.zeros(B), np.ones(B), seeds, 9)
     want = [int(np.floor(smp.uniform(int(seeds[r]), 9, r) * V)) for r in range(B)]
     assert tok.tolist() == want
+    zeros = np.zeros((B, V), np.float32)
+    zeros[:, ::2] = -0.0                               # -0 and +0 are equal values: greedy takes index 0
+    tok, _, _ = run(zeros, np.zeros(B), np.zeros(B), np.ones(B), seeds, 9)
+    assert not tok.any()
+    tok, _, _ = run(zeros, np.ones(B), np.zeros(B), np.ones(B), seeds, 9)
+    assert tok.tolist() == want                        # and sampling sees uniform logits
     rng = np.random.default_rng(3)
     lg = np.float32(rng.normal(0, 2, (B, V)))
     lg[:, ::2] = -np.inf

@@ -176,3 +176,29 @@ def test_gpu_fp8_pool_random_geometry(seed, p, G, L, causal, frac):
                                              b.scale, causal=causal)
             out, _ = db.prefill(causal=causal)
         check_parity(f64_of(out), want, "fp8 %s p=%d G=%d %s" % (kind, p, G, L))
+
+
+@pytest.mark.gpu
+@settings(max_examples=25, **SET)
+@given(seed=st.integers(0, 2 ** 20), V=st.sampled_from([1, 2, 3, 31, 32, 33, 257, 1000, 4096, 4097, 8193, 16385, 20011]),
+       sigma=st.sampled_from([0.0, 0.5, 2.0, 6.0]), bf16=st.booleans(), step=st.sampled_from([0, 1, 2 ** 32 + 3]))
+def test_gpu_sampling_random_rows(seed, V, sigma, bf16, step):
+    """Sampling (R28): every token valid against the oracle's fp64 interval, and the cluster kernel (1, 2, 4 or 8
+    CTAs per row by V) equal to the one-CTA kernel, on random rows with random filters."""
+    import torch
+    from tests.test_gpu_sampling import check_rows, run, unambiguous
+    rng = np.random.default_rng(seed)
+    B = 12
+    dtype = torch.bfloat16 if bf16 else torch.float32
+    lg = np.float32(rng.normal(0, 1, (B, V)) * sigma)
+    T = np.float32(rng.choice([0.0, 0.4, 1.0, 1.9], B))
+    K = rng.choice([0, 1, 3, 40, V], B).astype(np.int32)
+    P = np.float32(rng.choice([1.0, 0.97, 0.6, 0.1], B))
+    seeds = rng.integers(0, 2 ** 62, B)
+    a, lg64, _ = run(lg, T, K, P, seeds, step, dtype=dtype)
+    b, _, _ = run(lg, T, K, P, seeds, step, dtype=dtype, one_cta=True)
+    assert np.array_equal(a, b)
+    ok = np.array([T[r] == 0 or unambiguous(lg64[r], float(T[r]), int(K[r]) if K[r] < V else 0, float(P[r]))
+                   for r in range(B)])
+    if ok.any():   # rows whose top-k / top-p cut is within rounding have several valid supports: not checked
+        check_rows(a[ok], lg64[ok], T[ok], K[ok], P[ok], seeds[ok], step, rows=np.flatnonzero(ok))
