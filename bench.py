@@ -110,6 +110,24 @@ def append_bytes(b):
     return 2 * 2 * b.total_q * b.num_kv_heads * b.head_dim * 2
 
 
+def pack_step_inputs(torch, D, names):
+    """Move the tensors D.<name> into one device buffer (256-byte aligned slices; D.<name> become views into it) and
+    build its pinned host image.  Returns (device buffer, pinned host buffer, bytes of one upload)."""
+    parts = [getattr(D, n) for n in names]
+    offs, total = [], 0
+    for t in parts:
+        total = (total + 255) // 256 * 256
+        offs.append(total)
+        total += t.numel() * t.element_size()
+    dev_buf = torch.zeros(total, dtype=torch.uint8, device=parts[0].device)
+    for n, t, o in zip(names, parts, offs):
+        view = dev_buf[o:o + t.numel() * t.element_size()].view(t.dtype).view(t.shape)
+        view.copy_(t)
+        setattr(D, n, view)
+    host = dev_buf.cpu().pin_memory()
+    return dev_buf, host, total
+
+
 # ----------------------------------------------------------------------------- clocks
 
 class ClockSampler(threading.Thread):
@@ -511,6 +529,10 @@ def run_ours(args):
     bd = W.config5_long_context(num_pages=pool_pages)
     bp = W.config3_prefill()
     D5 = DeviceBatch(bd, device=dev)
+    # the per-step inputs of segment D live back to back in ONE device buffer (the batch's tensors are views into it),
+    # so that the end-to-end step uploads them from pinned host memory with one copy, as a serving engine would
+    step_dev, step_host, h2d = pack_step_inputs(torch, D5, ("q_decode", "k_new", "v_new", "slot_mapping", "block_table",
+                                                           "seq_lens"))
     D3 = DeviceBatch(bp, device=dev)
     NPARTS = 16
     S5, Hq5, Dh = bd.num_seqs, bd.num_q_heads, bd.head_dim
@@ -587,17 +609,11 @@ def run_ours(args):
     tokens_per_s = world * S5 / (t_segD * 1e-3)
 
     # ---- e2e: per-step inputs in pinned host memory, copied in; output copied out; same kernels
-    pin = lambda t: t.detach().cpu().pin_memory()
-    h_in = [pin(D5.q_decode), pin(D5.k_new), pin(D5.v_new), pin(D5.slot_mapping), pin(D5.block_table),
-            pin(D5.seq_lens)]
-    d_in = [D5.q_decode, D5.k_new, D5.v_new, D5.slot_mapping, D5.block_table, D5.seq_lens]
     h_out = torch.empty(out5.shape, dtype=out5.dtype).pin_memory()
-    h2d = sum(t.numel() * t.element_size() for t in h_in)
     d2h = h_out.numel() * h_out.element_size()
 
     def e2e_step():
-        for h, d in zip(h_in, d_in):
-            d.copy_(h, non_blocking=True)
+        step_dev.copy_(step_host, non_blocking=True)
         seg_decode()
         h_out.copy_(out5, non_blocking=True)
 
@@ -683,8 +699,10 @@ def run_ours(args):
                              "frac_of_sustained": pre_tfs / peaks["bf16_tflops_sustained"],
                              "frac_of_nominal_2250": pre_tfs / 2250.0, "ms": t_pre_max, "flops": flops},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms": t_e2e, "note": "segment D with q, new K/V rows, slot mapping, block table and seq_lens in "
-                                     "pinned host memory; the K/V pool is resident serving state"},
+                "ms": t_e2e, "note": "segment D with q, new K/V rows, slot mapping, block table and seq_lens (packed, one upload) in "
+                                     "pinned host memory; the K/V pool is resident serving state.  Steps run back to "
+                                     "back (a step reads 17x the L2 in K/V); the upload leaves the step's inputs in L2, "
+                                     "whereas `value` is timed behind an L2 flush with cold metadata"},
         "gpu_launches": timed_launches,
         "clocks": clocks,
     }
