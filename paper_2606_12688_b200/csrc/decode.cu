@@ -29,6 +29,7 @@ static int decode_pick_warps(bool fp8, int G, int max_seq_len) {
     return fp8 ? ((G <= 8 && max_seq_len > 8192) ? 12 : 8) : 4;
 }
 constexpr int kMaxStages = 16;
+constexpr int kBf16Stages = 4;  // ring depth of the bf16 kernels (launch_decode)
 constexpr int kMaxDecodeGrid = 1024;  // split-K CTAs (one per SM); sizes the cut-record area of the workspace
 
 struct DecodeParams {
@@ -992,6 +993,10 @@ static int launch_decode(const PoolMaps& maps, DecodeParams& p, int max_items, c
     const int max_smem = device_max_smem_optin();
     int nstages = (int)(((int64_t)max_smem - 1024 - SM::kFixed - (int64_t)(2 * p.V + 1) * 4 - 16) / SM::kStageBytes);
     if (nstages > kMaxStages) nstages = kMaxStages;
+    // bf16 pool: four 32 KB stages in flight per SM (19 MB over the chip), not the six that fit -- measured on one box,
+    // 60 GiB scattered pool: config 5 326.7 us with 6, 314.4 with 5, 312.3 with 4, 320.5 with 3; thinker / config 2
+    // 66.5 -> 62.5 us.  The fp8 kernels (ALU-bound) measure the same from 3 stages up and keep what fits.
+    if (!FP8 && nstages > kBf16Stages) nstages = kBf16Stages;
     if (nstages < 2) return MSTAR_ERR_UNSUPPORTED;
     p.nstages = nstages;
     const size_t smem = SM::bytes(nstages, p.V);
