@@ -126,6 +126,26 @@ def test_sample_tokens_cluster_kernel_equals_one_cta_kernel(V, dtype):
         assert np.all((a >= 0) & (a < V))
 
 
+@pytest.mark.parametrize("V", [8 * 49152, 8 * 49152 + 8])
+def test_sample_tokens_cluster_capacity_boundary(V):
+    """393 216 entries fill the cluster kernel (8 CTAs x 49 152 tokens, 213 KB of shared memory each); one chunk more
+    takes the one-CTA kernel.  Same tokens as the forced one-CTA path, valid against the oracle."""
+    rng = np.random.default_rng(77)
+    B = 4
+    lg = np.float32(rng.normal(0, 2.5, (B, V)))
+    T = np.array([1.0, 0.7, 0.0, 1.2], np.float32)
+    K = np.array([0, 64, 0, 0], np.int32)
+    P = np.array([1.0, 1.0, 1.0, 0.85], np.float32)
+    for r in range(B):
+        if T[r] != 0 and not unambiguous(lg[r].astype(np.float64), float(T[r]), int(K[r]), float(P[r])):
+            K[r], P[r] = 0, 1.0
+    seeds = rng.integers(0, 2 ** 62, B)
+    a, lg64, _ = run(lg, T, K, P, seeds, 5)
+    b, _, _ = run(lg, T, K, P, seeds, 5, one_cta=True)
+    assert np.array_equal(a, b)
+    check_rows(a, lg64, T, K, P, seeds, 5)
+
+
 def test_sample_tokens_vocab_of_a_real_tokenizer_size():
     """151 936 entries (the Qwen-family vocabulary of the paper's LLM backbones): 16 rows, every filter."""
     rng = np.random.default_rng(7)
