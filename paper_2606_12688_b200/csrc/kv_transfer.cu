@@ -114,9 +114,13 @@ __global__ void __launch_bounds__(256) kv_gather_kernel(PoolGeom src, const int3
     }
 }
 
-static unsigned copy_grid(int64_t n_chunks, int unroll) {
+// In-flight depth (A/B on one box, thinker pool p = 16 / a 4 x 32768 batch p = 32): copy_pages with 4 loads per thread
+// takes 99.3 / 172.0 us on 4 blocks per SM against 101.3 / 176.1 on 8 and 142 / 226 on 2; the gather with 1 load per
+// thread on 8 blocks per SM 111.6 / 185 us against 121.8 / 183 with 4 loads (its dependent look-ups -- cu_seqlens
+// search, block table -- already keep many rows in flight).
+static unsigned copy_grid(int64_t n_chunks, int unroll, int blocks_per_sm) {
     int64_t blocks = (n_chunks + 256LL * unroll - 1) / (256LL * unroll);
-    const int64_t max_blocks = (int64_t)device_sm_count() * 8;
+    const int64_t max_blocks = (int64_t)device_sm_count() * blocks_per_sm;
     if (blocks > max_blocks) blocks = max_blocks;
     return (unsigned)(blocks < 1 ? 1 : blocks);
 }
@@ -145,7 +149,7 @@ extern "C" int mstar_kv_copy_pages(const mstar_kv_pool* dst_pool, const mstar_kv
     const int32_t cpr = src_pool->head_dim / 8;
     const int64_t n_chunks = num_pairs * src_pool->num_kv_heads * src_pool->page_size * cpr;
     constexpr int UNROLL = 4;
-    kv_copy_pages_kernel<UNROLL><<<copy_grid(n_chunks, UNROLL), 256, 0, (cudaStream_t)stream>>>(
+    kv_copy_pages_kernel<UNROLL><<<copy_grid(n_chunks, UNROLL, 4), 256, 0, (cudaStream_t)stream>>>(
         geom_of(dst_pool), geom_of(src_pool), dst_pages, src_pages, n_chunks, cpr, src_pool->page_size,
         src_pool->num_kv_heads);
     MSTAR_CUDA_OK(cudaGetLastError());
@@ -166,8 +170,8 @@ extern "C" int mstar_kv_gather(void* k_out, void* v_out, const mstar_kv_pool* po
     if (!aligned(k_out, 16) || !aligned(v_out, 16)) return MSTAR_ERR_INVALID_ARG;
     const int32_t cpr = pool->head_dim / 8;
     const int64_t n_chunks = total_tokens * pool->num_kv_heads * cpr;
-    constexpr int UNROLL = 4;
-    kv_gather_kernel<UNROLL><<<copy_grid(n_chunks, UNROLL), 256, 0, (cudaStream_t)stream>>>(
+    constexpr int UNROLL = 1;
+    kv_gather_kernel<UNROLL><<<copy_grid(n_chunks, UNROLL, 8), 256, 0, (cudaStream_t)stream>>>(
         geom_of(pool), block_table, block_table_stride, seq_lens, cu_seqlens_out, num_seqs, (uint16_t*)k_out,
         (uint16_t*)v_out, n_chunks, cpr, pool->page_size, pool->num_kv_heads);
     MSTAR_CUDA_OK(cudaGetLastError());
