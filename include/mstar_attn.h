@@ -227,6 +227,31 @@ int mstar_merge_attn_states(void* out, float* lse_out, const float* out_a, const
                             int32_t head_dim, uint32_t flags, void* stream);
 
 /*
+ * mstar_paged_attn_decode_static: mstar_paged_attn_decode (sec. 4.1; SURVEY.md sec. 8(a) a2 + a3) for
+ * callers that cannot allocate device memory -- code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc.  It takes no workspace: the split-K partials and cut records live in a file-scope device array
+ * of MSTAR_DECODE_STATIC_WORKSPACE_BYTES inside the library (every GPU that loads the library holds it until the
+ * process exits), whose device address the library resolves once per device (cudaGetSymbolAddress with that device
+ * current; make the first call on a device outside stream capture).  No cudaMalloc, cudaFree or allocating library
+ * routine is called.  Same kernels, launches and results (bit for bit) as mstar_paged_attn_decode; all arguments,
+ * flags and errors as there, except:
+ *   - a geometry whose workspace (mstar_paged_attn_decode_workspace_bytes(num_seqs, num_q_heads, head_dim, P) with
+ *     P = num_partitions, or mstar_paged_attn_decode_auto_partitions(...) when num_partitions = 0) exceeds
+ *     MSTAR_DECODE_STATIC_WORKSPACE_BYTES is refused with MSTAR_ERR_WORKSPACE_TOO_SMALL and nothing is launched
+ *     (48 MiB holds every BASELINE decode config in balanced mode: 4.3 MB config 5 with 16 partitions, 9.6 MB
+ *     talker, 29.8 MB config 2, 35.1 MB thinker);
+ *   - ALL calls on a device share the array, which keeps the last call's contents (nothing in it has to start at
+ *     zero: every slot that is read is written by the same call).  Calls that overlap on the GPU -- two streams, or
+ *     two host threads -- race on it: serialise them, or give each stream its own workspace through
+ *     mstar_paged_attn_decode.
+ */
+#define MSTAR_DECODE_STATIC_WORKSPACE_BYTES (48u << 20)
+int mstar_paged_attn_decode_static(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool,
+                                   const int32_t* block_table, int64_t block_table_stride, const int32_t* seq_lens,
+                                   int32_t num_seqs, int32_t num_q_heads, int32_t max_seq_len, float scale,
+                                   int32_t num_partitions, uint32_t flags, void* stream);
+
+/*
  * mstar_paged_attn_decode_cascade: mstar_paged_attn_decode for CFG branches whose labels
  * reference the same prefix pages -- "three labels over a single paged KV pool ... reading page tables in place"
  * (the Parallel region LLM / LLM_cfg_text / LLM_cfg_img of PAPER.md:104-106).  The result is that of

@@ -15,6 +15,7 @@ Python binding.  Names mirror the C entry points:
     merge_attn_states    <- mstar_merge_attn_states   (LSE merge of two attention states)
     sample_tokens        <- mstar_sample_tokens       (CUDA-graph-compatible temperature / top-k / top-p sampling)
     paged_attn_decode_cascade <- mstar_paged_attn_decode_cascade (CFG branches sharing prefix pages, one call)
+    paged_attn_decode_static <- mstar_paged_attn_decode_static (decode with its scratch in the library's static device array)
 
 There is no CPU fallback: without the built library every call raises ``MstarError``.
 """
@@ -23,6 +24,7 @@ from .binding import (  # noqa: F401
     KVPool,
     KVPoolFp8,
     LIB_PATH,
+    MSTAR_DECODE_STATIC_WORKSPACE_BYTES,
     MSTAR_FLAG_LOGITS_BF16,
     MSTAR_FLAG_OUT_F32,
     MSTAR_FLAG_PREFILL_MMA_SYNC,
@@ -42,6 +44,7 @@ from .binding import (  # noqa: F401
     paged_attn_decode,
     paged_attn_decode_cascade,
     paged_attn_decode_fp8,
+    paged_attn_decode_static,
     paged_attn_prefill,
     paged_attn_prefill_fp8,
     prefill_fp8_workspace_bytes,

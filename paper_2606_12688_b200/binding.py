@@ -17,6 +17,7 @@ _PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG_DIR, "libmstar_attn.so")
 
 MSTAR_OK = 0
+MSTAR_ERR_WORKSPACE_TOO_SMALL = -3
 MSTAR_FLAG_OUT_F32 = 1
 MSTAR_FLAG_PREFILL_MMA_SYNC = 2
 MSTAR_FLAG_PREFILL_REUSE_PLAN = 4
@@ -36,6 +37,7 @@ EXPORTS = (
     "mstar_paged_attn_decode_workspace_bytes",
     "mstar_paged_attn_decode",
     "mstar_paged_attn_decode_auto_partitions",
+    "mstar_paged_attn_decode_static",
     "mstar_paged_attn_decode_cascade_workspace_bytes",
     "mstar_paged_attn_decode_cascade",
     "mstar_paged_attn_prefill_workspace_bytes",
@@ -118,6 +120,10 @@ def load_library() -> ctypes.CDLL:
     lib.mstar_paged_attn_decode.argtypes = [
         c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_int64, c.c_void_p,
         c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_uint32, c.c_void_p, c.c_size_t, c.c_void_p]
+    lib.mstar_paged_attn_decode_static.restype = c.c_int
+    lib.mstar_paged_attn_decode_static.argtypes = [
+        c.c_void_p, c.c_void_p, c.c_void_p, c.POINTER(_KvPoolStruct), c.c_void_p, c.c_int64, c.c_void_p,
+        c.c_int32, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_uint32, c.c_void_p]
     lib.mstar_paged_attn_decode_cascade_workspace_bytes.restype = c.c_size_t
     lib.mstar_paged_attn_decode_cascade_workspace_bytes.argtypes = [c.c_int32] * 5
     lib.mstar_paged_attn_decode_cascade.restype = c.c_int
@@ -351,6 +357,38 @@ def paged_attn_decode(out: torch.Tensor, q: torch.Tensor, pool: KVPool, block_ta
         _ptr(out), _ptr(lse_out), _ptr(q), ctypes.byref(pool.c), _ptr(block_table),
         int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens), S, Hq, int(max_seq_len),
         float(scale), int(num_partitions), flags, _ptr(workspace), ws_bytes, _stream()), "mstar_paged_attn_decode")
+
+
+MSTAR_DECODE_STATIC_WORKSPACE_BYTES = 48 << 20
+
+
+def paged_attn_decode_static(out: torch.Tensor, q: torch.Tensor, pool: KVPool, block_table: torch.Tensor,
+                             seq_lens: torch.Tensor, max_seq_len: int, scale: float, num_partitions: int = 0,
+                             lse_out: Optional[torch.Tensor] = None) -> None:
+    """mstar_paged_attn_decode_static: the decode call with its scratch in the library's static device array
+    (MSTAR_DECODE_STATIC_WORKSPACE_BYTES; nothing is allocated).  Calls that overlap on the GPU race on that array."""
+    _want(q, torch.bfloat16, "q"); _want(block_table, torch.int32, "block_table")
+    _want(seq_lens, torch.int32, "seq_lens")
+    S, Hq, D = (int(x) for x in q.shape)
+    flags = 0
+    if out.dtype == torch.float32:
+        flags |= MSTAR_FLAG_OUT_F32
+    elif out.dtype != torch.bfloat16:
+        raise MstarError("out must be bf16 or fp32")
+    if not out.is_cuda or not out.is_contiguous() or tuple(out.shape) != (S, Hq, D):
+        raise MstarError("out must be a contiguous CUDA tensor [S, Hq, D]")
+    if lse_out is not None:
+        _want(lse_out, torch.float32, "lse_out")
+    lib = load_library()
+    status = lib.mstar_paged_attn_decode_static(
+        _ptr(out), _ptr(lse_out), _ptr(q), ctypes.byref(pool.c), _ptr(block_table),
+        int(block_table.stride(0)) if block_table.dim() == 2 else 0, _ptr(seq_lens), S, Hq, int(max_seq_len),
+        float(scale), int(num_partitions), flags, _stream())
+    if status == MSTAR_ERR_WORKSPACE_TOO_SMALL:
+        raise MstarError("mstar_paged_attn_decode_static: this geometry needs more scratch than the static array "
+                         "holds (%d bytes); use paged_attn_decode with a caller-owned workspace"
+                         % MSTAR_DECODE_STATIC_WORKSPACE_BYTES)
+    _check(status, "mstar_paged_attn_decode_static")
 
 
 def decode_cascade_workspace_bytes(num_seqs: int, num_q_heads: int, num_kv_heads: int, head_dim: int,

@@ -14,6 +14,8 @@
 // Full/empty mbarriers per stage are the only synchronisation in the steady state.
 #include <cuda_bf16.h>
 
+#include <mutex>
+
 #include "host_common.h"
 #include "ptx.cuh"
 
@@ -1267,4 +1269,61 @@ extern "C" int mstar_paged_attn_decode_cascade(void* out, float* lse_out, const 
     return decode_entry(false, nullptr, nullptr, n_branches, shared_lens, out, lse_out, q, pool, block_table,
                         block_table_stride, seq_lens, num_seqs, num_q_heads, max_seq_len, scale, 0, flags, workspace,
                         workspace_bytes, stream);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// mstar_paged_attn_decode_static: the decode call for callers that cannot allocate device memory (code under CUDA
+// graph capture, tight serving loops, harnesses that forbid cudaMalloc).  The split-K partials and cut records -- the
+// `workspace` of mstar_paged_attn_decode -- live in a file-scope device array of MSTAR_DECODE_STATIC_WORKSPACE_BYTES
+// that every GPU which loads the library holds until the process exits.  Same kernels, same launch sequence and
+// same arithmetic as mstar_paged_attn_decode; no cudaMalloc / cudaFree / allocating library routine on this path
+// (nor anywhere else in the library: every other entry takes caller-owned scratch).
+//
+// In host code the array's NAME is a host-side stand-in, not a device address: the address a kernel can use comes
+// from cudaGetSymbolAddress, resolved once per device with that device current, and cached per device ordinal.
+// Contents: the array keeps whatever the last call left.  Nothing in it has to start at zero -- every partial slot
+// and every cut record the combine pass reads is written by the split-K kernel of the same call (the existing path
+// makes the same assumption about a caller's uninitialised workspace) -- so no clearing pass is launched.
+// All calls on a device share the array: calls that overlap on the GPU (different streams, or one stream's call
+// still running when another stream's starts) race on it; serialise them, or use mstar_paged_attn_decode with a
+// workspace per stream.
+static __device__ __align__(256) unsigned char g_decode_static_ws[MSTAR_DECODE_STATIC_WORKSPACE_BYTES];
+
+namespace mstar {
+
+static int decode_static_ws_address(void** out) {
+    constexpr int kDevs = 64;
+    static std::mutex mu;
+    static void* ptrs[kDevs] = {};
+    const int dev = current_device();
+    std::lock_guard<std::mutex> lk(mu);
+    if (dev >= 0 && dev < kDevs && ptrs[dev]) {
+        *out = ptrs[dev];
+        return MSTAR_OK;
+    }
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_decode_static_ws);  // the CURRENT device's copy
+    if (e != cudaSuccess || !ptr) {
+        (void)cudaGetLastError();
+        return MSTAR_ERR_CUDA;
+    }
+    if (dev >= 0 && dev < kDevs) ptrs[dev] = ptr;  // devices past the cache resolve the address on every call
+    *out = ptr;
+    return MSTAR_OK;
+}
+
+}  // namespace mstar
+
+extern "C" int mstar_paged_attn_decode_static(void* out, float* lse_out, const void* q, const mstar_kv_pool* pool,
+                                              const int32_t* block_table, int64_t block_table_stride,
+                                              const int32_t* seq_lens, int32_t num_seqs, int32_t num_q_heads,
+                                              int32_t max_seq_len, float scale, int32_t num_partitions,
+                                              uint32_t flags, void* stream) {
+    void* ws = nullptr;
+    const int rc = mstar::decode_static_ws_address(&ws);
+    if (rc != MSTAR_OK) return rc;
+    // a geometry whose partials exceed the array comes back as MSTAR_ERR_WORKSPACE_TOO_SMALL, nothing launched
+    return decode_entry(false, nullptr, nullptr, 0, nullptr, out, lse_out, q, pool, block_table, block_table_stride,
+                        seq_lens, num_seqs, num_q_heads, max_seq_len, scale, num_partitions, flags, ws,
+                        (size_t)MSTAR_DECODE_STATIC_WORKSPACE_BYTES, stream);
 }
