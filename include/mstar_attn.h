@@ -51,9 +51,8 @@ typedef enum {
 #define MSTAR_FLAG_OUT_F32 1u /* `out` is fp32 instead of bf16 (diagnostic: separates kernel error from
                                  output rounding).  Unknown bits => MSTAR_ERR_INVALID_ARG. */
 #define MSTAR_FLAG_PREFILL_MMA_SYNC 2u /* prefill only, diagnostic: use the warp-level mma.sync kernel instead
-                                          of the tcgen05/TMEM kernel.  head_dim 64 always takes this kernel: it is
-                                          a correctness path (about a fifth of the tcgen05 kernel's rate), no
-                                          BASELINE config prefills at head_dim 64. */
+                                          of the tcgen05/TMEM kernel (about a fifth of its rate at head_dim 128,
+                                          0.4 at head_dim 64).  Both head dims take the tcgen05 kernel otherwise. */
 
 #define MSTAR_FLAG_PREFILL_REUSE_PLAN 4u /* prefill only: `workspace` still holds the plan a previous call built
                                           for the SAME cu_seqlens_q, seq_lens, head geometry and causal flag (the

@@ -39,12 +39,12 @@ int get_pool_maps_fp8(const mstar_kv_pool* pool, PoolMaps* out);
 int make_rows_map(const void* base, int64_t rows, int32_t num_heads, int32_t head_dim, int32_t box_rows,
                   CUtensorMap* out);
 
-// tcgen05 / TMEM prefill kernel (prefill_umma.cu); head_dim 128 only
+// tcgen05 / TMEM prefill kernel (prefill_umma.cu); head_dim 128, or 64 on a bf16 pool
 int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, const int32_t* cu_seqlens_q,
                         const int32_t* block_table, int64_t bt_stride, const int32_t* seq_lens, int32_t S,
                         int32_t Hq, int32_t Hkv, int32_t page_size, int32_t max_q_len, float scale, int32_t causal,
                         void* out, float* lse, int32_t out_f32, int32_t reuse_plan, void* workspace,
-                        size_t workspace_bytes, cudaStream_t stream, int32_t kv_f16 = 0);
+                        size_t workspace_bytes, cudaStream_t stream, int32_t kv_f16 = 0, int32_t head_dim = 128);
 size_t prefill_umma_workspace_bytes(int32_t num_seqs, int32_t total_q, int32_t num_q_heads);
 
 // Properties of the CURRENT device (cudaGetDevice), cached per device ordinal; thread-safe.

@@ -341,11 +341,11 @@ extern "C" int mstar_paged_attn_prefill(void* out, float* lse_out, const void* q
     if (rc != MSTAR_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const int D = pool->head_dim, PAGE = pool->page_size;
-    if (D == 128 && p.G <= 128 && !(flags & MSTAR_FLAG_PREFILL_MMA_SYNC))  // tcgen05 / TMEM path
+    if ((D == 128 || D == 64) && p.G <= 128 && !(flags & MSTAR_FLAG_PREFILL_MMA_SYNC))  // tcgen05 / TMEM path
         return launch_prefill_umma(maps, q, total_q, cu_seqlens_q, block_table, block_table_stride, seq_lens, num_seqs,
                                    num_q_heads, pool->num_kv_heads, PAGE, max_q_len, scale, p.causal, out, lse_out,
                                    p.out_f32, (flags & MSTAR_FLAG_PREFILL_REUSE_PLAN) ? 1 : 0, workspace,
-                                   workspace_bytes, st);
+                                   workspace_bytes, st, /*kv_f16=*/0, D);
     if (D == 128 && PAGE == 16) return launch_prefill<128, 16>(maps, p, st);
     if (D == 128 && PAGE == 32) return launch_prefill<128, 32>(maps, p, st);
     if (D == 64 && PAGE == 16) return launch_prefill<64, 16>(maps, p, st);

@@ -184,12 +184,16 @@ __device__ __forceinline__ PuDesc pu_read_desc(const uint8_t* gbase, int uslot) 
 // fault, measured), so warps 10 and 11 -- idle in the bf16 kernel -- convert the Q tiles of every unit from bf16 to
 // fp16 in shared memory as soon as they land (exact for |q| in [2^-14, 65504]) and hand them to the MMA warp, and P
 // is rounded to fp16: Q K^T and P V are f16 x f16 MMAs.
-template <int PAGE, bool F16>
+// D = head_dim, 128 or 64.  head_dim 64 uses the first 64-column half of every Q / K / V tile and staging buffer and
+// the first 64 TMEM columns of each O accumulator (Q K^T contracts over 4 instead of 8 k-steps, P V has N = 64); the
+// shared-memory and TMEM maps stay those of head_dim 128.
+template <int PAGE, bool F16, int D = 128>
 __global__ void __launch_bounds__(kPuThreads, 1)
 prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_constant__ CUtensorMap kmap,
                     const __grid_constant__ CUtensorMap vmap, const __grid_constant__ CUtensorMap omap,
                     const PrefillUmmaParams p) {
-    constexpr int D = 128;
+    static_assert(D == 128 || D == 64, "head_dim");
+    constexpr int NH = D / 64;          // 64-column half tiles per row
     constexpr int PPS = kPuTok / PAGE;  // pages per stage
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -243,10 +247,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             const uint64_t pol_kv = policy_evict_last();   // K/V re-read by other query blocks of the sequence
             const uint64_t pol_q = policy_evict_first();
             // lane -> (K or V, page, half): PPS*2 ops for K on the low lanes, PPS*2 for V after them
-            constexpr int OPS1 = PPS * 2;
+            constexpr int OPS1 = PPS * NH;
             const int op_isv = lane / OPS1;
-            const int op_page = (lane % OPS1) / 2;
-            const int op_half = lane & 1;
+            const int op_page = (lane % OPS1) / NH;
+            const int op_half = lane % NH;
             const bool op_on = lane < 2 * OPS1;
             const PuDesc* list = reinterpret_cast<const PuDesc*>(p.plan + kPlanHeaderInts);
             // Lane 0 owns the scheduler state.  Fetches are pipelined two units deep: the atomic for unit
@@ -301,9 +305,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 for (int t = 0; t < 2; ++t) {
                     mbar_wait(bar(B_QEMPTY0 + t), qph[t] ^ 1);
                     qph[t] ^= 1;
-                    if (lane == 0) mbar_arrive_expect_tx(bar(B_QFULL0 + t), (uint32_t)(2 * rows_used * 128));
+                    if (lane == 0) mbar_arrive_expect_tx(bar(B_QFULL0 + t), (uint32_t)(NH * rows_used * 128));
                     __syncwarp();
-                    if (lane < 2)  // half
+                    if (lane < NH)  // half
                         tma_load_3d(base + kPuQ + (t * 2 + lane) * kPuHT, &qmap, bar(B_QFULL0 + t), lane * 64,
                                     x.kvh * p.G, x.r0 + x.t0 + t * p.tq, pol_q);
                 }
@@ -351,7 +355,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             // =============================== MMA ISSUER ===============================
             const uint32_t fmt = F16 ? 0u : 1u;  // operand format of Q, K, P and V
             const uint32_t idesc_qk = umma_idesc_f16(128, 128, fmt, fmt, 0, 0);
-            const uint32_t idesc_pv = umma_idesc_f16(128, 128, fmt, fmt, 0, 1);
+            const uint32_t idesc_pv = umma_idesc_f16(128, D, fmt, fmt, 0, 1);
             uint32_t qph[2] = {0, 0}, kph = 0, vph = 0, pph[2] = {0, 0}, oeph = 0, uph = 0;
             int ks = 0, vs = 0, uslot = 0;
             // Descriptors differ only in the 14-bit start-address field (bytes >> 4) of their low word: the bases are
@@ -364,7 +368,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                     const uint64_t a0 = dq + (uint64_t)(t * 2 * (kPuHT >> 4));
                     const uint64_t b0 = dk + (uint64_t)(kslot * 2 * (kPuHT >> 4));
 #pragma unroll
-                    for (int k = 0; k < 8; ++k) {
+                    for (int k = 0; k < D / 16; ++k) {
                         const uint32_t off = (uint32_t)((k >> 2) * (kPuHT >> 4) + (k & 3) * 2);
                         umma_ss(tmem + t * 128, a0 + off, b0 + off, idesc_qk, k > 0);
                     }
@@ -418,7 +422,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                             uint8_t* vg = gbase + kPuV + vs * 2 * kPuHT;
                             for (int i = nvalid * 8 + lane; i < kPuTok * 8; i += 32) {  // 16-B chunks of 128-B rows
                                 *reinterpret_cast<int4*>(vg + i * 16) = make_int4(0, 0, 0, 0);
-                                *reinterpret_cast<int4*>(vg + kPuHT + i * 16) = make_int4(0, 0, 0, 0);
+                                if (NH == 2) *reinterpret_cast<int4*>(vg + kPuHT + i * 16) = make_int4(0, 0, 0, 0);
                             }
                             fence_proxy_async_smem();
                             __syncwarp();
@@ -449,7 +453,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                                 const uint64_t a0 = dq + (uint64_t)(t * 2 * (kPuHT >> 4));
                                 const uint64_t b0 = dk + (uint64_t)(ks * 2 * (kPuHT >> 4));
 #pragma unroll
-                                for (int k = 0; k < 8; ++k) {
+                                for (int k = 0; k < D / 16; ++k) {
                                     const uint32_t off = (uint32_t)((k >> 2) * (kPuHT >> 4) + (k & 3) * 2);
                                     umma_ss(tmem + t * 128, a0 + off, b0 + off, idesc_qk, k > 0);
                                 }
@@ -488,7 +492,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 qph ^= 1;
                 const uint32_t qt = base + kPuQ + t * 2 * kPuHT;
 #pragma unroll 4
-                for (int c = lane; c < 2 * kPuHT / 16; c += 32) {
+                for (int c = lane; c < NH * kPuHT / 16; c += 32) {
                     uint32_t w0, w1, w2, w3;
                     ld_shared_v4(qt + c * 16, w0, w1, w2, w3);
                     st_shared_v4(qt + c * 16, bf16x2_to_f16x2(w0), bf16x2_to_f16x2(w1), bf16x2_to_f16x2(w2),
@@ -579,7 +583,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                         l *= alpha;
                         m_ref = m_new;
 #pragma unroll
-                        for (int cb = 0; cb < 4; ++cb) {
+                        for (int cb = 0; cb < D / 32; ++cb) {
                             uint32_t o[32];
                             tmem_ld_32x32b_x32(o_addr + cb * 32, o);
                             tmem_wait_ld();
@@ -644,16 +648,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             tc_fence_after();
             const float inv = 1.f / l;
             const size_t orow = ((size_t)(x.r0 + tok) * p.Hq + (size_t)x.kvh * p.G + head_l) * D;
-            uint32_t r[128];
+            uint32_t r[D];
             {
-                uint32_t(&r0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[0]);
-                uint32_t(&r1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[32]);
-                uint32_t(&r2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[64]);
-                uint32_t(&r3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&r[96]);
-                tmem_ld_32x32b_x32(o_addr, r0);
-                tmem_ld_32x32b_x32(o_addr + 32, r1);
-                tmem_ld_32x32b_x32(o_addr + 64, r2);
-                tmem_ld_32x32b_x32(o_addr + 96, r3);
+#pragma unroll
+                for (int cb = 0; cb < D / 32; ++cb)
+                    tmem_ld_32x32b_x32(o_addr + cb * 32, *reinterpret_cast<uint32_t(*)[32]>(&r[cb * 32]));
                 tmem_wait_ld();
             }
             // O is in registers: the tensor core may start the next unit's P V on this tile
@@ -667,7 +666,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
             if (via_tma) {
                 const uint32_t obuf = base + kPuO + t * kPuHT;
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
+                for (int h = 0; h < NH; ++h) {
                     // the previous store out of this buffer must have finished reading it
                     if ((warp & 3) == 0 && lane == 0) bulk_wait_group_read0();
                     named_bar_sync(1 + t, 128);
@@ -694,14 +693,14 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
                 if (p.out_f32) {
                     float* o = reinterpret_cast<float*>(p.out) + orow;
 #pragma unroll
-                    for (int i = 0; i < 128; i += 4)
+                    for (int i = 0; i < D; i += 4)
                         *reinterpret_cast<float4*>(o + i) =
                             make_float4(__uint_as_float(r[i]) * inv, __uint_as_float(r[i + 1]) * inv,
                                         __uint_as_float(r[i + 2]) * inv, __uint_as_float(r[i + 3]) * inv);
                 } else if (!via_tma) {
                     uint16_t* o = reinterpret_cast<uint16_t*>(p.out) + orow;
 #pragma unroll
-                    for (int i = 0; i < 128; i += 8) {
+                    for (int i = 0; i < D; i += 8) {
                         int4 v;
                         v.x = (int)pack_bf16x2(__uint_as_float(r[i]) * inv, __uint_as_float(r[i + 1]) * inv);
                         v.y = (int)pack_bf16x2(__uint_as_float(r[i + 2]) * inv, __uint_as_float(r[i + 3]) * inv);
@@ -723,7 +722,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap qmap, const __grid_const
 }
 
 // 3-D view (D, Hq, total_q) of a [total_q][Hq][128] bf16 tensor with box (64, G, tq) and 128-byte swizzle
-static int make_q_view_map(const void* ptr, int32_t total_q, int32_t Hq, int32_t G, int32_t tq, CUtensorMap* out) {
+static int make_q_view_map(const void* ptr, int32_t total_q, int32_t Hq, int32_t G, int32_t tq, int32_t D,
+                           CUtensorMap* out) {
     typedef CUresult (*Fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                            const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                            CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -738,8 +738,8 @@ static int make_q_view_map(const void* ptr, int32_t total_q, int32_t Hq, int32_t
         }
         encode = reinterpret_cast<Fn>(fp);
     }
-    cuuint64_t dims[3] = {128, (cuuint64_t)Hq, (cuuint64_t)total_q};
-    cuuint64_t strides[2] = {256, (cuuint64_t)Hq * 256};
+    cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)total_q};
+    cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)Hq * D * 2};
     cuuint32_t box[3] = {64, (cuuint32_t)G, (cuuint32_t)tq};
     cuuint32_t es[3] = {1, 1, 1};
     if (encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, es,
@@ -759,7 +759,8 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
                         const int32_t* block_table, int64_t bt_stride, const int32_t* seq_lens, int32_t S,
                         int32_t Hq, int32_t Hkv, int32_t page_size, int32_t max_q_len, float scale, int32_t causal,
                         void* out, float* lse, int32_t out_f32, int32_t reuse_plan, void* workspace,
-                        size_t workspace_bytes, cudaStream_t stream, int32_t kv_f16) {
+                        size_t workspace_bytes, cudaStream_t stream, int32_t kv_f16, int32_t head_dim) {
+    if (head_dim != 128 && !(head_dim == 64 && !kv_f16)) return MSTAR_ERR_UNSUPPORTED;
     PrefillUmmaParams p{};
     p.block_table = block_table;
     p.bt_stride = bt_stride;
@@ -780,13 +781,13 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
     // Q view: dims (D, Hq, total_q); box (64, G, tq): rows of a tile = token * G + head
     CUtensorMap qmap;
     {
-        const int st = make_q_view_map(q, total_q, Hq, p.G, p.tq, &qmap);
+        const int st = make_q_view_map(q, total_q, Hq, p.G, p.tq, head_dim, &qmap);
         if (st != MSTAR_OK) return st;
     }
     // output view for the TMA-store epilogue: same geometry as the Q view (bf16 output only)
     CUtensorMap omap = qmap;
     if (!out_f32) {
-        const int st = make_q_view_map(out, total_q, Hq, p.G, p.tq, &omap);
+        const int st = make_q_view_map(out, total_q, Hq, p.G, p.tq, head_dim, &omap);
         if (st != MSTAR_OK) return st;
     }
     if (!reuse_plan) {
@@ -797,11 +798,14 @@ int launch_prefill_umma(const PoolMaps& maps, const void* q, int32_t total_q, co
     int grid = device_sm_count();
     if (grid > max_units) grid = (int)max_units;
     if (grid < 1) grid = 1;
-    auto k16 = kv_f16 ? prefill_umma_kernel<16, true> : prefill_umma_kernel<16, false>;
-    auto k32 = kv_f16 ? prefill_umma_kernel<32, true> : prefill_umma_kernel<32, false>;
-    static PerDeviceOnce once16, once32, once16h, once32h;
-    MSTAR_CUDA_OK(set_max_dynamic_smem(kv_f16 ? once16h : once16, k16, kPuSmemBytes));
-    MSTAR_CUDA_OK(set_max_dynamic_smem(kv_f16 ? once32h : once32, k32, kPuSmemBytes));
+    const bool d64 = head_dim == 64;
+    auto k16 = kv_f16 ? prefill_umma_kernel<16, true, 128>
+                      : (d64 ? prefill_umma_kernel<16, false, 64> : prefill_umma_kernel<16, false, 128>);
+    auto k32 = kv_f16 ? prefill_umma_kernel<32, true, 128>
+                      : (d64 ? prefill_umma_kernel<32, false, 64> : prefill_umma_kernel<32, false, 128>);
+    static PerDeviceOnce once16, once32, once16h, once32h, once16s, once32s;
+    MSTAR_CUDA_OK(set_max_dynamic_smem(kv_f16 ? once16h : (d64 ? once16s : once16), k16, kPuSmemBytes));
+    MSTAR_CUDA_OK(set_max_dynamic_smem(kv_f16 ? once32h : (d64 ? once32s : once32), k32, kPuSmemBytes));
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3(kPuThreads);

@@ -54,6 +54,17 @@ def test_prefill_adversarial_other_group_sizes(kind, G, p):
     tpar.run_prefill_case(b)
 
 
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("G,p", [(7, 16), (8, 32)])
+def test_prefill_adversarial_head_dim_64(kind, G, p):
+    """The head_dim-64 instantiation of the tcgen05 kernel (one 64-column half per tile, P V with N = 64, the lazy
+    rescale over 64 TMEM columns): every adversarial kind over up to 17 KV stages, causal and flow-step mask."""
+    b = adv_batch(kind, [1200, 700, 129, 2100], [400, 700, 129, 260], seed=540 + KINDS.index(kind), Hq=2 * G, Hkv=2,
+                  D=64, p=p)
+    tpar.run_prefill_case(b)
+    tpar.run_prefill_case(b, causal=False)
+
+
 def test_prefill_ramp_rescales_o_in_tmem_with_fp32_output():
     """The ramp with fp32 output: kernel error alone (bf16 P, lazy rescale of O and l) without output rounding."""
     b = adv_batch("ramp", [1500, 640], [700, 640], seed=530)
