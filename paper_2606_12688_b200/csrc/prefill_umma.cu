@@ -102,18 +102,33 @@ prefill_plan_kernel(const int32_t* __restrict__ cu_seqlens_q, const int32_t* __r
         if (unit_of(i, d)) atomicAdd(&hist[min(d.T, kPlanBuckets - 1)], Hkv);
     }
     __syncthreads();
-    // inclusive suffix sum: scan[b] = sum over b' >= b of hist[b']  (heaviest bucket first in the list)
-    const int mine = hist[tid];
-    scan[tid] = mine;
-    __syncthreads();
-    for (int off = 1; off < kPlanBuckets; off <<= 1) {
-        const int add = (tid + off < kPlanBuckets) ? scan[tid + off] : 0;
-        __syncthreads();
-        scan[tid] += add;
-        __syncthreads();
+    // suffix sums (heaviest bucket first in the list): thread tid owns bucket b = last - tid, so an inclusive PREFIX
+    // scan over tid is the sum over the buckets >= b; warp shuffles + one pass over the 32 warp totals (the
+    // log-step scan through shared memory cost 20 block barriers, a third of this kernel's time)
+    const int b = kPlanBuckets - 1 - tid, lane = tid & 31, wrp = tid >> 5;
+    const int mine = hist[b];
+    int incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
     }
-    const int num_units = scan[0];
-    hist[tid] = scan[tid] - mine;  // cursor: first list position of bucket tid
+    if (lane == 31) scan[wrp] = incl;
+    __syncthreads();
+    if (wrp == 0) {
+        const int w = scan[lane];
+        int wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += t;
+        }
+        scan[32 + lane] = wi - w;      // exclusive offset of warp `lane`
+        if (lane == 31) scan[64] = wi;  // all units
+    }
+    __syncthreads();
+    const int num_units = scan[64];
+    hist[b] = incl + scan[32 + wrp] - mine;  // cursor: first list position of bucket b
     __syncthreads();
     PuDesc* list = reinterpret_cast<PuDesc*>(plan + kPlanHeaderInts);
     for (int64_t i = tid; i < total; i += kPlanBuckets) {
