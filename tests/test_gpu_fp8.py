@@ -122,10 +122,30 @@ def test_decode_fp8_len1_is_the_dequantised_v_row():
         pg = int(b.compact_block_table[s, 0])
         for h in range(8):
             g = h // 4
-            # p = 1, l = 1: out = bf16(v_scale) ... the kernel folds v_scale into P (rounded to bf16), so the row is the
-            # code values times bf16(v_scale)
-            vs_b = float(torch.tensor(float(vs[pg, g])).to(torch.bfloat16).to(torch.float64))
-            assert np.array_equal(got[s, h], (t[v8[pg, g, 0]] * vs_b).astype(np.float32).astype(np.float64))
+            # p = 1, l = 1: the row is the code values times v_scale.  The kernel folds v_scale into P as a bf16
+            # operand and, in items of a single stage, feeds the residual of that rounding through a second MMA: what
+            # is left is 2^-16 relative (before that residual pass the row was codes * bf16(v_scale), 2^-8 relative)
+            want = t[v8[pg, g, 0]] * float(vs[pg, g])
+            assert np.all(np.abs(got[s, h] - want) <= np.abs(want) * 2.0 ** -15)
+
+
+def test_decode_fp8_short_rows_found_by_the_soak_run():
+    """The example the property tests found at 20 x their examples (MSTAR_SOAK=20): rows of one token whose |v| is
+    3.4, where the rounding of p * v_scale to a bf16 operand and the output rounding added up to 2.03e-2.  Single-stage
+    items now carry the residual of that rounding through a second MMA."""
+    from tests.test_properties import decode_batch
+    seed, p, G, L = 195, 32, 4, [1, 257, 1, 33, 257]
+    b = decode_batch(seed, (p, 128, G, 2), L)
+    ks, vs = W.fp8_page_scales(seed % 97, b.num_pages, b.num_kv_heads)
+    db = DeviceBatchFp8(b, ks, vs)
+    db.quantise_store()
+    db.append()
+    k8, v8, cks, cvs = oracle_pool(b, ks, vs)
+    want, _ = ofp8.paged_decode_fp8(decode_q(b), k8, v8, cks, cvs, b.compact_block_table, b.seq_lens, b.scale)
+    for parts in (0, 1, 3):
+        out, _ = db.decode(num_partitions=parts)
+        a, _ = check_parity(f64_of(out), want, "soak example parts=%d" % parts)
+        assert a <= 1.6e-2     # |out| < 4: the output's own rounding is 7.8e-3, the rest is the arithmetic's
 
 
 def test_decode_fp8_subnormal_codes_are_exact():

@@ -16,6 +16,14 @@ geometry = st.tuples(st.sampled_from([16, 32]), st.sampled_from([64, 128]), st.s
                      st.sampled_from([1, 2, 3]))
 lens = st.lists(st.sampled_from(EDGE), min_size=1, max_size=6)
 SET = dict(deadline=None, derandomize=True, suppress_health_check=list(HealthCheck))
+# soak runs: MSTAR_SOAK=k multiplies the number of examples of every property below (profiles/r2_sanitizer.md)
+import os as _os
+_SOAK = max(1, int(_os.environ.get("MSTAR_SOAK", "1")))
+_settings = settings
+
+
+def settings(max_examples=100, **kw):   # noqa: F811 -- the decorator below, scaled
+    return _settings(max_examples=max_examples * _SOAK, **kw)
 
 
 def decode_batch(seed, geo, L):
