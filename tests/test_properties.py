@@ -15,10 +15,12 @@ EDGE = [0, 1, 2, 15, 16, 17, 31, 32, 33, 63, 64, 65, 127, 128, 129, 200, 257]
 geometry = st.tuples(st.sampled_from([16, 32]), st.sampled_from([64, 128]), st.sampled_from([1, 4, 7, 8]),
                      st.sampled_from([1, 2, 3]))
 lens = st.lists(st.sampled_from(EDGE), min_size=1, max_size=6)
-SET = dict(deadline=None, derandomize=True, suppress_health_check=list(HealthCheck))
-# soak runs: MSTAR_SOAK=k multiplies the number of examples of every property below (profiles/r2_sanitizer.md)
+# soak runs (profiles/r2_sanitizer.md): MSTAR_SOAK=k multiplies the number of examples of every property below;
+# MSTAR_SOAK_RANDOM=1 lifts the derandomisation, so that `pytest --hypothesis-seed=N` draws other examples
 import os as _os
 _SOAK = max(1, int(_os.environ.get("MSTAR_SOAK", "1")))
+SET = dict(deadline=None, derandomize=not _os.environ.get("MSTAR_SOAK_RANDOM"), database=None,
+           suppress_health_check=list(HealthCheck))
 _settings = settings
 
 
