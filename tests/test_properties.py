@@ -212,3 +212,47 @@ def test_gpu_sampling_random_rows(seed, V, sigma, bf16, step):
                    for r in range(B)])
     if ok.any():   # rows whose top-k / top-p cut is within rounding have several valid supports: not checked
         check_rows(a[ok], lg64[ok], T[ok], K[ok], P[ok], seeds[ok], step, rows=np.flatnonzero(ok))
+
+
+BIG_LENS = st.lists(st.integers(0, 5000), min_size=2, max_size=8)
+
+
+@pytest.mark.gpu
+@settings(max_examples=6, **SET)
+@given(seed=st.integers(0, 2 ** 20), p=st.sampled_from([16, 32]), D=st.sampled_from([64, 128]),
+       G=st.sampled_from([1, 2, 4, 7, 8, 12, 16]), Hkv=st.sampled_from([1, 2, 4]), L=BIG_LENS,
+       parts=st.sampled_from([0, 0, 1, 2, 5, 16]), causal=st.booleans(),
+       frac=st.lists(st.sampled_from([0.0, 0.02, 0.3, 1.0]), min_size=8, max_size=8))
+def test_gpu_large_random_geometry(seed, p, D, G, Hkv, L, parts, causal, frac):
+    """Lengths up to 5000 (tens of KV stages and work units per sequence, ragged across the batch), every group
+    size and both head dims: decode on all rows, prefill (tcgen05 kernel) on sampled rows of every sequence."""
+    from tests.gpu_util import DeviceBatch, f64_of
+    geo = (p, D, G, Hkv)
+    what = "large %s %s" % (geo, L)
+    # decode
+    b = decode_batch(seed, geo, L)
+    if b.total_q:
+        k, v = compact_pool_after_append(b)
+        want, want_lse = oracle.paged_decode(decode_q(b), k, v, b.compact_block_table, b.seq_lens, b.scale)
+        db = DeviceBatch(b)
+        db.append()
+        out, lse = db.decode(num_partitions=parts)
+        check_parity(f64_of(out), want, "decode " + what)
+        got_lse = f64_of(lse)
+        fin = np.isfinite(want_lse)
+        assert np.array_equal(np.isneginf(got_lse), np.isneginf(want_lse))
+        assert np.abs(got_lse[fin] - want_lse[fin]).max(initial=0.0) < 2e-3
+    # prefill
+    b = prefill_batch(seed + 1, geo, L, frac)
+    if b.total_q:
+        k, v = compact_pool_after_append(b)
+        rng = np.random.default_rng(seed)
+        rows = np.unique(np.concatenate([rng.integers(0, b.total_q, 48), b.cu_seqlens_q[:-1][b.q_lens > 0],
+                                         (b.cu_seqlens_q[1:] - 1)[b.q_lens > 0]]))
+        want, want_lse = oracle.paged_prefill(b.q, b.cu_seqlens_q, k, v, b.compact_block_table, b.seq_lens, b.scale,
+                                              causal=causal, rows=rows)
+        db = DeviceBatch(b)
+        db.append()
+        out, lse = db.prefill(causal=causal)
+        check_parity(f64_of(out)[rows], want, "prefill " + what)
+        assert np.abs(f64_of(lse)[rows] - want_lse).max(initial=0.0) < 2e-3
