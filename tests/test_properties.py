@@ -256,3 +256,70 @@ def test_gpu_large_random_geometry(seed, p, D, G, Hkv, L, parts, causal, frac):
         out, lse = db.prefill(causal=causal)
         check_parity(f64_of(out)[rows], want, "prefill " + what)
         assert np.abs(f64_of(lse)[rows] - want_lse).max(initial=0.0) < 2e-3
+
+
+@pytest.mark.gpu
+@settings(max_examples=5, **SET)
+@given(seed=st.integers(0, 2 ** 20), p=st.sampled_from([16, 32]), G=st.sampled_from([1, 4, 7, 8, 12, 16]),
+       Hkv=st.sampled_from([1, 2, 4]), L=st.lists(st.integers(0, 3000), min_size=2, max_size=7),
+       long_one=st.sampled_from([0, 0, 8300, 12000]), parts=st.sampled_from([0, 0, 1, 3, 16]), causal=st.booleans(),
+       frac=st.lists(st.sampled_from([0.0, 0.02, 0.3, 1.0]), min_size=8, max_size=8))
+def test_gpu_fp8_large_random_geometry(seed, p, G, Hkv, L, long_one, parts, causal, frac):
+    """The quantised pool on long ragged batches: a sequence past 8192 tokens selects the 12-warp decode kernel
+    (G <= 8); decode on all rows, the fp8 prefill on sampled rows."""
+    from oracle import fp8 as ofp8
+    from tests.gpu_util import DeviceBatchFp8, f64_of
+    from tests.test_gpu_fp8 import oracle_pool
+    geo = (p, 128, G, Hkv)
+    L = list(L) + ([long_one] if long_one else [])
+    what = "fp8 large %s %s" % (geo, L)
+    b = decode_batch(seed, geo, L)
+    if b.total_q:
+        ks, vs = W.fp8_page_scales(seed % 89, b.num_pages, b.num_kv_heads)
+        db = DeviceBatchFp8(b, ks, vs)
+        db.quantise_store()
+        db.append()
+        k8, v8, cks, cvs = oracle_pool(b, ks, vs)
+        want, want_lse = ofp8.paged_decode_fp8(decode_q(b), k8, v8, cks, cvs, b.compact_block_table, b.seq_lens, b.scale)
+        out, lse = db.decode(num_partitions=parts)
+        check_parity(f64_of(out), want, "decode " + what)
+        fin = np.isfinite(want_lse)
+        assert np.abs(f64_of(lse)[fin] - want_lse[fin]).max(initial=0.0) < 2e-3
+        del db
+    Ls = [min(l, 3000) for l in L]
+    b = prefill_batch(seed + 1, geo, Ls, frac)
+    if b.total_q:
+        ks, vs = W.fp8_page_scales(seed % 83, b.num_pages, b.num_kv_heads)
+        db = DeviceBatchFp8(b, ks, vs)
+        db.quantise_store()
+        db.append()
+        k8, v8, cks, cvs = oracle_pool(b, ks, vs)
+        rng = np.random.default_rng(seed)
+        rows = np.unique(np.concatenate([rng.integers(0, b.total_q, 32), b.cu_seqlens_q[:-1][b.q_lens > 0],
+                                         (b.cu_seqlens_q[1:] - 1)[b.q_lens > 0]]))
+        want, _ = ofp8.paged_prefill_fp8(b.q, b.cu_seqlens_q, k8, v8, cks, cvs, b.compact_block_table, b.seq_lens,
+                                         b.scale, causal=causal, rows=rows)
+        out, _ = db.prefill(causal=causal)
+        check_parity(f64_of(out)[rows], want, "prefill " + what)
+
+
+@pytest.mark.gpu
+@settings(max_examples=6, **SET)
+@given(seed=st.integers(0, 2 ** 20), p=st.sampled_from([16, 32]), D=st.sampled_from([64, 128]),
+       G=st.sampled_from([1, 4, 7, 8, 12]), B=st.sampled_from([2, 3, 4]),
+       shared=st.lists(st.integers(0, 200), min_size=1, max_size=5),
+       sfx=st.lists(st.integers(1, 700), min_size=20, max_size=20))
+def test_gpu_cascade_large_random_geometry(seed, p, D, G, B, shared, sfx):
+    """Cascade decode with shared contexts up to 200 pages and private suffixes up to 700 tokens, 2 to 4 branches."""
+    from tests.gpu_util import DeviceBatch, f64_of
+    from tests.test_gpu_cascade import cfg_batch
+    shared_r = [s * p for s in shared]
+    sf = [[sfx[(r * B + j) % 20] for j in range(B)] for r in range(len(shared_r))]
+    b = cfg_batch(seed, shared_r, sf, B, G * 2, 2, D, p)
+    k, v = compact_pool_after_append(b)
+    want, want_lse = oracle.paged_decode(decode_q(b), k, v, b.compact_block_table, b.seq_lens, b.scale)
+    db = DeviceBatch(b)
+    db.append()
+    out, lse = db.decode_cascade(B, shared_r)
+    check_parity(f64_of(out), want, "cascade large p=%d D=%d G=%d B=%d" % (p, D, G, B))
+    assert np.abs(f64_of(lse) - want_lse).max() < 2e-3
