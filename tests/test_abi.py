@@ -77,3 +77,19 @@ def test_missing_library_fails_loudly(monkeypatch, tmp_path):
     monkeypatch.setattr(binding, "LIB_PATH", str(tmp_path / "nope.so"))
     with pytest.raises(binding.MstarError, match="no CPU fallback"):
         binding.load_library()
+
+
+def test_header_compiles_as_plain_c(tmp_path):
+    """include/mstar_attn.h is a C header (extern "C" guards, no C++ types): gcc -std=c99 -pedantic takes it."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        import pytest
+        pytest.skip("no gcc")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    src = tmp_path / "h.c"
+    src.write_text('#include "mstar_attn.h"\nint main(void) { return (int)(MSTAR_DECODE_STATIC_WORKSPACE_BYTES >> 30); }\n')
+    r = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(root, "include"),
+                        "-c", str(src), "-o", str(tmp_path / "h.o")], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
