@@ -323,3 +323,33 @@ def test_gpu_cascade_large_random_geometry(seed, p, D, G, B, shared, sfx):
     out, lse = db.decode_cascade(B, shared_r)
     check_parity(f64_of(out), want, "cascade large p=%d D=%d G=%d B=%d" % (p, D, G, B))
     assert np.abs(f64_of(lse) - want_lse).max() < 2e-3
+
+
+@pytest.mark.gpu
+@settings(max_examples=8, **SET)
+@given(seed=st.integers(0, 2 ** 20), kind=st.sampled_from(list(W.ADVERSARIAL_KINDS)), p=st.sampled_from([16, 32]),
+       D=st.sampled_from([64, 128]), G=st.sampled_from([1, 4, 7, 8, 16]),
+       L=st.lists(st.integers(1, 1500), min_size=1, max_size=5), parts=st.sampled_from([0, 1, 3, 16]),
+       causal=st.booleans(), frac=st.lists(st.sampled_from([0.02, 0.3, 1.0]), min_size=5, max_size=5))
+def test_gpu_adversarial_values_random_geometry(seed, kind, p, D, G, L, parts, causal, frac):
+    """The adversarial value patterns (dominant keys, the ramp that forces the lazy rescale, huge logits, zero
+    queries, constant keys) on random geometries: decode and both prefill kernels against the oracle."""
+    from tests.gpu_util import DeviceBatch, f64_of
+    geo = (p, D, G, 2)
+    what = "%s %s %s" % (kind, geo, L)
+    b = W.make_adversarial(decode_batch(seed, geo, L), kind, stage=64, seed=seed)
+    k, v = compact_pool_after_append(b)
+    want, want_lse = oracle.paged_decode(decode_q(b), k, v, b.compact_block_table, b.seq_lens, b.scale)
+    db = DeviceBatch(b)
+    db.append()
+    out, lse = db.decode(num_partitions=parts)
+    check_parity(f64_of(out), want, "decode " + what)
+    assert np.abs(f64_of(lse) - want_lse).max(initial=0.0) < 2e-3
+    b = W.make_adversarial(prefill_batch(seed + 1, geo, L, frac), kind, stage=128, seed=seed)
+    k, v = compact_pool_after_append(b)
+    want, _ = oracle.paged_prefill(b.q, b.cu_seqlens_q, k, v, b.compact_block_table, b.seq_lens, b.scale, causal=causal)
+    db = DeviceBatch(b)
+    db.append()
+    for mma_sync in (False, True):
+        out, _ = db.prefill(causal=causal, mma_sync=mma_sync)
+        check_parity(f64_of(out), want, "prefill %s mma_sync=%d" % (what, mma_sync))
