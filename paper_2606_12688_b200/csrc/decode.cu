@@ -32,6 +32,7 @@ static int decode_pick_warps(bool fp8, int G, int max_seq_len) {
     return fp8 ? ((G <= 8 && max_seq_len > 8192) ? 12 : 8) : 4;
 }
 constexpr int kMaxStages = 16;
+constexpr int kItemCostBf16 = 2, kItemCostFp8 = 2;  // start-up of a stream in tiles (balanced mode; measured)
 constexpr int kBf16Stages = 4;  // ring depth of the bf16 kernels (launch_decode)
 constexpr int kMaxDecodeGrid = 1024;  // split-K CTAs (one per SM); sizes the cut-record area of the workspace
 
@@ -61,6 +62,8 @@ struct DecodeParams {
     // one stream by nparts.
     int32_t balanced;
     int32_t per_min;
+    int32_t item_cost;  // balanced mode: the start-up of a stream (Q load, first page ids, merge, partial write) counted
+                        // in tiles when the CTA ranges are cut: a stream of nt tiles costs nt + item_cost
     int4* cut;  // [gridDim.x] per CTA: {s, kvh, pieces, 0} of the cut stream that BEGINS in its range, s = -1 if none
     // quantised pool (FP8 instantiations): value = e4m3(code) * scale[page][kv head]
     const float* k_scale;
@@ -241,7 +244,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         auto scan_round = [&](int s0, int len) {
             const int s = s0 + lane;
             if (s < p.V) lens[s] = len;
-            const int n = (len + p.chunk - 1) / p.chunk;
+            // fixed partitions: partitions of the sequence; balanced: its cost per kv head, tiles + start-up
+            const int n = (len + p.chunk - 1) / p.chunk + ((p.balanced && len > 0) ? p.item_cost : 0);
             int incl = n;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -331,42 +335,49 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
             }
         };
         if (p.balanced) {
-            // cum[] holds tiles per sequence (chunk == TOK); flat tile id = cum[s]*Hkv + kvh*nt_s + tile
+            // cum[] holds the COST of a sequence per kv head: nc = tiles + item_cost (chunk == TOK).  The streams
+            // (sequence, kv head) lie end to end on the cost axis, a stream at [cum[s]*Hkv + kvh*nc, + nc): first its
+            // start-up slot of item_cost units, then one unit per tile.  CTA b owns the tiles whose cost position lies
+            // in [b*per, (b+1)*per): equal cost, not equal tile counts -- a CTA whose range holds many short streams
+            // gets fewer tiles.
+            const int K = p.item_cost;
             const int64_t N = (int64_t)carry * p.Hkv;
             int64_t per = (N + gridDim.x - 1) / gridDim.x;
             if (per < p.per_min) per = p.per_min;
-            const int64_t fa = (int64_t)blockIdx.x * per;
-            const int64_t fb = (fa + per < N) ? fa + per : N;
+            const int64_t ca = (int64_t)blockIdx.x * per;
+            const int64_t cb = (ca + per < N) ? ca + per : N;
             bool cut_here = false;  // a stream begins in this range and continues past its end
-            if (fa < N) {
-                int lo = 0, hi = p.V;  // cum[lo]*Hkv <= fa < cum[hi]*Hkv
+            if (ca < N) {
+                int lo = 0, hi = p.V;  // cum[lo]*Hkv <= ca < cum[hi]*Hkv
                 while (hi - lo > 1) {
                     const int mid = (lo + hi) >> 1;
-                    if ((int64_t)cum[mid] * p.Hkv <= fa) lo = mid; else hi = mid;
+                    if ((int64_t)cum[mid] * p.Hkv <= ca) lo = mid; else hi = mid;
                 }
                 int s = lo;
-                int64_t f = fa;
-                while (f < fb) {
-                    const int nt = cum[s + 1] - cum[s];
+                int64_t c = ca;
+                while (c < cb) {
+                    const int nc = cum[s + 1] - cum[s], nt = nc - K;
                     const int64_t F0 = (int64_t)cum[s] * p.Hkv;
-                    const int kvh = (int)((f - F0) / nt);
-                    const int tile = (int)((f - F0) - (int64_t)kvh * nt);
-                    const int64_t fs = F0 + (int64_t)kvh * nt;  // flat start of this stream
-                    const int ntl = (int)(((int64_t)(nt - tile) < fb - f) ? (nt - tile) : (fb - f));
-                    const int piece = (int)((int64_t)blockIdx.x - fs / per);
+                    const int kvh = (int)((c - F0) / nc);
+                    const int r = (int)((c - F0) - (int64_t)kvh * nc);
+                    const int64_t cs = F0 + (int64_t)kvh * nc + K;  // cost position of the stream's first tile
+                    const int tile = r > K ? r - K : 0;
+                    const int64_t ct = cs + tile;                   // cost position of this tile (>= c)
+                    if (ct >= cb) break;  // the range ends inside the start-up slot: the tiles belong to the next CTA
+                    const int ntl = (int)(((int64_t)(nt - tile) < cb - ct) ? (nt - tile) : (cb - ct));
+                    const int piece = (int)((int64_t)blockIdx.x - cs / per);
+                    const int pieces = (int)((cs + nt - 1) / per - cs / per) + 1;
                     const int whole = (tile == 0 && ntl == nt) ? 1 : 0;
                     if (p.casc_B) {  // every stream leaves partials: the CTA with its first tile records the count
-                        if (tile == 0 && lane == 0 && !op_isv)
-                            p.vpieces[(size_t)s * p.Hkv + kvh] = (int)((fs + nt - 1) / per - fs / per) + 1;
+                        if (tile == 0 && lane == 0 && !op_isv) p.vpieces[(size_t)s * p.Hkv + kvh] = pieces;
                     } else if (tile == 0 && !whole) {
                         cut_here = true;
-                        if (lane == 0 && !op_isv)
-                            p.cut[blockIdx.x] = make_int4(s, kvh, (int)((fs + nt - 1) / per - fs / per) + 1, 0);
+                        if (lane == 0 && !op_isv) p.cut[blockIdx.x] = make_int4(s, kvh, pieces, 0);
                     }
                     const int L = lens[s];
                     const int tok0 = tile * TOK;
                     emit_item(s, kvh, piece, tok0, min(L - tok0, ntl * TOK), whole);
-                    f += ntl;
+                    c = ct + ntl;
                     if (tile + ntl == nt && kvh == p.Hkv - 1) {
                         ++s;
                         while (s < p.V && cum[s + 1] == cum[s]) ++s;  // sequences without tokens
@@ -1123,6 +1134,7 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, in
     partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, tok, &p.chunk, &p.nparts);
     if (num_partitions == 0)
         p.balanced = balanced_plan(max_seq_len > 0 ? max_seq_len : 1, tok, &p.nparts, &p.per_min) ? 1 : 0;
+    p.item_cost = p.balanced ? (fp8 ? kItemCostFp8 : kItemCostBf16) : 0;
     p.direct = (p.nparts == 1) && !casc;
     p.slots = p.nparts;
     p.V = num_seqs;
