@@ -132,7 +132,7 @@ int mstar_kv_gather(void* k_out, void* v_out, const mstar_kv_pool* pool, const i
  *                  [i*c, (i+1)*c) with c = ceil(max_seq_len/P) rounded up to a multiple of 64; partitions
  *                  past a sequence's end are empty; 1 = no combine pass.  0 = balanced: the 64-token
  *                  tiles of all (sequence, kv head) streams are laid end to end and every CTA takes an
- *                  equal contiguous range, so ragged batches finish together; a stream that lies inside
+ *                  contiguous range of equal cost (tiles + 2 per stream), so ragged batches finish together; a stream that lies inside
  *                  one range is finished by its CTA, a stream cut by range boundaries (at most one per
  *                  CTA) is merged by the combine pass (the cut points depend on seq_lens and the SM
  *                  count only, never on page ids).
@@ -265,7 +265,7 @@ int mstar_paged_attn_decode_static(void* out, float* lse_out, const void* q, con
  *                  undefined).  0 = nothing shared.
  * One call = one split-K launch over prefix streams (the kernel's Q load fetches the rows of every branch, q stays
  * in its natural [S][Hq][D] layout) and suffix streams, laid end to end in 64-token tiles and cut
- * into equal CTA ranges as in the balanced mode of mstar_paged_attn_decode, plus one combine launch that merges the
+ * into CTA ranges of equal cost as in the balanced mode of mstar_paged_attn_decode, plus one combine launch that merges the
  * prefix and suffix pieces of every (sequence, head) row by log-sum-exp.  Deterministic, CUDA-graph capturable.
  * bf16 pool only.  Other arguments, flags and errors as mstar_paged_attn_decode (num_partitions is always 0).
  */

@@ -55,7 +55,7 @@ struct DecodeParams {
     int32_t direct;  // nparts == 1: write the final output, no combine pass
     int32_t nstages;
     // balanced mode (num_partitions = 0): the (sequence, kv head) streams are laid end to end in 64-token tiles and
-    // every CTA takes an equal, contiguous range of them.  A stream that lies inside one range is finished by its CTA
+    // every CTA takes a contiguous range of them, equal in cost (item_cost below).  A stream that lies inside one range is finished by its CTA
     // (final output, no partial); a stream cut by range boundaries yields one partial per piece, and the CTA that
     // holds its first piece records it in cut[] for the combine pass -- at most one record per CTA, since only the
     // last stream of a range can continue into the next.  chunk == decode_tok then; per_min bounds the pieces of
