@@ -138,7 +138,10 @@ int mstar_kv_gather(void* k_out, void* v_out, const mstar_kv_pool* pool, const i
  *                  count only, never on page ids).
  *   workspace      device, >= mstar_paged_attn_decode_workspace_bytes(...) bytes, 16-B aligned
  *   scale          must be positive and finite (MSTAR_ERR_INVALID_ARG otherwise)
- * Requires Hq % Hkv == 0 and Hq/Hkv <= 16 (MSTAR_ERR_UNSUPPORTED otherwise), and num_seqs <= 16384
+ * Requires Hq % Hkv == 0.  Hq/Hkv <= 16 heads share one pass over a kv head's K/V; a larger group is processed as d
+ * sub-groups of Hq/Hkv/d <= 16 heads, d the smallest such divisor (32 = 2 x 16, 24 = 2 x 12, 17 = 17 x 1), each a
+ * stream of its own over the same K/V, whose repeated reads are L2 hits (cascade calls: MSTAR_ERR_UNSUPPORTED above
+ * 16).  num_seqs <= 16384
  * (MSTAR_ERR_UNSUPPORTED: the per-sequence work-list prefix sums live in shared memory).
  */
 size_t mstar_paged_attn_decode_workspace_bytes(int32_t num_seqs, int32_t num_q_heads, int32_t head_dim,

@@ -41,7 +41,9 @@ struct DecodeParams {
     const int32_t* block_table;
     int64_t bt_stride;
     const int32_t* seq_lens;
-    int32_t S, Hq, Hkv, G;
+    int32_t S, Hq, Hkv, G;  // Hkv, G: VIRTUAL kv heads and heads per virtual kv head (kv_div below)
+    int32_t kv_div;          // Hq/Hkv > 16: a kv head's group is split into kv_div sub-groups of G <= 16 heads, each
+                             // its own stream over the same K/V (virtual kv head v reads real kv head v / kv_div)
     int32_t chunk;   // tokens per partition, multiple of the stage size (decode_tok)
     int32_t nparts;  // partition slots per (sequence, head) in the workspace (per set: a cascade row has two sets)
     int32_t slots;   // partial slots of a row = its stride in part_O / part_m / part_l (nparts; cascade 2 nparts)
@@ -279,6 +281,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
         // hand one work item to the consumers and stream its K/V tiles into the ring
         auto emit_item = [&](int s, int kvh, int part, int tok0, int ntok, int whole) {
             const int ntiles = (ntok + TOK - 1) / TOK;
+            const int kvh_r = kvh / p.kv_div;  // the pool's kv head
             int nb = 1;
             if (p.casc_B) {  // s is a virtual sequence: translate to (first real sequence, branches, token offset)
                 whole = 0;
@@ -320,7 +323,8 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                     if (lane < OPS && op_page < npg1) pg_next = __ldg(bt + (t + 1) * PPS + op_page);
                 }
                 float pg_scale = 0.f;  // FP8: requested before the ring wait, which hides its latency
-                if (FP8 && pg >= 0) pg_scale = __ldg((op_isv ? p.v_scale : p.k_scale) + (size_t)pg * p.Hkv + kvh);
+                if (FP8 && pg >= 0)
+                    pg_scale = __ldg((op_isv ? p.v_scale : p.k_scale) + (size_t)pg * (p.Hkv / p.kv_div) + kvh_r);
                 mbar_wait(empty_bar(st), ph ^ 1);
                 if (FP8) {
                     if (pg >= 0) sc_ring[(st * 2 + op_isv) * 16 + op_page] = pg_scale;
@@ -330,7 +334,7 @@ decode_splitk_kernel(const __grid_constant__ CUtensorMap kmap, const __grid_cons
                 __syncwarp();
                 if (pg >= 0)
                     tma_load_4d(ring + st * SM::kStageBytes + op_off, op_isv ? &vmap : &kmap, full_bar(st),
-                                op_half * 64, 0, kvh, pg, pol);
+                                op_half * 64, 0, kvh_r, pg, pol);
                 if (++st == nstages) { st = 0; ph ^= 1; }
             }
         };
@@ -1121,8 +1125,20 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, in
     if (!aligned(out, 16) || !aligned(q, 16) || !aligned(block_table, 4) || !aligned(seq_lens, 4))
         return MSTAR_ERR_INVALID_ARG;
     if (num_q_heads % pool->num_kv_heads) return MSTAR_ERR_INVALID_ARG;
-    const int G = num_q_heads / pool->num_kv_heads;
-    if (G > 16) return MSTAR_ERR_UNSUPPORTED;
+    // more than 16 heads per kv head: kv_div sub-groups of G <= 16 heads, each a stream of its own over the same K/V
+    // (the repeats are L2 hits: the sub-groups' streams are neighbours in the work list)
+    const int Greal = num_q_heads / pool->num_kv_heads;
+    int kv_div = 1;
+    if (Greal > 16) {
+        for (int d = 2; d <= Greal; ++d)
+            if (Greal % d == 0 && Greal / d <= 16) {
+                kv_div = d;
+                break;
+            }
+        if (kv_div == 1 || n_branches > 0) return MSTAR_ERR_UNSUPPORTED;  // a prime group size; cascade calls
+    }
+    const int G = Greal / kv_div;
+    const int Hkv_v = pool->num_kv_heads * kv_div;
     if (num_seqs > 16384) return MSTAR_ERR_UNSUPPORTED;
     const bool casc = n_branches > 0;
     if (casc && (!shared_lens || !aligned(shared_lens, 4) || num_seqs % n_branches)) return MSTAR_ERR_INVALID_ARG;
@@ -1131,7 +1147,8 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, in
     DecodeParams p{};
     const int nw = decode_pick_warps(fp8, G, max_seq_len);
     const int32_t tok = decode_tok(nw);
-    partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, tok, &p.chunk, &p.nparts);
+    partition_plan(num_seqs, pool->num_kv_heads, max_seq_len, num_partitions, tok, &p.chunk, &p.nparts);  // as the
+    // workspace query does (mstar_paged_attn_decode_auto_partitions takes the pool's kv heads)
     if (num_partitions == 0)
         p.balanced = balanced_plan(max_seq_len > 0 ? max_seq_len : 1, tok, &p.nparts, &p.per_min) ? 1 : 0;
     p.item_cost = p.balanced ? (fp8 ? kItemCostFp8 : kItemCostBf16) : 0;
@@ -1174,7 +1191,8 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, in
     p.seq_lens = seq_lens;
     p.S = num_seqs;
     p.Hq = num_q_heads;
-    p.Hkv = pool->num_kv_heads;
+    p.Hkv = Hkv_v;
+    p.kv_div = kv_div;
     p.G = G;
     p.scale_log2 = scale * 1.4426950408889634f;
     p.out = out;
@@ -1187,7 +1205,7 @@ static int decode_entry(bool fp8, const float* k_scale, const float* v_scale, in
     rc = fp8 ? get_pool_maps_fp8(pool, &maps) : get_pool_maps(pool, &maps);
     if (rc != MSTAR_OK) return rc;
 
-    const int64_t max_items64 = (int64_t)p.V * p.nparts * pool->num_kv_heads;
+    const int64_t max_items64 = (int64_t)p.V * p.nparts * Hkv_v;
     const int max_items = max_items64 > (1 << 30) ? (1 << 30) : (int)max_items64;
     cudaStream_t st = (cudaStream_t)stream;
     const bool g16 = G > 8;

@@ -390,3 +390,9 @@ def test_prefill_fp8_config3_full_size_sampled_rows_every_sequence():
     rng = np.random.default_rng(11)
     rows = np.unique(np.concatenate([rng.integers(0, b.total_q, 48), b.cu_seqlens_q[:-1], b.cu_seqlens_q[1:] - 1]))
     print("fp8 prefill config 3", run_prefill_case(b, causal=True, rows=rows, check_f32=False))
+
+
+def test_decode_fp8_more_than_16_heads_per_kv_head():
+    """Hq / Hkv = 32 on the quantised pool: two sub-groups of 16 heads over the same codes and scales."""
+    b = small_batch(390, [1, 65, 700, 0, 129, 2300], Hq=32, Hkv=1, p=16)
+    run_case(b, parts_list=(0, 1, 3))

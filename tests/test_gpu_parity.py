@@ -471,3 +471,33 @@ def test_error_codes():
                                 0.125, num_partitions=1)
     with pytest.raises(mstar.MstarError, match="INVALID_ARG"):   # non-positive scale
         mstar.paged_attn_decode(out, db.q_decode, db.pool, db.block_table, db.seq_lens, 33, 0.0, num_partitions=1)
+
+
+@pytest.mark.parametrize("Hq,Hkv,D,p", [(32, 1, 128, 16), (48, 2, 64, 32), (40, 2, 128, 32), (64, 1, 128, 16)])
+def test_decode_more_than_16_heads_per_kv_head(Hq, Hkv, D, p):
+    """Hq / Hkv = 32, 24, 20, 64: the group is split into sub-groups of at most 16 heads (2 x 16, 2 x 12, 2 x 10, 4 x 16), each a
+    stream of its own over the same K/V; every partition mode."""
+    b = small_batch(470 + Hq, [1, 65, 700, 0, 129, 2300, 64], Hq=Hq, Hkv=Hkv, D=D, p=p)
+    db = DeviceBatch(b)
+    db.append()
+    k, v = compact_pool_after_append(b)
+    want, want_lse = oracle.paged_decode(decode_q(b), k, v, b.compact_block_table, b.seq_lens, b.scale)
+    for parts in (0, 1, 3, 16):
+        out, lse = db.decode(num_partitions=parts)
+        check_parity(f64_of(out), want, "G=%d parts=%d" % (Hq // Hkv, parts))
+        got = f64_of(lse)
+        fin = np.isfinite(want_lse)
+        assert np.array_equal(np.isneginf(got), np.isneginf(want_lse))
+        assert np.abs(got[fin] - want_lse[fin]).max(initial=0.0) < 2e-3
+
+
+def test_decode_prime_group_size_above_16():
+    """Hq / Hkv = 17 has no divisor that leaves sub-groups of 2 .. 16 heads: every head becomes a stream of its own."""
+    b = small_batch(480, [40, 3, 300], Hq=17, Hkv=1, D=128, p=16)
+    db = DeviceBatch(b)
+    db.append()
+    k, v = compact_pool_after_append(b)
+    want, _ = oracle.paged_decode(decode_q(b), k, v, b.compact_block_table, b.seq_lens, b.scale)
+    for parts in (0, 2):
+        out, _ = db.decode(num_partitions=parts)
+        check_parity(f64_of(out), want, "G=17 parts=%d" % parts)
