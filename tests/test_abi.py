@@ -65,8 +65,10 @@ def test_host_validation_without_gpu(lib):
                                        0x80, None, 0, None) == -1                     # unknown flag bit
     assert lib.mstar_paged_attn_decode(0x100, None, 0x100, ctypes.byref(ok), 0x100, 4, 0x100, 2, 3, 64, 0.1, 1,
                                        0, None, 0, None) == -1                        # Hq % Hkv != 0
-    assert lib.mstar_paged_attn_decode(0x100, None, 0x100, ctypes.byref(ok), 0x100, 4, 0x100, 2, 68, 64, 0.1, 1,
-                                       0, None, 0, None) == -2                        # G = 34 > 16
+    assert lib.mstar_paged_attn_decode(0x100, None, 0x100, ctypes.byref(ok), 0x100, 4, 0x100, 20000, 4, 64, 0.1, 1,
+                                       0, None, 0, None) == -2                        # num_seqs > 16384
+    assert lib.mstar_paged_attn_decode_cascade(0x100, None, 0x100, ctypes.byref(ok), 0x100, 4, 0x100, 0x100, 4, 2,
+                                               68, 64, 0.1, 0, 0x100, 1 << 20, None) == -2   # cascade, G = 34 > 16
     assert lib.mstar_paged_attn_decode(0x100, None, 0x100, ctypes.byref(ok), 0x100, 4, 0x100, 2, 4, 4096, 0.1, 8,
                                        0, None, 0, None) == -1                        # partitions but no workspace
 
